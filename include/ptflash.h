@@ -1,0 +1,157 @@
+/* ptflash.h -- C ABI of libptflash: batched isothermal two-phase (vapour-liquid) flash of N independent
+ * mixtures at given (P, T, z) under the Soave-Redlich-Kwong equation of state, on one NVIDIA B200 (sm_100a).
+ *
+ * The operation is the one PTFlash (arXiv 2205.03090) defines in section 2.1: for every
+ * mixture decide "single phase" or "two phases"; in the latter case return the vapour mole fraction
+ * beta (= theta_V), the liquid composition x and the vapour composition y satisfying the mass balance
+ * (1a), (1b) and the iso-fugacity condition (2).  The method is the paper's (section 2.2, Fig. 2,
+ * PAPER.md:51-111; App. A-C): Wilson K-values (eq. 6) -> 3 successive-substitution
+ * probes -> Michelsen's two-sided tangent-plane stability test (eq. 3-5, SS then trust-region Newton,
+ * App. B.1) -> Rachford-Rice (eq. 7, App. C) + successive substitution + trust-region Newton on the
+ * Gibbs energy (eq. 8, App. B.2).  Every iteration rebuilds the SRK mixture parameters (A.2), solves the
+ * cubic (A.3) choosing the root of minimum Gibbs energy, and evaluates ln-fugacity coefficients (A.6).
+ * Every step runs in hand-written fp64 CUDA kernels; there is no CPU fallback.
+ *
+ * Layout: all per-mixture arrays are structure-of-arrays, fp64, component-major: element (i, n) of z, x,
+ * y, lnK lives at [i * N + n] (i = component 0..nc-1, n = mixture 0..N-1).  P, T, beta, phase, ... are [N].
+ * Units: T and Tc in K; P in the same unit as Pc (bar in the benchmark configs); the gas constant cancels.
+ *
+ * Threading: a handle may be used by one thread at a time; calls on one handle are serialised on the
+ * stream given.  Use one handle per stream for concurrency.
+ */
+#ifndef PTFLASH_H
+#define PTFLASH_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ptflash_handle_s* ptflash_handle_t;
+
+#define PTFLASH_OK 0
+#define PTFLASH_EINVAL (-1) /* null handle / null required pointer / N < 0 / unknown option */
+#define PTFLASH_ECUDA (-2)  /* CUDA allocation, copy or launch failure; text in ptflash_last_error() */
+
+#define PTFLASH_MAX_NC 16
+
+/* out_phase values */
+#define PTFLASH_PHASE_INVALID (-1) /* non-finite input, P <= 0, T <= 0, z_i < 0 or |sum z - 1| > 1e-9: beta, x, y = NaN */
+#define PTFLASH_PHASE_SINGLE 1
+#define PTFLASH_PHASE_TWO 2
+
+/* out_status bits (per mixture; problems are data, never call failures -- cf. Alg. 1 PAPER.md:550-552,
+ * which returns the indices of unconverged samples) */
+#define PTFLASH_ST_STAB_CAP 1      /* a stability trial hit its iteration cap */
+#define PTFLASH_ST_SPLIT_CAP 2     /* the phase split hit its iteration cap */
+#define PTFLASH_ST_BAND 4          /* 0 < |tpd_min| < band (1e-9): label decided inside the near-zero TPD band */
+#define PTFLASH_ST_SPLIT_FAILED 8  /* "unstable" verdict but the split ended trivial or with beta outside (0,1): reported as single phase */
+#define PTFLASH_ST_LNK0_REJECTED 32 /* caller-supplied lnK0 non-finite or |lnK0| > 700: Wilson used instead */
+
+/* flags[n] bits for ptflash_flash_ex (interface effect of the paper's classifier/initializer, section 4.3
+ * caller-supplied K estimates and a "known unstable" verdict) */
+#define PTFLASH_FLAG_SKIP_STABILITY 1 /* go straight to the phase split from lnK0 */
+#define PTFLASH_FLAG_USE_LNK0 2       /* use lnK0 instead of Wilson for the probe and the stability starts */
+
+/* ptflash_create: bind a component system to the current CUDA device.
+ *   nc      number of components, 2..PTFLASH_MAX_NC
+ *   Tc, Pc, omega   HOST arrays [nc]: critical temperature (K), critical pressure, acentric factor (Table 1)
+ *   kij     HOST array [nc*nc] row-major, symmetric, zero diagonal (A.2b PAPER.md:415); NULL = all zero
+ * Everything is copied; the caller keeps its arrays.  Returns NULL on failure (bad nc, null pointer,
+ * non-finite or non-positive Tc/Pc, asymmetric kij, CUDA error); reason in ptflash_last_error(). */
+ptflash_handle_t ptflash_create(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij);
+
+/* ptflash_flash: flash N mixtures.  All pointers are DEVICE pointers on the handle's device.
+ *   z [nc][N], P [N], T [N]          inputs (section 2.1); z is normalised once internally (z / sum z)
+ *   out_beta [N]                      two-phase: vapour fraction in (0,1); single phase: 1 if Z_feed > 1/3 else 0
+ *   out_x, out_y [nc][N]              two-phase: liquid / vapour mole fractions (each sums to 1); single phase: both = z
+ *   out_phase [N]                     number of phases: 1, 2, or -1 (invalid input)
+ *   out_iters [N] (may be NULL)       number of K-value updates performed (probe + split SS + split Newton)
+ *   stream                            cudaStream_t (NULL = legacy default stream)
+ * Asynchronous: enqueues work on `stream` and returns; outputs are valid once the stream reaches that point.
+ * The caller owns every buffer; inputs and outputs must not alias.  The handle owns a workspace that
+ * grows on first use (a growth synchronises the stream).  N == 0 is a no-op.  Returns PTFLASH_OK / EINVAL / ECUDA. */
+int ptflash_flash(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T,
+                  double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
+                  void* stream);
+
+/* Extended call: same nine arrays plus optional ones (NULL = absent). */
+typedef struct ptflash_io {
+  int64_t N;
+  const double* z;           /* [nc][N] */
+  const double* P;           /* [N] */
+  const double* T;           /* [N] */
+  const double* lnK0;        /* optional in  [nc][N]: initial ln K (warm start, BASELINE config 5) */
+  const uint8_t* flags;      /* optional in  [N]: PTFLASH_FLAG_* (ignored where lnK0 is NULL) */
+  double* out_beta;          /* [N] */
+  double* out_x;             /* [nc][N] */
+  double* out_y;             /* [nc][N] */
+  int32_t* out_phase;        /* [N] */
+  int32_t* out_iters;        /* optional out [N] */
+  double* out_tpd_min;       /* optional out [N]: minimum reduced TPD found (eq. 3; probe value for probe-proved mixtures; NaN when stability was skipped) */
+  double* out_lnK;           /* optional out [nc][N]: converged ln K (0 for single phase) */
+  int32_t* out_status;       /* optional out [N]: PTFLASH_ST_* bits */
+  int32_t* out_stab_iters;   /* optional out [N]: stability iterations (SS + Newton, both starts) */
+} ptflash_io_t;
+int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream);
+
+/* End-to-end variant with HOST buffers (same meaning and layout as ptflash_flash; pinned memory recommended):
+ * copies inputs host->device, runs the flash, copies results device->host on `stream`, then synchronises.
+ * Staging buffers belong to the handle. */
+int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T,
+                       double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
+                       void* stream);
+
+/* Synchronises the handle's last stream, frees constants and workspace.  NULL is a no-op. */
+int ptflash_destroy(ptflash_handle_t h);
+
+/* Options (tolerances and caps); defaults in brackets follow DESIGN.md section 3 / PAPER.md:79,90,97,105,558 */
+enum {
+  PTFLASH_OPT_TOL_SS = 0,          /* SS residual target, stability and split [1e-10] */
+  PTFLASH_OPT_TOL_NEWTON_G = 1,    /* Newton gradient target [1e-12] */
+  PTFLASH_OPT_TOL_NEWTON_STEP = 2, /* Newton step below which the full step is applied and iteration stops [1e-10] */
+  PTFLASH_OPT_PROBE_MARGIN = 3,    /* probe: "negative" means < -margin [1e-8] */
+  PTFLASH_OPT_TRIVIAL_TOL = 4,     /* trivial stability solution: max|lnW - lnz| < tol [1e-6] */
+  PTFLASH_OPT_BAND = 5,            /* near-zero TPD band [1e-9] */
+  PTFLASH_OPT_PROBE_ITERS = 6,     /* [3] */
+  PTFLASH_OPT_STAB_SS_ITERS = 7,   /* [9] */
+  PTFLASH_OPT_STAB_TR_ITERS = 8,   /* [60] */
+  PTFLASH_OPT_SPLIT_SS_ITERS = 9,  /* [9]: SS iterations before switching to Newton */
+  PTFLASH_OPT_SPLIT_TR_ITERS = 10, /* [60] */
+  PTFLASH_OPT_USE_NEWTON = 11,     /* [1]; 0 = pure successive substitution */
+  PTFLASH_OPT_SS_CAP = 12,         /* [100000]: SS cap when Newton is off or theta stays outside (0,1) */
+  PTFLASH_OPT_ENGINE = 13,         /* [1] 1 = staged persistent kernels with work queues; 0 = single run-to-completion kernel */
+  PTFLASH_NUM_OPTS = 14
+};
+int ptflash_set_option(ptflash_handle_t h, int key, double value);
+int ptflash_get_option(ptflash_handle_t h, int key, double* value);
+
+/* Counters of the last completed call, shaped like the paper's profiler (Table 4).
+ * Synchronises the handle's last stream. */
+typedef struct ptflash_stats {
+  int64_t n_total, n_invalid;
+  int64_t n_probe_case1, n_probe_case2, n_probe_case3; /* section 2.2.3 */
+  int64_t n_stability;      /* mixtures sent to the stability analysis */
+  int64_t n_stab_newton;    /* stability trials that needed the trust-region stage */
+  int64_t n_split;          /* mixtures sent to the phase split */
+  int64_t n_split_newton;   /* phase splits that needed the trust-region stage */
+  int64_t n_two_phase;
+  int64_t kernel_launches;  /* kernels launched by the last call */
+} ptflash_stats_t;
+int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out);
+
+/* FP64 roofline probe: runs an unrolled independent-DFMA kernel on every SM for `iters` iterations and returns
+ * the achieved FP64 FLOP/s (used by bench.py as the measured denominator of the ALU roofline). */
+int ptflash_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, void* stream);
+
+/* Text of the last error on the calling thread ("" if none). */
+const char* ptflash_last_error(void);
+
+/* Library version string, e.g. "ptflash-b200 0.1 (sm_100a)". */
+const char* ptflash_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PTFLASH_H */

@@ -1,0 +1,222 @@
+"""Thin Python binding of the libptflash C ABI (include/ptflash.h): argument marshalling only.
+
+Every numerical step runs in the CUDA kernels behind the ABI.  PyTorch is used for device memory and
+streams, nothing else.  There is NO fallback: if libptflash.so is missing or fails to load, every
+entry point raises (build it with `python -m paper_2205_03090_b200.build`).
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+_HERE = Path(__file__).resolve().parent
+_LIB_PATH = _HERE / "libptflash.so"
+_lib = None
+
+PTFLASH_OK, PTFLASH_EINVAL, PTFLASH_ECUDA = 0, -1, -2
+ST_STAB_CAP, ST_SPLIT_CAP, ST_BAND, ST_SPLIT_FAILED, ST_LNK0_REJECTED = 1, 2, 4, 8, 32
+FLAG_SKIP_STABILITY, FLAG_USE_LNK0 = 1, 2
+OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band", "probe_iters",
+           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine"]
+EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
+           "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_fp64_peak",
+           "ptflash_last_error", "ptflash_version"]
+
+
+class PTFlashError(RuntimeError):
+    pass
+
+
+class _Io(C.Structure):
+    _fields_ = [("N", C.c_int64), ("z", C.c_void_p), ("P", C.c_void_p), ("T", C.c_void_p), ("lnK0", C.c_void_p),
+                ("flags", C.c_void_p), ("out_beta", C.c_void_p), ("out_x", C.c_void_p), ("out_y", C.c_void_p),
+                ("out_phase", C.c_void_p), ("out_iters", C.c_void_p), ("out_tpd_min", C.c_void_p),
+                ("out_lnK", C.c_void_p), ("out_status", C.c_void_p), ("out_stab_iters", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("n_total", "n_invalid", "n_probe_case1", "n_probe_case2", "n_probe_case3",
+                                         "n_stability", "n_stab_newton", "n_split", "n_split_newton", "n_two_phase",
+                                         "kernel_launches")]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+def load_library():
+    """Load libptflash.so (once).  Raises PTFlashError if it is not built -- there is no CPU path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise PTFlashError(f"{_LIB_PATH} not found: the CUDA extension is not built "
+                           "(run `python -m paper_2205_03090_b200.build`); there is no CPU fallback")
+    L = C.CDLL(str(_LIB_PATH))
+    vp, dp, i64 = C.c_void_p, C.POINTER(C.c_double), C.c_int64
+    L.ptflash_create.restype = vp
+    L.ptflash_create.argtypes = [C.c_int, dp, dp, dp, dp]
+    L.ptflash_flash.restype = C.c_int
+    L.ptflash_flash.argtypes = [vp, i64] + [vp] * 9
+    L.ptflash_flash_ex.restype = C.c_int
+    L.ptflash_flash_ex.argtypes = [vp, C.POINTER(_Io), vp]
+    L.ptflash_flash_host.restype = C.c_int
+    L.ptflash_flash_host.argtypes = [vp, i64] + [vp] * 9
+    L.ptflash_destroy.restype = C.c_int
+    L.ptflash_destroy.argtypes = [vp]
+    L.ptflash_set_option.restype = C.c_int
+    L.ptflash_set_option.argtypes = [vp, C.c_int, C.c_double]
+    L.ptflash_get_option.restype = C.c_int
+    L.ptflash_get_option.argtypes = [vp, C.c_int, dp]
+    L.ptflash_get_stats.restype = C.c_int
+    L.ptflash_get_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.ptflash_fp64_peak.restype = C.c_int
+    L.ptflash_fp64_peak.argtypes = [C.c_int, dp, dp, vp]
+    L.ptflash_last_error.restype = C.c_char_p
+    L.ptflash_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != PTFLASH_OK:
+        raise PTFlashError(f"{what} failed ({rc}): {load_library().ptflash_last_error().decode()}")
+
+
+def _darr(a):
+    import numpy as np
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ptr(t):
+    """Device (or host) address of a torch tensor / numpy array; None -> NULL."""
+    if t is None:
+        return None
+    if hasattr(t, "data_ptr"):
+        assert t.is_contiguous()
+        return C.c_void_p(t.data_ptr())
+    return C.c_void_p(t.ctypes.data)
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+# ---- the ABI, same names ---------------------------------------------------------------------
+def ptflash_create(nc, Tc, Pc, omega, kij=None):
+    L = load_library()
+    _a, pTc = _darr(Tc)
+    _b, pPc = _darr(Pc)
+    _c, pom = _darr(omega)
+    _d, pk = _darr(kij) if kij is not None else (None, None)
+    h = L.ptflash_create(int(nc), pTc, pPc, pom, pk)
+    if not h:
+        raise PTFlashError("ptflash_create failed: " + L.ptflash_last_error().decode())
+    return C.c_void_p(h)
+
+
+def ptflash_flash(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=None, stream=None):
+    _check(load_library().ptflash_flash(h, int(N), _ptr(z), _ptr(P), _ptr(T), _ptr(out_beta), _ptr(out_x), _ptr(out_y),
+                                        _ptr(out_phase), _ptr(out_iters), _stream(stream)), "ptflash_flash")
+
+
+def ptflash_flash_ex(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=None, lnK0=None, flags=None,
+                     out_tpd_min=None, out_lnK=None, out_status=None, out_stab_iters=None, stream=None):
+    io = _Io(int(N), *[(_ptr(t).value if t is not None else None) for t in
+                       (z, P, T, lnK0, flags, out_beta, out_x, out_y, out_phase, out_iters, out_tpd_min, out_lnK,
+                        out_status, out_stab_iters)])
+    _check(load_library().ptflash_flash_ex(h, C.byref(io), _stream(stream)), "ptflash_flash_ex")
+
+
+def ptflash_flash_host(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=None, stream=None):
+    _check(load_library().ptflash_flash_host(h, int(N), _ptr(z), _ptr(P), _ptr(T), _ptr(out_beta), _ptr(out_x),
+                                             _ptr(out_y), _ptr(out_phase), _ptr(out_iters), _stream(stream)),
+           "ptflash_flash_host")
+
+
+def ptflash_destroy(h):
+    _check(load_library().ptflash_destroy(h), "ptflash_destroy")
+
+
+def ptflash_set_option(h, key, value):
+    k = OPTIONS.index(key) if isinstance(key, str) else int(key)
+    _check(load_library().ptflash_set_option(h, k, float(value)), "ptflash_set_option")
+
+
+def ptflash_get_option(h, key):
+    k = OPTIONS.index(key) if isinstance(key, str) else int(key)
+    v = C.c_double(0)
+    _check(load_library().ptflash_get_option(h, k, C.byref(v)), "ptflash_get_option")
+    return v.value
+
+
+def ptflash_get_stats(h) -> dict:
+    s = Stats()
+    _check(load_library().ptflash_get_stats(h, C.byref(s)), "ptflash_get_stats")
+    return s.as_dict()
+
+
+def ptflash_fp64_peak(iters=4096, stream=None):
+    """Measured FP64 FLOP/s of an independent-DFMA kernel on the current device -> (flops_per_s, ms)."""
+    f, ms = C.c_double(0), C.c_double(0)
+    _check(load_library().ptflash_fp64_peak(int(iters), C.byref(f), C.byref(ms), _stream(stream)), "ptflash_fp64_peak")
+    return f.value, ms.value
+
+
+def ptflash_version() -> str:
+    return load_library().ptflash_version().decode()
+
+
+# ---- convenience wrapper (allocation only) ----------------------------------------------------
+class PTFlash:
+    """Owns a handle for one component system; `flash` allocates the outputs with torch and calls the ABI."""
+
+    def __init__(self, Tc, Pc, omega, kij=None, **options):
+        self.nc = len(Tc)
+        self.h = ptflash_create(self.nc, Tc, Pc, omega, kij)
+        for k, v in options.items():
+            ptflash_set_option(self.h, k, v)
+
+    @classmethod
+    def from_system(cls, system, **options):
+        return cls(system.Tc, system.Pc, system.omega, system.kij, **options)
+
+    def set_option(self, key, value):
+        ptflash_set_option(self.h, key, value)
+
+    def stats(self):
+        return ptflash_get_stats(self.h)
+
+    def flash(self, z, P, T, lnK0=None, flags=None, extended=True, stream=None):
+        """z [nc, N], P [N], T [N]: CUDA float64 tensors -> dict of CUDA tensors."""
+        import torch
+        assert z.is_cuda and z.dtype == torch.float64 and z.shape[0] == self.nc
+        N = z.shape[1]
+        dev = z.device
+        f64 = dict(dtype=torch.float64, device=dev)
+        i32 = dict(dtype=torch.int32, device=dev)
+        out = dict(beta=torch.empty(N, **f64), x=torch.empty(self.nc, N, **f64), y=torch.empty(self.nc, N, **f64),
+                   phase=torch.empty(N, **i32), iters=torch.empty(N, **i32))
+        if extended:
+            out.update(tpd_min=torch.empty(N, **f64), lnK=torch.empty(self.nc, N, **f64),
+                       status=torch.empty(N, **i32), stab_iters=torch.empty(N, **i32))
+            ptflash_flash_ex(self.h, N, z, P, T, out["beta"], out["x"], out["y"], out["phase"], out["iters"],
+                             lnK0=lnK0, flags=flags, out_tpd_min=out["tpd_min"], out_lnK=out["lnK"],
+                             out_status=out["status"], out_stab_iters=out["stab_iters"], stream=stream)
+        else:
+            ptflash_flash(self.h, N, z, P, T, out["beta"], out["x"], out["y"], out["phase"], out["iters"], stream=stream)
+        return out
+
+    def close(self):
+        if self.h is not None:
+            ptflash_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,286 @@
+// ptflash_api.cu -- the C ABI of libptflash (include/ptflash.h): handle management, argument validation,
+// workspace ownership, option table, host-buffer variant and the FP64 roofline probe.  No torch types,
+// no CPU fallback: every numerical step runs in the kernels of ptflash_nc.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+
+#include "../../include/ptflash.h"
+#include "ptflash_launch.h"
+
+namespace {
+
+thread_local std::string g_err;
+void set_err(const std::string& s) { g_err = s; }
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  set_err(std::string(what) + ": " + cudaGetErrorString(e));
+  return false;
+}
+
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1};
+
+}  // namespace
+
+struct ptflash_handle_s {
+  int device;
+  ptf::SysHost sys;
+  double opts[PTFLASH_NUM_OPTS];
+  cudaStream_t last_stream;
+  bool used;
+  // workspace of the staged engine (device) and its size
+  void* ws;
+  size_t ws_bytes;
+  // staging buffers of ptflash_flash_host (device)
+  void* stage;
+  size_t stage_bytes;
+  // host mirror of the stage counters of the last call
+  ptf::StageCounters* counters_host;  // pinned
+  int64_t last_N;
+  int last_launches;
+};
+
+namespace {
+
+ptf::Opt make_opt(const double* o) {
+  ptf::Opt r;
+  r.tol_ss = o[PTFLASH_OPT_TOL_SS];
+  r.tol_newton_g = o[PTFLASH_OPT_TOL_NEWTON_G];
+  r.tol_newton_step = o[PTFLASH_OPT_TOL_NEWTON_STEP];
+  r.probe_margin = o[PTFLASH_OPT_PROBE_MARGIN];
+  r.trivial_tol = o[PTFLASH_OPT_TRIVIAL_TOL];
+  r.band = o[PTFLASH_OPT_BAND];
+  r.probe_iters = (int)o[PTFLASH_OPT_PROBE_ITERS];
+  r.stab_ss_iters = (int)o[PTFLASH_OPT_STAB_SS_ITERS];
+  r.stab_tr_iters = (int)o[PTFLASH_OPT_STAB_TR_ITERS];
+  r.split_ss_iters = (int)o[PTFLASH_OPT_SPLIT_SS_ITERS];
+  r.split_tr_iters = (int)o[PTFLASH_OPT_SPLIT_TR_ITERS];
+  r.use_newton = (int)o[PTFLASH_OPT_USE_NEWTON];
+  r.ss_cap = (int)o[PTFLASH_OPT_SS_CAP];
+  return r;
+}
+
+ptf::launch_fn pick_launcher(int nc, int engine) {
+  using namespace ptf;
+#define PTF_CASE(NC) case NC: return engine ? launch_staged_##NC : launch_mono_##NC;
+  switch (nc) {
+    PTF_CASE(2) PTF_CASE(3) PTF_CASE(4) PTF_CASE(5) PTF_CASE(6) PTF_CASE(7) PTF_CASE(8) PTF_CASE(9)
+    PTF_CASE(10) PTF_CASE(11) PTF_CASE(12) PTF_CASE(13) PTF_CASE(14) PTF_CASE(15) PTF_CASE(16)
+  }
+#undef PTF_CASE
+  return nullptr;
+}
+
+bool ensure(void** buf, size_t* have, size_t need, cudaStream_t st, const char* what) {
+  if (*have >= need) return true;
+  // growth: wait for work that may still use the old buffer, then reallocate
+  if (!cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize")) return false;
+  if (*buf) cudaFree(*buf);
+  *buf = nullptr;
+  *have = 0;
+  if (!cuda_ok(cudaMalloc(buf, need), what)) return false;
+  *have = need;
+  return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ptflash_last_error(void) { return g_err.c_str(); }
+const char* ptflash_version(void) { return "ptflash-b200 0.1 (sm_100a, fp64)"; }
+
+ptflash_handle_t ptflash_create(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij) {
+  g_err.clear();
+  if (nc < 2 || nc > PTFLASH_MAX_NC) { set_err("ptflash_create: nc must be in [2, 16]"); return nullptr; }
+  if (!Tc || !Pc || !omega) { set_err("ptflash_create: null Tc/Pc/omega"); return nullptr; }
+  for (int i = 0; i < nc; ++i) {
+    if (!std::isfinite(Tc[i]) || !std::isfinite(Pc[i]) || !std::isfinite(omega[i]) || Tc[i] <= 0.0 || Pc[i] <= 0.0) {
+      set_err("ptflash_create: Tc and Pc must be finite and positive, omega finite");
+      return nullptr;
+    }
+  }
+  if (kij) {
+    for (int i = 0; i < nc; ++i) {
+      if (kij[i * nc + i] != 0.0) { set_err("ptflash_create: kij diagonal must be zero"); return nullptr; }
+      for (int j = 0; j < nc; ++j) {
+        if (!std::isfinite(kij[i * nc + j]) || kij[i * nc + j] != kij[j * nc + i]) {
+          set_err("ptflash_create: kij must be finite and symmetric");
+          return nullptr;
+        }
+      }
+    }
+  }
+  int dev = 0;
+  if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return nullptr;
+  ptflash_handle_s* h = new ptflash_handle_s();
+  std::memset(h, 0, sizeof(*h));
+  h->device = dev;
+  ptf::SysHost& s = h->sys;
+  s.nc = nc;
+  s.kij_zero = 1;
+  for (int i = 0; i < nc; ++i) {
+    // A.2d-g PAPER.md:420-427 folded into per-component constants (see ptflash_device.cuh)
+    const double m = 0.480 + 1.574 * omega[i] - 0.176 * omega[i] * omega[i];
+    const double k = std::sqrt(0.42748 / Pc[i]);
+    s.u[i] = k * Tc[i] * (1.0 + m);
+    s.v[i] = k * std::sqrt(Tc[i]) * m;
+    s.wb[i] = 0.08664 * Tc[i] / Pc[i];
+    s.lnpc[i] = std::log(Pc[i]);
+    s.wil[i] = 5.373 * (1.0 + omega[i]);  // eq. 6
+    s.tc[i] = Tc[i];
+    for (int j = 0; j < nc; ++j) {
+      const double kk = kij ? kij[i * nc + j] : 0.0;
+      s.omk[i * nc + j] = 1.0 - kk;
+      if (kk != 0.0) s.kij_zero = 0;
+    }
+  }
+  std::memcpy(h->opts, kDefaultOpts, sizeof(kDefaultOpts));
+  if (!cuda_ok(cudaMallocHost((void**)&h->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete h; return nullptr; }
+  std::memset(h->counters_host, 0, sizeof(ptf::StageCounters));
+  return h;
+}
+
+int ptflash_destroy(ptflash_handle_t h) {
+  if (!h) return PTFLASH_OK;
+  int rc = PTFLASH_OK;
+  cudaSetDevice(h->device);
+  if (h->used && !cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) rc = PTFLASH_ECUDA;
+  if (h->ws) cudaFree(h->ws);
+  if (h->stage) cudaFree(h->stage);
+  if (h->counters_host) cudaFreeHost(h->counters_host);
+  delete h;
+  return rc;
+}
+
+int ptflash_set_option(ptflash_handle_t h, int key, double value) {
+  if (!h || key < 0 || key >= PTFLASH_NUM_OPTS || !std::isfinite(value)) { set_err("ptflash_set_option: bad handle/key/value"); return PTFLASH_EINVAL; }
+  h->opts[key] = value;
+  return PTFLASH_OK;
+}
+int ptflash_get_option(ptflash_handle_t h, int key, double* value) {
+  if (!h || !value || key < 0 || key >= PTFLASH_NUM_OPTS) { set_err("ptflash_get_option: bad handle/key"); return PTFLASH_EINVAL; }
+  *value = h->opts[key];
+  return PTFLASH_OK;
+}
+
+int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
+  g_err.clear();
+  if (!h || !io) { set_err("ptflash_flash: null handle or io"); return PTFLASH_EINVAL; }
+  if (io->N < 0) { set_err("ptflash_flash: N < 0"); return PTFLASH_EINVAL; }
+  if (io->N == 0) return PTFLASH_OK;
+  if (!io->z || !io->P || !io->T || !io->out_beta || !io->out_x || !io->out_y || !io->out_phase) {
+    set_err("ptflash_flash: null required pointer");
+    return PTFLASH_EINVAL;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int engine = (int)h->opts[PTFLASH_OPT_ENGINE];
+  ptf::launch_fn fn = pick_launcher(h->sys.nc, engine);
+  if (!fn) { set_err("ptflash_flash: no kernel for this nc"); return PTFLASH_EINVAL; }
+  ptf::Io d;
+  d.N = io->N;
+  d.z = io->z; d.P = io->P; d.T = io->T;
+  d.lnK0 = io->lnK0;
+  d.flags = io->lnK0 ? io->flags : nullptr;
+  d.beta = io->out_beta; d.x = io->out_x; d.y = io->out_y;
+  d.phase = io->out_phase; d.iters = io->out_iters;
+  d.tpd_min = io->out_tpd_min; d.lnK = io->out_lnK; d.status = io->out_status; d.stab_iters = io->out_stab_iters;
+  if (engine) {
+    const size_t need = ptf::staged_workspace_bytes(h->sys.nc, io->N);
+    if (!ensure(&h->ws, &h->ws_bytes, need, st, "cudaMalloc(workspace)")) return PTFLASH_ECUDA;
+  }
+  const ptf::Opt o = make_opt(h->opts);
+  const int launches = fn(h->sys, o, d, h->ws, st);
+  if (launches < 0) { cuda_ok(cudaGetLastError(), "kernel launch"); if (g_err.empty()) set_err("kernel launch failed"); return PTFLASH_ECUDA; }
+  if (engine) {
+    // stage counters -> pinned host mirror (read by ptflash_get_stats after a synchronise)
+    if (!cuda_ok(cudaMemcpyAsync(h->counters_host, h->ws, sizeof(ptf::StageCounters), cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync(counters)"))
+      return PTFLASH_ECUDA;
+  }
+  h->last_stream = st;
+  h->used = true;
+  h->last_N = io->N;
+  h->last_launches = launches;
+  return PTFLASH_OK;
+}
+
+int ptflash_flash(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T, double* out_beta,
+                  double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters, void* stream) {
+  ptflash_io_t io;
+  std::memset(&io, 0, sizeof(io));
+  io.N = N; io.z = z; io.P = P; io.T = T;
+  io.out_beta = out_beta; io.out_x = out_x; io.out_y = out_y; io.out_phase = out_phase; io.out_iters = out_iters;
+  return ptflash_flash_ex(h, &io, stream);
+}
+
+int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T, double* out_beta,
+                       double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters, void* stream) {
+  g_err.clear();
+  if (!h) { set_err("ptflash_flash_host: null handle"); return PTFLASH_EINVAL; }
+  if (N < 0) { set_err("ptflash_flash_host: N < 0"); return PTFLASH_EINVAL; }
+  if (N == 0) return PTFLASH_OK;
+  if (!z || !P || !T || !out_beta || !out_x || !out_y || !out_phase) { set_err("ptflash_flash_host: null required pointer"); return PTFLASH_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nc = h->sys.nc;
+  const size_t nd = (size_t)N;
+  // device staging: z, P, T, beta, x, y (doubles), phase, iters (int32)
+  const size_t n_dbl = nd * (size_t)(nc + 2 + 1 + 2 * nc);
+  const size_t need = n_dbl * sizeof(double) + 2 * nd * sizeof(int32_t);
+  if (!ensure(&h->stage, &h->stage_bytes, need, st, "cudaMalloc(staging)")) return PTFLASH_ECUDA;
+  double* dz = (double*)h->stage;
+  double* dP = dz + nd * nc;
+  double* dT = dP + nd;
+  double* dbeta = dT + nd;
+  double* dx = dbeta + nd;
+  double* dy = dx + nd * nc;
+  int32_t* dphase = (int32_t*)(dy + nd * nc);
+  int32_t* diters = dphase + nd;
+  if (!cuda_ok(cudaMemcpyAsync(dz, z, nd * nc * sizeof(double), cudaMemcpyHostToDevice, st), "H2D z")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(dP, P, nd * sizeof(double), cudaMemcpyHostToDevice, st), "H2D P")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(dT, T, nd * sizeof(double), cudaMemcpyHostToDevice, st), "H2D T")) return PTFLASH_ECUDA;
+  const int rc = ptflash_flash(h, N, dz, dP, dT, dbeta, dx, dy, dphase, out_iters ? diters : nullptr, stream);
+  if (rc != PTFLASH_OK) return rc;
+  if (!cuda_ok(cudaMemcpyAsync(out_beta, dbeta, nd * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H beta")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(out_x, dx, nd * nc * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H x")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(out_y, dy, nd * nc * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H y")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(out_phase, dphase, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st), "D2H phase")) return PTFLASH_ECUDA;
+  if (out_iters && !cuda_ok(cudaMemcpyAsync(out_iters, diters, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st), "D2H iters")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
+  return PTFLASH_OK;
+}
+
+int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
+  if (!h || !out) { set_err("ptflash_get_stats: null argument"); return PTFLASH_EINVAL; }
+  std::memset(out, 0, sizeof(*out));
+  if (!h->used) return PTFLASH_OK;
+  if (!cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
+  const ptf::StageCounters& c = *h->counters_host;
+  out->n_total = h->last_N;
+  out->kernel_launches = h->last_launches;
+  if ((int)h->opts[PTFLASH_OPT_ENGINE]) {
+    out->n_invalid = c.n_invalid;
+    out->n_probe_case1 = c.n_case1;
+    out->n_probe_case2 = c.n_case2;
+    out->n_probe_case3 = c.n_case3;
+    out->n_stability = c.n_stab;
+    out->n_stab_newton = c.n_stab_newton;
+    out->n_split = c.n_split;
+    out->n_split_newton = c.n_split_newton;
+    out->n_two_phase = c.n_two_phase;
+  }
+  return PTFLASH_OK;
+}
+
+int ptflash_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, void* stream) {
+  g_err.clear();
+  if (iters <= 0 || !flops_per_s) { set_err("ptflash_fp64_peak: bad arguments"); return PTFLASH_EINVAL; }
+  double fl = 0.0, ms = 0.0;
+  if (ptf::run_fp64_peak(iters, &fl, &ms, (cudaStream_t)stream) != 0) { cuda_ok(cudaGetLastError(), "fp64 peak kernel"); return PTFLASH_ECUDA; }
+  *flops_per_s = fl;
+  if (elapsed_ms) *elapsed_ms = ms;
+  return PTFLASH_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,37 @@
+// ptflash_nc.cu -- kernel instantiations for ONE component count; compiled once per NC with -DPTF_NC=<k>
+// (nvcc -gencode arch=compute_100a,code=sm_100a), so the 15 variants build in parallel.
+#include "ptflash_launch.h"
+#include "ptflash_flash.cuh"
+
+#ifndef PTF_NC
+#error "compile with -DPTF_NC=<2..16>"
+#endif
+
+#define PTF_CAT2(a, b) a##b
+#define PTF_CAT(a, b) PTF_CAT2(a, b)
+
+namespace ptf {
+
+#ifdef PTF_STUB
+// development build that left this component count out
+int PTF_CAT(launch_mono_, PTF_NC)(const SysHost&, const Opt&, const Io&, void*, cudaStream_t) { return -1; }
+int PTF_CAT(launch_staged_, PTF_NC)(const SysHost&, const Opt&, const Io&, void*, cudaStream_t) { return -1; }
+}  // namespace ptf
+#else
+
+int PTF_CAT(launch_mono_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io, void*, cudaStream_t st) {
+  constexpr int NC = PTF_NC;
+  const Sys<NC> s = narrow<NC>(hs);
+  const int threads = 128;
+  const int64_t blocks = (io.N + threads - 1) / threads;
+  flash_mono_kernel<NC><<<(unsigned)blocks, threads, 0, st>>>(s, o, io);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// TEMPORARY until the staged engine lands: same kernel
+int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io, void* ws, cudaStream_t st) {
+  return PTF_CAT(launch_mono_, PTF_NC)(hs, o, io, ws, st);
+}
+
+}  // namespace ptf
+#endif
