@@ -2,6 +2,7 @@
 // (nvcc -gencode arch=compute_100a,code=sm_100a), so the 15 variants build in parallel.
 #include "ptflash_launch.h"
 #include "ptflash_flash.cuh"
+#include "ptflash_staged.cuh"
 
 #ifndef PTF_NC
 #error "compile with -DPTF_NC=<2..16>"
@@ -28,9 +29,8 @@ int PTF_CAT(launch_mono_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io,
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-// TEMPORARY until the staged engine lands: same kernel
 int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io, void* ws, cudaStream_t st) {
-  return PTF_CAT(launch_mono_, PTF_NC)(hs, o, io, ws, st);
+  return launch_staged<PTF_NC>(hs, o, io, ws, st);
 }
 
 }  // namespace ptf

@@ -1,5 +1,6 @@
 // ptflash_peak.cu -- FP64 roofline probe (independent DFMA chains on every SM) and workspace sizing.
 #include "ptflash_launch.h"
+#include "ptflash_staged.cuh"
 
 namespace ptf {
 
@@ -48,8 +49,7 @@ int run_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, cudaStream
 }
 
 size_t staged_workspace_bytes(int nc, int64_t N) {
-  (void)nc; (void)N;
-  return sizeof(StageCounters);
+  return carve_workspace(nc, N, nullptr, nullptr);
 }
 
 }  // namespace ptf

@@ -1,0 +1,417 @@
+// ptflash_staged.cuh -- engine 1: the flash as a sequence of stage kernels connected by work queues in HBM.
+//
+// The paper vectorises every stage over the surviving samples and compacts with a boolean mask after EVERY
+// iteration, with the host in the loop (synchronizer, eq. 10, Alg. 1; barriers
+// at the entry of stability and split).  Here a mixture's iterate stays in registers for a whole
+// stage; only the per-stage hand-over (ids + O(nc) doubles) goes through HBM, and the queues are built on the
+// device with warp-aggregated atomics (ballot + popc prefix), so the host never waits:
+//
+//   K1a init        all N: validate, normalise, ln z, d = ln z + lnphi(z), first Rachford-Rice window test
+//                   -> q_probe | q_stab (probe case 1) | q_split (caller said "unstable")
+//   K1b probe       q_probe: 3 phase-split SS iterations + Delta G/tpd test (section 2.2.3)
+//                   -> q_stab (cases 1, 2) | q_split (case 3)
+//   K2  stab_ss     2 x q_stab (one work item per start): <= 9 SS iterations (eq. 5) -> done | q_stab_newton
+//   K3  stab_newton q_stab_newton: trust-region Newton (B.1-B.3)
+//   K4  stab_decide q_stab: label + K seed -> single-phase store | q_split
+//   K5  split_ss    q_split: <= 9 SS iterations (Fig. 1) -> store | q_split_newton
+//   K6  split_newton q_split_newton: trust-region Newton on G (B.4-B.5) -> store
+//
+// Every kernel is persistent-style: a fixed grid sized from the SM count walks its queue with a grid-stride
+// loop, reading the queue length from device memory.
+#pragma once
+#include "ptflash_flash.cuh"
+#include "ptflash_launch.h"
+
+namespace ptf {
+
+enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_COUNT = 8 };
+enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_ITER_SHIFT = 8 };
+
+struct Work {
+  StageCounters* ctr;
+  int* qcount;  // [Q_COUNT]
+  int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton;
+  double *lnz, *d, *lnK;   // [NC][N]
+  double* lnW;             // [2][NC][N]
+  double *tm, *sumW;       // [2][N]
+  double *Zfeed, *tpdmin;  // [N]
+  int* tflags;             // [2][N]
+  int *status, *iters, *stabit;  // [N]
+};
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// Carves the workspace; with base == nullptr only the size is computed.
+inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align256(bytes); return p; };
+  const size_t n = (size_t)N, c = (size_t)nc;
+  char* p;
+  p = take(sizeof(StageCounters)); if (w) w->ctr = (StageCounters*)p;
+  p = take(Q_COUNT * sizeof(int)); if (w) w->qcount = (int*)p;
+  p = take(n * 4); if (w) w->q_probe = (int*)p;
+  p = take(n * 4); if (w) w->q_stab = (int*)p;
+  p = take(2 * n * 4); if (w) w->q_stab_newton = (int*)p;
+  p = take(n * 4); if (w) w->q_split = (int*)p;
+  p = take(n * 4); if (w) w->q_split_newton = (int*)p;
+  p = take(c * n * 8); if (w) w->lnz = (double*)p;
+  p = take(c * n * 8); if (w) w->d = (double*)p;
+  p = take(c * n * 8); if (w) w->lnK = (double*)p;
+  p = take(2 * c * n * 8); if (w) w->lnW = (double*)p;
+  p = take(2 * n * 8); if (w) w->tm = (double*)p;
+  p = take(2 * n * 8); if (w) w->sumW = (double*)p;
+  p = take(n * 8); if (w) w->Zfeed = (double*)p;
+  p = take(n * 8); if (w) w->tpdmin = (double*)p;
+  p = take(2 * n * 4); if (w) w->tflags = (int*)p;
+  p = take(n * 4); if (w) w->status = (int*)p;
+  p = take(n * 4); if (w) w->iters = (int*)p;
+  p = take(n * 4); if (w) w->stabit = (int*)p;
+  return off;
+}
+
+// Warp-aggregated append: lanes with pred == true get consecutive slots of the queue (ballot + prefix popc).
+__device__ __forceinline__ void queue_push(bool pred, int* __restrict__ count, int* __restrict__ queue, int value) {
+  const unsigned active = __activemask();
+  const unsigned mask = __ballot_sync(active, pred);
+  if (mask == 0u) return;
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(mask) - 1;
+  int base = 0;
+  if (lane == leader) base = atomicAdd(count, __popc(mask));
+  base = __shfl_sync(active, base, leader);
+  if (pred) queue[base + __popc(mask & ((1u << lane) - 1u))] = value;
+}
+
+__device__ __forceinline__ void count_add(bool pred, long long* ctr) {
+  const unsigned active = __activemask();
+  const unsigned mask = __ballot_sync(active, pred);
+  if (mask && (int)(threadIdx.x & 31) == __ffs(mask) - 1) atomicAdd((unsigned long long*)ctr, (unsigned long long)__popc(mask));
+}
+
+// context of a mixture already validated by K1a
+template <int NC>
+__device__ __forceinline__ void reload_ctx(const Sys<NC>& S, const Io& io, const Work& w, int n, bool need_ref, MixCtx<NC>& m,
+                                           double& P, double& T) {
+  load_feed<NC>(io, n, m.z, P, T);
+  eos_setup<NC>(S, P, T, m.sa, m.bi);
+  if (need_ref) {
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      m.lnz[i] = w.lnz[(int64_t)i * io.N + n];
+      m.d[i] = w.d[(int64_t)i * io.N + n];
+    }
+  }
+}
+
+#define PTF_GRID_STRIDE(idx, total) \
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (total); idx += (int64_t)gridDim.x * blockDim.x)
+
+// ---- K1a ------------------------------------------------------------------------------------------
+template <int NC>
+__global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                              const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t Npad = (io.N + 31) & ~(int64_t)31;  // whole warps stay together for the ballots
+  PTF_GRID_STRIDE(idx, Npad) {
+    const bool in = idx < io.N;
+    const int n = (int)idx;
+    MixCtx<NC> m;
+    double P = 1.0, T = 1.0, Zf = 0.0;
+    bool valid = false;
+    if (in) {
+      valid = load_feed<NC>(io, n, m.z, P, T);
+      if (!valid) store_invalid<NC>(io, n);
+    }
+    count_add(in && !valid, &w.ctr->n_invalid);
+    int dest = -1;  // 0 probe, 1 stab, 2 split
+    if (valid) {
+      feed_reference<NC>(S, P, T, m, Zf);
+      int status = 0, fl = 0;
+      double lnKs[NC];
+      const bool have0 = start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        w.lnz[(int64_t)i * io.N + n] = m.lnz[i];
+        w.d[(int64_t)i * io.N + n] = m.d[i];
+      }
+      w.Zfeed[n] = Zf;
+      w.status[n] = status;
+      w.iters[n] = 0;
+      w.stabit[n] = 0;
+      if (have0 && (fl & 1)) {
+        dest = 2;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnKs[i];
+        w.tpdmin[n] = __longlong_as_double(0x7ff8000000000000LL);
+      } else if (o.probe_iters == 0) {
+        dest = 1;
+      } else {
+        // first Rachford-Rice of the probe: theta in (0,1) <=> window exists, f(0) > 0 and f(1) < 0
+        double f0 = 0.0, f1 = 0.0, Kmax = 0.0, Kmin = 1.0e300;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          if (m.z[i] > 0.0) {
+            const double K = exp(lnKs[i]);
+            Kmax = fmax(Kmax, K);
+            Kmin = fmin(Kmin, K);
+            f0 = fma(m.z[i], K - 1.0, f0);
+            f1 += m.z[i] * (K - 1.0) / K;
+          }
+        }
+        dest = (Kmax > 1.0 && Kmin < 1.0 && f0 > 0.0 && f1 < 0.0) ? 0 : 1;
+      }
+    }
+    count_add(dest == 1, &w.ctr->n_case1);
+    queue_push(dest == 0, &w.qcount[Q_PROBE], w.q_probe, n);
+    queue_push(dest == 1, &w.qcount[Q_STAB], w.q_stab, n);
+    queue_push(dest == 2, &w.qcount[Q_SPLIT], w.q_split, n);
+  }
+}
+
+// ---- K1b ------------------------------------------------------------------------------------------
+template <int NC>
+__global__ void __launch_bounds__(128) k_probe(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                               const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_PROBE];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    int pcase = 0, n = 0;
+    if (in) {
+      n = w.q_probe[idx];
+      MixCtx<NC> m;
+      double P, T;
+      reload_ctx<NC>(S, io, w, n, true, m, P, T);
+      int status = 0, fl = 0, iters = 0;
+      double lnK[NC];
+      start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
+      double tpd_min = 0.0;
+      pcase = probe<NC>(S, o, m, lnK, tpd_min, iters);
+      w.iters[n] = iters;
+      if (pcase == 3) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnK[i];
+        w.tpdmin[n] = tpd_min;
+      }
+    }
+    count_add(pcase == 1, &w.ctr->n_case1);
+    count_add(pcase == 2, &w.ctr->n_case2);
+    count_add(pcase == 3, &w.ctr->n_case3);
+    queue_push(pcase == 1 || pcase == 2, &w.qcount[Q_STAB], w.q_stab, n);
+    queue_push(pcase == 3, &w.qcount[Q_SPLIT], w.q_split, n);
+  }
+}
+
+// ---- K2 -------------------------------------------------------------------------------------------
+template <int NC>
+__device__ __forceinline__ void store_trial(const Io& io, const Work& w, int n, int sidx, const StabState<NC>& st) {
+  const int64_t N = io.N;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = st.lnW[i];
+  w.tm[(int64_t)sidx * N + n] = st.tm;
+  w.sumW[(int64_t)sidx * N + n] = st.sumW;
+  w.tflags[(int64_t)sidx * N + n] = (st.converged ? TF_CONVERGED : 0) | (st.stationary_exact ? TF_EXACT : 0) |
+                                    (st.capped ? TF_CAPPED : 0) | (st.iters << TF_ITER_SHIFT);
+}
+
+template <int NC>
+__global__ void __launch_bounds__(128) k_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                 const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    bool need_newton = false;
+    int item = 0;
+    if (in) {
+      const int n = w.q_stab[idx >> 1];
+      const int sidx = (int)(idx & 1);  // 0 vapour-like, 1 liquid-like
+      item = (n << 1) | sidx;
+      MixCtx<NC> m;
+      double P, T;
+      reload_ctx<NC>(S, io, w, n, true, m, P, T);
+      int status = 0, fl = 0;
+      double lnKs[NC];
+      start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
+      StabState<NC> st;
+      stab_init<NC>(m, lnKs, sidx ? -1.0 : 1.0, st);
+      stab_ss<NC>(S, o, m, st);
+      need_newton = !st.converged && o.use_newton;
+      store_trial<NC>(io, w, n, sidx, st);
+    }
+    queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
+  }
+}
+
+// ---- K3 -------------------------------------------------------------------------------------------
+template <int NC>
+__global__ void __launch_bounds__(128) k_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                     const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_STAB_NEWTON];
+  PTF_GRID_STRIDE(idx, cnt) {
+    const int item = w.q_stab_newton[idx];
+    const int n = item >> 1, sidx = item & 1;
+    MixCtx<NC> m;
+    double P, T;
+    reload_ctx<NC>(S, io, w, n, true, m, P, T);
+    StabState<NC> st;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) st.lnW[i] = w.lnW[((int64_t)sidx * NC + i) * io.N + n];
+    st.tm = 0.0; st.sumW = 1.0;
+    st.iters = w.tflags[(int64_t)sidx * io.N + n] >> TF_ITER_SHIFT;
+    st.converged = false; st.stationary_exact = false; st.capped = false;
+    stab_newton<NC>(S, o, m, st);
+    store_trial<NC>(io, w, n, sidx, st);
+  }
+}
+
+// ---- K4 -------------------------------------------------------------------------------------------
+template <int NC>
+__global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                     const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_STAB];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  const int64_t N = io.N;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    bool unstable = false;
+    int n = 0;
+    if (in) {
+      n = w.q_stab[idx];
+      MixCtx<NC> m;
+      double P, T;
+      load_feed<NC>(io, n, m.z, P, T);
+#pragma unroll
+      for (int i = 0; i < NC; ++i) m.lnz[i] = w.lnz[(int64_t)i * N + n];
+      StabState<NC> sv, sl;
+      StabRes rv, rl;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) { sv.lnW[i] = w.lnW[(int64_t)i * N + n]; sl.lnW[i] = w.lnW[((int64_t)NC + i) * N + n]; }
+      const int fv = w.tflags[n], fl_ = w.tflags[N + n];
+      sv.tm = w.tm[n]; sv.sumW = w.sumW[n]; sv.iters = fv >> TF_ITER_SHIFT;
+      sv.converged = fv & TF_CONVERGED; sv.stationary_exact = fv & TF_EXACT; sv.capped = fv & TF_CAPPED;
+      sl.tm = w.tm[N + n]; sl.sumW = w.sumW[N + n]; sl.iters = fl_ >> TF_ITER_SHIFT;
+      sl.converged = fl_ & TF_CONVERGED; sl.stationary_exact = fl_ & TF_EXACT; sl.capped = fl_ & TF_CAPPED;
+      stab_finish<NC>(o, m, sv, rv);
+      stab_finish<NC>(o, m, sl, rl);
+      double lnK[NC], tpd_min = 0.0;
+      int status = w.status[n];
+      unstable = stab_decide<NC>(o, m, rv, rl, sv.lnW, sl.lnW, lnK, tpd_min, status);
+      const int stab_iters = rv.iters + rl.iters;
+      if (unstable) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = lnK[i];
+        w.tpdmin[n] = tpd_min;
+        w.status[n] = status;
+        w.stabit[n] = stab_iters;
+      } else {
+        store_result<NC>(io, n, false, 0.0, m.z, m.z, m.z, lnK, w.Zfeed[n], w.iters[n], status, tpd_min, stab_iters);
+      }
+    }
+    queue_push(unstable, &w.qcount[Q_SPLIT], w.q_split, n);
+  }
+}
+
+// ---- K5 / K6 --------------------------------------------------------------------------------------
+template <int NC>
+__device__ __forceinline__ void finish_split(const Io& io, const Work& w, int n, const MixCtx<NC>& m, const SplitState<NC>& st,
+                                             const double (&x)[NC], const double (&y)[NC]) {
+  SplitRes sp;
+  split_finish<NC>(st, sp);
+  int status = w.status[n] | sp.status;
+  if (!sp.two_phase) status |= ST_SPLIT_FAILED;
+  store_result<NC>(io, n, sp.two_phase, sp.theta, m.z, x, y, st.lnK, w.Zfeed[n], w.iters[n] + sp.iters, status, w.tpdmin[n],
+                   w.stabit[n]);
+  count_add(sp.two_phase, &w.ctr->n_two_phase);
+}
+
+template <int NC>
+__global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                  const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_SPLIT];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    bool go_newton = false;
+    int n = 0;
+    if (in) {
+      n = w.q_split[idx];
+      MixCtx<NC> m;
+      double P, T;
+      reload_ctx<NC>(S, io, w, n, false, m, P, T);
+      SplitState<NC> st;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) st.lnK[i] = w.lnK[(int64_t)i * io.N + n];
+      double x[NC], y[NC];
+      split_ss<NC>(S, o, m, st, x, y);
+      go_newton = st.go_newton;
+      if (go_newton) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = st.lnK[i];
+        w.iters[n] += st.iters;
+        w.status[n] |= st.status;
+      } else {
+        finish_split<NC>(io, w, n, m, st, x, y);
+      }
+    }
+    queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
+  }
+}
+
+template <int NC>
+__global__ void __launch_bounds__(128) k_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                      const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_SPLIT_NEWTON];
+  PTF_GRID_STRIDE(idx, cnt) {
+    const int n = w.q_split_newton[idx];
+    MixCtx<NC> m;
+    double P, T;
+    reload_ctx<NC>(S, io, w, n, false, m, P, T);
+    SplitState<NC> st;
+    double K[NC], x[NC], y[NC];
+#pragma unroll
+    for (int i = 0; i < NC; ++i) { st.lnK[i] = w.lnK[(int64_t)i * io.N + n]; K[i] = exp(st.lnK[i]); }
+    st.iters = 0; st.status = 0; st.converged = false; st.failed = false; st.go_newton = true;
+    rr_solve<NC>(K, m.z, st.theta, x, y);  // the same Rachford-Rice that ended the SS stage
+    split_newton<NC>(S, o, m, st, x, y);
+    finish_split<NC>(io, w, n, m, st, x, y);
+  }
+}
+
+// counters that are simply queue lengths
+static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    w.ctr->n_stab = w.qcount[Q_STAB];
+    w.ctr->n_stab_newton = w.qcount[Q_STAB_NEWTON];
+    w.ctr->n_split = w.qcount[Q_SPLIT];
+    w.ctr->n_split_newton = w.qcount[Q_SPLIT_NEWTON];
+  }
+}
+
+template <int NC>
+int launch_staged(const SysHost& hs, const Opt& o, const Io& io, void* workspace, cudaStream_t st) {
+  const Sys<NC> s = narrow<NC>(hs);
+  Work w;
+  carve_workspace(NC, io.N, (char*)workspace, &w);
+  if (cudaMemsetAsync(workspace, 0, align256(sizeof(StageCounters)) + align256(Q_COUNT * sizeof(int)), st) != cudaSuccess) return -1;
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int threads = 128;
+  auto grid_for = [&](int64_t items) {
+    const int64_t need = (items + threads - 1) / threads;
+    const int64_t cap = (int64_t)sms * 16;
+    return (unsigned)(need < cap ? (need > 0 ? need : 1) : cap);
+  };
+  const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
+  k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k_probe<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k_stab_ss<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
+  k_stab_newton<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
+  k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k_split_ss<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k_split_newton<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k_finalize_counters<<<1, 32, 0, st>>>(w);
+  return cudaGetLastError() == cudaSuccess ? 8 : -1;
+}
+
+}  // namespace ptf
