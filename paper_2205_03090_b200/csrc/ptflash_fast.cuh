@@ -1,0 +1,276 @@
+// ptflash_fast.cuh -- register-resident, warm-started variants of the device functions in ptflash_device.cuh,
+// used by the stage kernels of engine 1.  Same operations, same decisions (admissible roots Z > B, minimum
+// Gibbs energy, Rachford-Rice window), different iteration paths:
+//   * the cubic (A.3) is iterated from the previous root of the same phase (2-3 Newton steps) and falls back to
+//     the monotone side-selected Newton; the other roots come from the deflated quadratic (A.5);
+//   * Rachford-Rice (eq. 7) starts from the previous theta and stops after the first Newton step below 1e-8
+//     of the window (App. C: "When the Newton step size is smaller than 1.0e-8, the iteration stops";
+//     the step is applied, so the error is ~1e-16);
+//   * everything is __forceinline__ so per-mixture vectors stay in registers (no struct passing through local memory);
+//   * symmetric nc x nc systems live in registers as a packed lower triangle with compile-time indices.
+#pragma once
+#include "ptflash_device.cuh"
+
+namespace ptf {
+
+// packed lower-triangle index, i >= j
+__host__ __device__ constexpr int tri(int i, int j) { return i * (i + 1) / 2 + j; }
+
+// ------------------------------------------------------------------------------------------------
+// cubic with warm start.  Zg: previous root of this phase (<= 0: none).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, double& lnZmB, double& L) {
+  const double r0 = A * B, r1 = A - B * (1.0 + B);
+  double Z = Zg;
+  bool ok = false;
+  if (Zg > B) {
+    // plain Newton from the previous root; accept only a clean quadratic finish
+#pragma unroll 1
+    for (int k = 0; k < 4; ++k) {
+      const double df = cub_df(Z, r1);
+      const double dz = cub_f(Z, r1, r0) / df;
+      const double Zn = Z - dz;
+      if (!(Zn > B) || !(Zn < 2.0 + B)) break;   // also catches NaN / df == 0
+      Z = Zn;
+      if (fabs(dz) <= 1.0e-8 * Zn) { ok = true; break; }
+    }
+    if (ok) {
+      // one more guarded step brings the root to rounding (and detects a linear-rate, i.e. nearly double, root)
+      const double df = cub_df(Z, r1);
+      const double dz = cub_f(Z, r1, r0) / df;
+      if (fabs(dz) <= 1.0e-13 * Z) Z -= dz; else ok = false;
+    }
+  }
+  if (!ok) {
+    const double third = 1.0 / 3.0;
+    const bool up = (B < third) && (cub_f(third, r1, r0) > 0.0);
+    Z = up ? B : 1.0 + B;
+#pragma unroll 1
+    for (int k = 0; k < 100; ++k) {
+      const double df = cub_df(Z, r1);
+      if (!(df > 0.0)) break;
+      const double Zn = Z - cub_f(Z, r1, r0) / df;
+      if (up ? !(Zn > Z) : !(Zn < Z)) break;
+      Z = Zn;
+    }
+  }
+  double zmin = Z, zmax = Z;
+  const double p = Z - 1.0, q = fma(p, Z, r1);
+  const double disc = fma(p, p, -4.0 * q);
+  if (disc >= 0.0) {
+    const double sq = sqrt(disc);
+    const double t = (p >= 0.0) ? -0.5 * (p + sq) : 0.5 * (sq - p);
+    double ra = t, rb = (t != 0.0) ? q / t : -p - t;
+    ra = cub_polish(ra, r1, r0);
+    rb = cub_polish(rb, r1, r0);
+    if (ra > B) { zmin = fmin(zmin, ra); zmax = fmax(zmax, ra); }
+    if (rb > B) { zmin = fmin(zmin, rb); zmax = fmax(zmax, rb); }
+  }
+  double lz = log(zmin - B), ll = log1p(B / zmin);
+  if (zmax != zmin) {
+    const double AoB = A / B;
+    const double lz2 = log(zmax - B), ll2 = log1p(B / zmax);
+    const double gl = zmin - 1.0 - lz - AoB * ll;
+    const double gv = zmax - 1.0 - lz2 - AoB * ll2;
+    if (gv < gl) { zmin = zmax; lz = lz2; ll = ll2; }
+  }
+  lnZmB = lz;
+  L = ll;
+  return zmin;
+}
+
+// ------------------------------------------------------------------------------------------------
+// lnphi of composition c (sum c = 1) given sqrt(A_i), B_i.  e.Z on entry = warm start (<= 0: none).
+// KIJ0: all k_ij == 0, S_i = sqrt(A_i) * sum_j sqrt(A_j) c_j.
+// ------------------------------------------------------------------------------------------------
+template <int NC, bool KIJ0>
+__device__ __forceinline__ void lnphi_fast(const Sys<NC>& S, const double (&sa)[NC], const double (&bi)[NC],
+                                           const double (&c)[NC], double (&lp)[NC], double (&Sv)[NC], Eos& e) {
+  double t[NC];
+#pragma unroll
+  for (int j = 0; j < NC; ++j) t[j] = sa[j] * c[j];
+  if (KIJ0) {
+    double sum = 0.0;
+#pragma unroll
+    for (int j = 0; j < NC; ++j) sum += t[j];
+#pragma unroll
+    for (int i = 0; i < NC; ++i) Sv[i] = sa[i] * sum;
+  } else {
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+      for (int j = 0; j < NC; j += 2) {
+        a0 = fma(S.omk[i * NC + j], t[j], a0);
+        if (j + 1 < NC) a1 = fma(S.omk[i * NC + j + 1], t[j + 1], a1);
+      }
+      Sv[i] = sa[i] * (a0 + a1);
+    }
+  }
+  double A = 0.0, B = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    A = fma(c[i], Sv[i], A);
+    B = fma(c[i], bi[i], B);
+  }
+  e.A = A;
+  e.B = B;
+  e.Z = pick_root_fast(A, B, e.Z, e.lnZmB, e.L);
+  const double invB = 1.0 / B;
+  e.q = e.L * invB;
+  const double zm1 = e.Z - 1.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    const double b = bi[i] * invB;
+    lp[i] = fma(b, zm1, -e.lnZmB) - e.q * fma(2.0, Sv[i], -A * b);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Coefficients of M_ij = n dlnphi_i/dn_j (unit total moles) in the form
+//   M_ij = e_i p_j + c_j - Dq_j u_i + 2q (S_i - A_ij),   e_i = B_i/B, u_i = 2 S_i - A e_i
+// so that a matrix entry costs four FMAs (derivation: DESIGN.md section 3; identical to dlnphi()).
+// ------------------------------------------------------------------------------------------------
+struct MCoef {
+  double invB, A, q2, zA2, zBB, zm1, qA, invZmB, B, cL1, cL2, q;
+};
+__device__ __forceinline__ MCoef mcoef(const Eos& e) {
+  MCoef m;
+  const double A = e.A, B = e.B, Z = e.Z;
+  const double FZ = fma(fma(3.0, Z, -2.0), Z, A - B - B * B);
+  const double iFZ = 1.0 / FZ;
+  const double ZA = -(Z - B) * iFZ;
+  const double ZB = fma(1.0 + 2.0 * B, Z, A) * iFZ;
+  const double iZZB = 1.0 / (Z * (Z + B));
+  m.invB = 1.0 / B;
+  m.A = A; m.B = B; m.q = e.q;
+  m.q2 = 2.0 * e.q;
+  m.zA2 = 2.0 * ZA;
+  m.zBB = ZB * B;
+  m.zm1 = Z - 1.0;
+  m.qA = e.q * A;
+  m.invZmB = 1.0 / (Z - B);
+  m.cL1 = (Z - ZB * B) * iZZB;   // DL_j / B = cL1 eps_j - cL2 sig_j
+  m.cL2 = 2.0 * ZA * iZZB;
+  return m;
+}
+// per-column scalars p_j, c_j, Dq_j from eps_j = e_j - 1 and sig_j = S_j - A
+__device__ __forceinline__ void mcol(const MCoef& m, double eps, double sig, double& p, double& c, double& Dq) {
+  const double DZ = fma(m.zA2, sig, m.zBB * eps);
+  p = fma(-eps, m.zm1, DZ) + fma(m.q2, sig, -m.qA * eps);
+  c = -(DZ - m.B * eps) * m.invZmB;
+  Dq = fma(m.cL1, eps, -m.cL2 * sig) - m.q * eps;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Rachford-Rice with warm start.  theta on entry: previous solution (used if inside the sign bracket).
+// Returns false when there is no window.  Produces normalised x, y.
+// ------------------------------------------------------------------------------------------------
+template <int NC>
+__device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)[NC], double& theta, double (&x)[NC],
+                                        double (&y)[NC]) {
+  double Kmax = 0.0, Kmin = 1.0e300;
+  double km1[NC];
+  double f0 = 0.0, f1 = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    const bool a = z[i] > 0.0;
+    km1[i] = a ? K[i] - 1.0 : 0.0;
+    if (a) { Kmax = fmax(Kmax, K[i]); Kmin = fmin(Kmin, K[i]); }
+    f0 = fma(z[i], km1[i], f0);
+    f1 += z[i] * km1[i] / K[i];
+  }
+  if (!(Kmax > 1.0) || !(Kmin < 1.0)) return false;
+  const double al = 1.0 / (1.0 - Kmax), ar = 1.0 / (1.0 - Kmin);
+  double lo = al, hi = ar, th;
+  if (f0 > 0.0) {
+    if (f1 < 0.0) { lo = 0.0; hi = 1.0; th = f0 / (f0 - f1); }
+    else if (f1 == 0.0) { lo = hi = 1.0; th = 1.0; }
+    else { lo = 1.0; th = fmin(1.0 + 0.5 * (ar - 1.0), 2.0); }
+  } else if (f0 < 0.0) { hi = 0.0; th = fmax(0.5 * al, -1.0); }
+  else { lo = hi = 0.0; th = 0.0; }
+  if (theta > lo && theta < hi) th = theta;
+  if (!(th > lo && th < hi)) th = 0.5 * (lo + hi);
+  const double scale = 1.0e-8 * fmin(ar - al, 1.0);
+#pragma unroll 1
+  for (int it = 0; it < 100; ++it) {
+    if (!(hi > lo)) break;
+    double f = 0.0, df = 0.0;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      const double r = 1.0 / fma(km1[i], th, 1.0);
+      const double a = z[i] * km1[i] * r;
+      f += a;
+      df = fma(-a, km1[i] * r, df);
+    }
+    if (f > 0.0) lo = th; else if (f < 0.0) hi = th; else break;
+    const double u = th - al, w = ar - th;
+    const double h = u * w * f;
+    const double dh = (w - u) * f + u * w * df;
+    double tn = th - h / dh;
+    const bool inside = (tn > lo && tn < hi);
+    if (!inside) tn = 0.5 * (lo + hi);
+    const double step = fabs(tn - th);
+    th = tn;
+    if (inside && step <= scale) break;   // quadratic convergence: the applied step leaves an error ~ step^2
+    if (step <= 2.3e-16 * fabs(th)) break;
+  }
+  theta = th;
+  double sx = 0.0, sy = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    const double xi = (z[i] > 0.0) ? z[i] / fma(km1[i], th, 1.0) : 0.0;
+    x[i] = xi;
+    y[i] = K[i] * xi;
+    sx += xi;
+    sy += y[i];
+  }
+  const double isx = 1.0 / sx, isy = 1.0 / sy;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) { x[i] *= isx; y[i] *= isy; }
+  return true;
+}
+
+// ------------------------------------------------------------------------------------------------
+// In-register Cholesky of a packed symmetric matrix (lower triangle, compile-time indices) and solve
+// (L L^T) s = -g.  On exit Lm holds L with the INVERSE diagonal on the diagonal.  Returns false if not
+// positive definite.
+// ------------------------------------------------------------------------------------------------
+template <int NC>
+__device__ __forceinline__ bool chol_packed(double (&Lm)[NC * (NC + 1) / 2], const double (&g)[NC], double (&s)[NC]) {
+  bool pd = true;
+#pragma unroll
+  for (int j = 0; j < NC; ++j) {
+    double acc = Lm[tri(j, j)];
+#pragma unroll
+    for (int k = 0; k < j; ++k) acc = fma(-Lm[tri(j, k)], Lm[tri(j, k)], acc);
+    pd = pd && (acc > 0.0);
+    const double inv = rsqrt(acc);
+    Lm[tri(j, j)] = inv;
+#pragma unroll
+    for (int i = j + 1; i < NC; ++i) {
+      double a = Lm[tri(i, j)];
+#pragma unroll
+      for (int k = 0; k < j; ++k) a = fma(-Lm[tri(i, k)], Lm[tri(j, k)], a);
+      Lm[tri(i, j)] = a * inv;
+    }
+  }
+  double yv[NC];
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    double acc = -g[i];
+#pragma unroll
+    for (int k = 0; k < i; ++k) acc = fma(-Lm[tri(i, k)], yv[k], acc);
+    yv[i] = acc * Lm[tri(i, i)];
+  }
+#pragma unroll
+  for (int i = NC - 1; i >= 0; --i) {
+    double acc = yv[i];
+#pragma unroll
+    for (int k = i + 1; k < NC; ++k) acc = fma(-Lm[tri(k, i)], s[k], acc);
+    s[i] = acc * Lm[tri(i, i)];
+  }
+  return pd;
+}
+
+}  // namespace ptf

@@ -3,6 +3,7 @@
 #include "ptflash_launch.h"
 #include "ptflash_flash.cuh"
 #include "ptflash_staged.cuh"
+#include "ptflash_stage2.cuh"
 
 #ifndef PTF_NC
 #error "compile with -DPTF_NC=<2..16>"
@@ -30,6 +31,10 @@ int PTF_CAT(launch_mono_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io,
 }
 
 int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io, void* ws, cudaStream_t st) {
+  #if PTF_NC <= 12
+  // register-resident fast path (packed nc x nc systems fit the register file up to nc = 12)
+  if (o.use_newton) return launch_stage2<PTF_NC>(hs, o, io, ws, st);
+#endif
   return launch_staged<PTF_NC>(hs, o, io, ws, st);
 }
 

@@ -1,0 +1,786 @@
+// ptflash_stage2.cuh -- optimised stage kernels of engine 1 (see ptflash_staged.cuh for the pipeline).
+//
+//   k2_probe / k2_stab_ss / k2_split_ss   one work item per thread, iterate in registers, warm-started cubic and
+//                                         Rachford-Rice, everything inlined (no per-mixture struct in local memory)
+//   k2_stab_newton / k2_split_newton      persistent warps with LANE REFILL: every lane owns one work item; one loop
+//                                         trip = one trust-region iteration (one lnphi evaluation per phase + one
+//                                         packed in-register Cholesky); a lane whose item finishes stores it and
+//                                         pulls the next item from a global ticket (warp ballot + popc prefix), so
+//                                         early finishers do not stall their warp (north_star subsystem 4; the
+//                                         paper's per-iteration mask-and-compact, eq. 10).
+#pragma once
+#include "ptflash_fast.cuh"
+#include "ptflash_staged.cuh"
+
+namespace ptf {
+
+// per-(P,T) arrays + active mask of mixture n (already validated and normalised by k_init)
+template <int NC>
+__device__ __forceinline__ void load_pt(const Sys<NC>& S, const Io& io, int n, double (&sa)[NC], double (&bi)[NC], double& P,
+                                        double& T) {
+  P = io.P[n];
+  T = io.T[n];
+  eos_setup<NC>(S, P, T, sa, bi);
+}
+
+template <int NC>
+__device__ __forceinline__ void load_z(const Io& io, int n, double (&z)[NC]) {
+  double sz = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) { z[i] = io.z[(int64_t)i * io.N + n]; sz += z[i]; }
+#pragma unroll
+  for (int i = 0; i < NC; ++i) z[i] = z[i] / sz;
+}
+
+// one successive-substitution iteration of the phase split (Fig. 1): K = exp(lnK), RR, lnphi(x), lnphi(y),
+// lnK <- lnphi(x) - lnphi(y).  Returns false if Rachford-Rice has no window.  rk = max |d lnK|.
+template <int NC, bool KIJ0>
+__device__ __forceinline__ bool split_iteration(const Sys<NC>& S, const double (&sa)[NC], const double (&bi)[NC],
+                                                const double (&z)[NC], double (&lnK)[NC], double& theta, double (&x)[NC],
+                                                double (&y)[NC], double (&lpx)[NC], double (&lpy)[NC], double& Zx, double& Zy,
+                                                double& rk, bool update) {
+  double K[NC], Sv[NC];
+#pragma unroll
+  for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+  if (!rr_fast<NC>(K, z, theta, x, y)) return false;
+  if (!update) return true;
+  Eos e;
+  e.Z = Zx;
+  lnphi_fast<NC, KIJ0>(S, sa, bi, x, lpx, Sv, e);
+  Zx = e.Z;
+  e.Z = Zy;
+  lnphi_fast<NC, KIJ0>(S, sa, bi, y, lpy, Sv, e);
+  Zy = e.Z;
+  rk = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i)
+    if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = fmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
+  return true;
+}
+
+// ---- K1b: probe -----------------------------------------------------------------------------------
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(128) k2_probe(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_PROBE];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    int pcase = 0, n = 0;
+    if (in) {
+      n = w.q_probe[idx];
+      double sa[NC], bi[NC], z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
+      double P, T;
+      load_pt<NC>(S, io, n, sa, bi, P, T);
+      load_z<NC>(io, n, z);
+      int status = 0, fl = 0;
+      start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
+      double theta = -1.0e300, Zx = 0.0, Zy = 0.0, rk = 0.0;
+      int iters = 0;
+      pcase = 2;
+#pragma unroll 1
+      for (int it = 0; it < o.probe_iters; ++it) {
+        double K[NC];
+#pragma unroll
+        for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+        if (!rr_fast<NC>(K, z, theta, x, y) || !(theta > 0.0) || !(theta < 1.0)) { pcase = 1; break; }
+        Eos e;
+        double Sv[NC];
+        e.Z = Zx;
+        lnphi_fast<NC, KIJ0>(S, sa, bi, x, lpx, Sv, e);
+        Zx = e.Z;
+        e.Z = Zy;
+        lnphi_fast<NC, KIJ0>(S, sa, bi, y, lpy, Sv, e);
+        Zy = e.Z;
+#pragma unroll
+        for (int i = 0; i < NC; ++i)
+          if (z[i] > 0.0) lnK[i] = lpx[i] - lpy[i];
+        iters++;
+      }
+      (void)rk;
+      double tpd_min = 0.0;
+      if (pcase == 2 && o.probe_iters > 0) {
+        double tx = 0.0, ty = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          const double di = w.d[(int64_t)i * io.N + n];
+          if (x[i] > 0.0) tx = fma(x[i], log(x[i]) + lpx[i] - di, tx);
+          if (y[i] > 0.0) ty = fma(y[i], log(y[i]) + lpy[i] - di, ty);
+        }
+        const double dG = (1.0 - theta) * tx + theta * ty;
+        const double mn = fmin(dG, fmin(tx, ty));
+        if (mn < -o.probe_margin) { tpd_min = mn; pcase = 3; }
+      }
+      w.iters[n] = iters;
+      if (pcase == 3) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnK[i];
+        w.tpdmin[n] = tpd_min;
+      }
+    }
+    count_add(pcase == 1, &w.ctr->n_case1);
+    count_add(pcase == 2, &w.ctr->n_case2);
+    count_add(pcase == 3, &w.ctr->n_case3);
+    queue_push(pcase == 1 || pcase == 2, &w.qcount[Q_STAB], w.q_stab, n);
+    queue_push(pcase == 3, &w.qcount[Q_SPLIT], w.q_split, n);
+  }
+}
+
+// ---- K2: stability SS -----------------------------------------------------------------------------
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                  const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  const int64_t N = io.N;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    bool need_newton = false;
+    int item = 0;
+    if (in) {
+      const int n = w.q_stab[idx >> 1];
+      const int sidx = (int)(idx & 1);  // 0 vapour-like, 1 liquid-like
+      item = (n << 1) | sidx;
+      double sa[NC], bi[NC], lnW[NC], d[NC], W[NC], lp[NC], Sv[NC];
+      double P, T;
+      load_pt<NC>(S, io, n, sa, bi, P, T);
+      const unsigned act = (unsigned)w.actmask[n];
+      {
+        int status = 0, fl = 0;
+        double lnKs[NC];
+        start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
+        const double side = sidx ? -1.0 : 1.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          d[i] = w.d[(int64_t)i * N + n];
+          lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], w.lnz[(int64_t)i * N + n]) : 0.0;
+        }
+      }
+      Eos e;
+      e.Z = 0.0;
+      const int ss_max = o.use_newton ? o.stab_ss_iters : o.ss_cap;
+      bool converged = false, capped = false;
+      int iters = 0;
+      double tm = 0.0, sumW = 1.0;
+      auto eval = [&]() -> double {
+        sumW = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { W[i] = ((act >> i) & 1u) ? exp(lnW[i]) : 0.0; sumW += W[i]; }
+        const double inv = 1.0 / sumW;
+        double wn[NC];
+#pragma unroll
+        for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
+        lnphi_fast<NC, KIJ0>(S, sa, bi, wn, lp, Sv, e);
+        double rmax = 0.0;
+        tm = 1.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          const double r = ((act >> i) & 1u) ? lnW[i] + lp[i] - d[i] : 0.0;
+          rmax = fmax(rmax, fabs(r));
+          tm = fma(W[i], r - 1.0, tm);
+        }
+        return rmax;
+      };
+#pragma unroll 1
+      for (int k = 0; k < ss_max; ++k) {
+        const double rmax = eval();
+        if (rmax < o.tol_ss) { converged = true; break; }
+#pragma unroll
+        for (int i = 0; i < NC; ++i)
+          if ((act >> i) & 1u) lnW[i] = d[i] - lp[i];  // eq. 5
+        iters++;
+      }
+      if (!converged && !o.use_newton) { eval(); capped = true; }
+      need_newton = !converged && o.use_newton;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = lnW[i];
+      w.tm[(int64_t)sidx * N + n] = tm;
+      w.sumW[(int64_t)sidx * N + n] = sumW;
+      w.tflags[(int64_t)sidx * N + n] = (converged ? TF_CONVERGED : 0) | (capped ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
+    }
+    queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
+  }
+}
+
+// ---- lane refill ----------------------------------------------------------------------------------
+// Lanes with want == true take consecutive tickets; returns the ticket (>= total means the queue is exhausted).
+__device__ __forceinline__ int64_t take_ticket(bool want, int* __restrict__ ticket) {
+  const unsigned mask = __ballot_sync(0xffffffffu, want);
+  if (mask == 0u) return -1;
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(mask) - 1;
+  int base = 0;
+  if (lane == leader) base = atomicAdd(ticket, __popc(mask));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  return want ? (int64_t)base + __popc(mask & ((1u << lane) - 1u)) : -1;
+}
+
+// Trust-region bookkeeping shared by the two Newton kernels: the eta sequence of tr_subproblem() as a
+// resumable state machine, so the (large, fully unrolled) build-factor-solve body appears once in the code.
+struct EtaSearch {
+  double eta, eta_lo, eta_hi, eta0;
+  int phase, k;   // phase 0: eta = 0; 1: growing (x8); 2: geometric bisection; 3: done; 4: failed
+  __device__ __forceinline__ void start(double e0) { eta = 0.0; eta_lo = 0.0; eta_hi = 0.0; eta0 = e0; phase = 0; k = 0; }
+  // feed the outcome of the attempt at `eta`; returns true if `s` of this attempt should be kept
+  __device__ __forceinline__ bool feed(bool good, double sn, double Delta, double& kept_sn) {
+    bool keep = false;
+    if (phase == 0) {
+      if (good) { keep = true; kept_sn = sn; phase = 3; }
+      else { phase = 1; eta = eta0; k = 0; }
+    } else if (phase == 1) {
+      if (good) { keep = true; kept_sn = sn; eta_hi = eta; phase = 2; k = 0; }
+      else { eta_lo = eta; eta *= 8.0; if (++k >= 60) phase = 4; }
+    } else if (phase == 2) {
+      if (good) { keep = true; kept_sn = sn; eta_hi = eta; } else eta_lo = eta;
+      ++k;
+    }
+    if (phase == 2) {
+      if (kept_sn >= 0.5 * Delta || (eta_lo > 0.0 && eta_hi / eta_lo < 1.5) || k >= 12) phase = 3;
+      else eta = (eta_lo > 0.0) ? sqrt(eta_lo * eta_hi) : eta_hi * 0.125;
+    }
+    return keep;
+  }
+};
+
+// ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                      const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  constexpr int NT = NC * (NC + 1) / 2;
+  constexpr unsigned FULL = 0xffffffffu;
+  const int64_t N = io.N;
+  const int total = w.qcount[Q_STAB_NEWTON];
+  int* ticket = &w.qcount[Q_TICKET_STAB];
+  // ---- lane state ----
+  bool busy = false, exhausted = false, first = true, reeval = false;
+  int n = 0, sidx = 0, iters = 0, tr_it = 0;
+  unsigned act = 0u;
+  double spt = 0.0, sT = 0.0, pt = 0.0;   // sqrt(P)/T, sqrt(T), P/T: sqrt(A_i), B_i are rebuilt from constants
+  double beta[NC], s[NC];                 // accepted point (beta = 2 sqrt(W), B.1a) and pending step
+  double tm = 0.0, rmax_acc = 0.0, pred = 0.0, Delta = 1.0, Delta_cap = 8.0, snorm = 0.0, Zw = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) { beta[i] = 0.0; s[i] = 0.0; }
+
+#pragma unroll 1
+  while (true) {
+    // ---- refill idle lanes from the ticket ----
+    if (__any_sync(FULL, !busy && !exhausted)) {
+      const int64_t tk = take_ticket(!busy && !exhausted, ticket);
+      if (tk >= 0) {
+        if (tk < total) {
+          const int item = w.q_stab_newton[tk];
+          n = item >> 1;
+          sidx = item & 1;
+          const double P = io.P[n], T = io.T[n];
+          sT = sqrt(T);
+          spt = sqrt(P) / T;
+          pt = P / T;
+          act = (unsigned)w.actmask[n];
+#pragma unroll
+          for (int i = 0; i < NC; ++i) {
+            beta[i] = ((act >> i) & 1u) ? 2.0 * exp(0.5 * w.lnW[((int64_t)sidx * NC + i) * N + n]) : 0.0;
+            s[i] = 0.0;
+          }
+          iters = w.tflags[(int64_t)sidx * N + n] >> TF_ITER_SHIFT;
+          tr_it = 0;
+          first = true;
+          reeval = false;
+          Zw = 0.0;
+          busy = true;
+        } else {
+          exhausted = true;
+        }
+      }
+    }
+    if (!__any_sync(FULL, busy)) break;
+    if (!busy) continue;
+
+    // ---- evaluate tm and its gradient at the trial point beta + s ----
+    double sa[NC], bi[NC], W[NC], lp[NC], Sv[NC], r[NC];
+    double sumW = 0.0;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));
+      bi[i] = pt * S.wb[i];
+      const double h = 0.5 * (beta[i] + s[i]);
+      W[i] = h * h;                                          // B.1d
+      r[i] = ((act >> i) & 1u) ? 2.0 * log(h) : 0.0;         // ln W_i
+      sumW += W[i];
+    }
+    Eos e;
+    e.Z = Zw;
+    {
+      const double inv = 1.0 / sumW;
+      double wn[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
+      lnphi_fast<NC, KIJ0>(S, sa, bi, wn, lp, Sv, e);
+    }
+    Zw = e.Z;
+    double rmax = 0.0, tm_new = 1.0;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - w.d[(int64_t)i * N + n] : 0.0;
+      rmax = fmax(rmax, fabs(r[i]));
+      tm_new = fma(W[i], r[i] - 1.0, tm_new);
+    }
+    // ---- accept / reject the pending step (B.3) ----
+    bool accepted = true;
+    if (first) {
+      double bn = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) bn = fma(beta[i], beta[i], bn);
+      Delta = fmax(1.0, 0.5 * sqrt(bn));
+      Delta_cap = 8.0 * Delta;
+    } else if (!reeval) {
+      const double act_red = tm_new - tm;
+      accepted = (act_red < 0.0) || (rmax < rmax_acc);
+      if (accepted) {
+        if (fabs(pred) > 1.0e-13) {
+          const double ratio = fabs(act_red / pred);
+          if (ratio <= 0.25) Delta *= 0.5;
+          else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
+        }
+      } else {
+        Delta = 0.5 * fmin(Delta, snorm);
+        reeval = true;   // next trip re-evaluates at the accepted point (s = 0) and continues from there
+      }
+    }
+    if (!accepted) {
+#pragma unroll
+      for (int i = 0; i < NC; ++i) s[i] = 0.0;
+      continue;
+    }
+#pragma unroll
+    for (int i = 0; i < NC; ++i) { beta[i] += s[i]; s[i] = 0.0; }
+    tm = tm_new;
+    rmax_acc = rmax;
+    first = false;
+    reeval = false;
+
+    // ---- convergence / cap, else one trust-region iteration ----
+    bool finish = false, fin_conv = false, fin_exact = false, fin_cap = false;
+    if (rmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+    else if (tr_it >= o.stab_tr_iters) { finish = true; fin_cap = true; }
+    else {
+      tr_it++;
+      iters++;
+      const MCoef mc = mcoef(e);
+      const double isq = rsqrt(sumW);
+      double g[NC], st[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) g[i] = 0.5 * beta[i] * r[i];   // B.2a
+      EtaSearch es;
+      es.start(1.0e-3);
+      double kept_sn = 0.0;
+#pragma unroll 1
+      while (es.phase < 3) {
+        double Lm[NT];
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+          const double ej = bi[j] * mc.invB;
+          double pj, cj, Dqj;
+          mcol(mc, ej - 1.0, Sv[j] - mc.A, pj, cj, Dqj);
+          const double hj = 0.5 * beta[j] * isq;
+#pragma unroll
+          for (int i = j; i < NC; ++i) {
+            const double ei = bi[i] * mc.invB;
+            const double ui = fma(2.0, Sv[i], -mc.A * ei);
+            const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
+            const double Mij = fma(ei, pj, cj) - fma(Dqj, ui, mc.q2 * (Aij - Sv[i]));
+            const double hi_ = 0.5 * beta[i] * isq;
+            double hij = hi_ * hj * Mij;                                   // B.2b
+            if (i == j) hij += 1.0 + 0.5 * r[i] + es.eta;
+            Lm[tri(i, j)] = hij;
+          }
+        }
+        bool good = chol_packed<NC>(Lm, g, st);
+        double sn = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          sn = fma(st[i], st[i], sn);
+          if (((act >> i) & 1u) && !(beta[i] + st[i] > 0.0)) good = false;
+        }
+        sn = sqrt(sn);
+        good = good && (sn <= Delta);
+        const double eta_used = es.eta;
+        if (es.feed(good, sn, Delta, kept_sn)) {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) s[i] = st[i];
+          snorm = sn;
+          // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
+          double sg = 0.0;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) sg = fma(s[i], g[i], sg);
+          pred = 0.5 * sg - 0.5 * eta_used * sn * sn;
+          fin_exact = (eta_used == 0.0);
+        }
+      }
+      if (es.phase == 4) { finish = true; fin_cap = true; fin_exact = false; }
+      else {
+        double smax = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(s[i]));
+        if (fin_exact && smax < o.tol_newton_step) {
+          // quadratic-convergence finish: apply the full Newton step and stop
+          finish = true;
+          fin_conv = true;
+          sumW = 0.0;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) {
+            beta[i] += s[i];
+            const double h = 0.5 * beta[i];
+            sumW = fma(h, h, sumW);
+          }
+        } else fin_exact = false;
+      }
+    }
+    if (finish) {
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+        w.lnW[((int64_t)sidx * NC + i) * N + n] = ((act >> i) & 1u) ? 2.0 * log(0.5 * beta[i]) : 0.0;
+      w.tm[(int64_t)sidx * N + n] = tm;
+      w.sumW[(int64_t)sidx * N + n] = sumW;
+      w.tflags[(int64_t)sidx * N + n] = (fin_conv ? TF_CONVERGED : 0) | ((fin_conv && fin_exact) ? TF_EXACT : 0) |
+                                        (fin_cap ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
+      busy = false;
+    }
+  }
+}
+
+
+// ---- K5: phase-split SS ---------------------------------------------------------------------------
+template <int NC>
+__device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, const double (&z)[NC], bool converged,
+                                            bool failed, double theta, int st_iters, int st_status, const double (&x)[NC],
+                                            const double (&y)[NC], const double (&lnK)[NC]) {
+  int status = w.status[n] | st_status;
+  bool two = false;
+  if (failed) status |= ST_SPLIT_FAILED;
+  else if (converged && theta > 0.0 && theta < 1.0) two = true;
+  else status |= ST_SPLIT_FAILED;
+  store_result<NC>(io, n, two, theta, z, x, y, lnK, w.Zfeed[n], w.iters[n] + st_iters, status, w.tpdmin[n], w.stabit[n]);
+  count_add(two, &w.ctr->n_two_phase);
+}
+
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(128) k2_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                   const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t cnt = w.qcount[Q_SPLIT];
+  const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  const int64_t N = io.N;
+  PTF_GRID_STRIDE(idx, pad) {
+    const bool in = idx < cnt;
+    bool go_newton = false;
+    int n = 0;
+    if (in) {
+      n = w.q_split[idx];
+      double sa[NC], bi[NC], z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
+      double P, T;
+      load_pt<NC>(S, io, n, sa, bi, P, T);
+      load_z<NC>(io, n, z);
+#pragma unroll
+      for (int i = 0; i < NC; ++i) lnK[i] = w.lnK[(int64_t)i * N + n];
+      double theta = -1.0e300, Zx = 0.0, Zy = 0.0, r_prev = -1.0, rk = 0.0;
+      bool converged = false, failed = false;
+      int k = 0, status = 0;
+#pragma unroll 1
+      while (true) {
+        double mk = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i)
+          if (z[i] > 0.0) mk = fmax(mk, fabs(lnK[i]));
+        if (mk < 1.0e-9) { failed = true; break; }
+        const bool last_rr = o.use_newton && k >= o.split_ss_iters;
+        // Rachford-Rice first; the lnphi evaluations only if this is not the hand-over point
+        double K[NC];
+#pragma unroll
+        for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+        if (!rr_fast<NC>(K, z, theta, x, y)) { failed = true; break; }
+        if (last_rr && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
+        if (k >= o.ss_cap) { status |= ST_SPLIT_CAP; break; }
+        {
+          Eos e;
+          double Sv[NC];
+          e.Z = Zx;
+          lnphi_fast<NC, KIJ0>(S, sa, bi, x, lpx, Sv, e);
+          Zx = e.Z;
+          e.Z = Zy;
+          lnphi_fast<NC, KIJ0>(S, sa, bi, y, lpy, Sv, e);
+          Zy = e.Z;
+        }
+        rk = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i)
+          if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = fmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
+        ++k;
+        bool conv = false;
+        if (rk < 1.0e-14) conv = true;
+        else if (r_prev > 0.0 && rk < o.tol_ss) {
+          const double rho = rk / r_prev;
+          if (rho < 1.0 && rk * rho / (1.0 - rho) < o.tol_ss) conv = true;
+        }
+        r_prev = rk;
+        if (conv) {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+          if (!rr_fast<NC>(K, z, theta, x, y)) failed = true; else converged = true;
+          break;
+        }
+      }
+      if (go_newton) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = lnK[i];
+        w.iters[n] += k;
+        w.status[n] |= status;
+      } else {
+        store_split<NC>(io, w, n, z, converged, failed, theta, k, status, x, y, lnK);
+      }
+    }
+    queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
+  }
+}
+
+// ---- K6: phase-split trust-region Newton on G (B.4-B.5), persistent warps with lane refill --------
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                       const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  constexpr int NT = NC * (NC + 1) / 2;
+  constexpr unsigned FULL = 0xffffffffu;
+  const int64_t N = io.N;
+  const int total = w.qcount[Q_SPLIT_NEWTON];
+  int* ticket = &w.qcount[Q_TICKET_SPLIT];
+  bool busy = false, exhausted = false, first = true, reeval = false;
+  int n = 0, tr_it = 0, status = 0;
+  unsigned act = 0u;
+  double spt = 0.0, sT = 0.0, pt = 0.0;
+  double nV[NC], s[NC];   // accepted vapour mole numbers (B.4) and pending step
+  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, Zx = 0.0, Zy = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) { nV[i] = 0.0; s[i] = 0.0; }
+
+#pragma unroll 1
+  while (true) {
+    if (__any_sync(FULL, !busy && !exhausted)) {
+      const int64_t tk = take_ticket(!busy && !exhausted, ticket);
+      if (tk >= 0) {
+        if (tk < total) {
+          n = w.q_split_newton[tk];
+          const double P = io.P[n], T = io.T[n];
+          sT = sqrt(T);
+          spt = sqrt(P) / T;
+          pt = P / T;
+          act = (unsigned)w.actmask[n];
+          // the Rachford-Rice that ended the SS stage: n^V = theta y
+          double z[NC], K[NC], x[NC], y[NC];
+          load_z<NC>(io, n, z);
+#pragma unroll
+          for (int i = 0; i < NC; ++i) K[i] = exp(w.lnK[(int64_t)i * N + n]);
+          double theta = -1.0e300;
+          rr_fast<NC>(K, z, theta, x, y);
+#pragma unroll
+          for (int i = 0; i < NC; ++i) { nV[i] = fmin(theta * y[i], z[i]); s[i] = 0.0; }
+          tr_it = 0;
+          status = 0;
+          first = true;
+          reeval = false;
+          Delta = 0.25;
+          Zx = 0.0;
+          Zy = 0.0;
+          busy = true;
+        } else {
+          exhausted = true;
+        }
+      }
+    }
+    if (!__any_sync(FULL, busy)) break;
+    if (!busy) continue;
+
+    // ---- evaluate G (eq. 8) and its gradient (B.5a) at the trial point n^V + s ----
+    double sa[NC], bi[NC], z[NC], x[NC], y[NC], lp[NC], Sx[NC], Sy[NC], gt[NC];
+    load_z<NC>(io, n, z);
+    double theta = 0.0;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));
+      bi[i] = pt * S.wb[i];
+      theta += nV[i] + s[i];
+    }
+    {
+      const double it = 1.0 / theta, il = 1.0 / (1.0 - theta);
+#pragma unroll
+      for (int i = 0; i < NC; ++i) { const double v = nV[i] + s[i]; y[i] = v * it; x[i] = (z[i] - v) * il; }
+    }
+    Eos ex, ey;
+    ex.Z = Zx;
+    lnphi_fast<NC, KIJ0>(S, sa, bi, x, lp, Sx, ex);
+    Zx = ex.Z;
+    double G_new = 0.0, gmax = 0.0;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      double fx = 0.0;
+      if ((act >> i) & 1u) { fx = log(x[i]) + lp[i]; G_new = fma(z[i] - (nV[i] + s[i]), fx, G_new); }
+      gt[i] = -fx;
+    }
+    ey.Z = Zy;
+    lnphi_fast<NC, KIJ0>(S, sa, bi, y, lp, Sy, ey);
+    Zy = ey.Z;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      if ((act >> i) & 1u) { const double fy = log(y[i]) + lp[i]; G_new = fma(nV[i] + s[i], fy, G_new); gt[i] += fy; }
+      gmax = fmax(gmax, fabs(gt[i]));
+    }
+    // ---- accept / reject ----
+    bool accepted = true;
+    if (!first && !reeval) {
+      const double act_red = G_new - G;
+      accepted = (act_red < 0.0) || (gmax < gmax_acc);
+      if (accepted) {
+        if (fabs(pred) > 1.0e-13) {
+          const double ratio = fabs(act_red / pred);
+          if (ratio <= 0.25) Delta *= 0.5;
+          else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
+        }
+      } else {
+        Delta = 0.5 * fmin(Delta, snorm);
+        reeval = true;
+      }
+    }
+    if (!accepted) {
+#pragma unroll
+      for (int i = 0; i < NC; ++i) s[i] = 0.0;
+      continue;
+    }
+#pragma unroll
+    for (int i = 0; i < NC; ++i) { nV[i] += s[i]; s[i] = 0.0; }
+    G = G_new;
+    gmax_acc = gmax;
+    first = false;
+    reeval = false;
+
+    bool finish = false, fin_conv = false;
+    if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+    else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
+    else {
+      tr_it++;
+      const MCoef mx = mcoef(ex), my = mcoef(ey);
+      const double tt = theta * (1.0 - theta), itt = 1.0 / tt;
+      const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
+      double D[NC], st[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) D[i] = ((act >> i) & 1u) ? z[i] / (x[i] * y[i]) : 1.0;
+      EtaSearch es;
+      es.start(1.0e-3 * itt);
+      double kept_sn = 0.0;
+      bool exact = false;
+#pragma unroll 1
+      while (es.phase < 3) {
+        double Lm[NT];
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+          const double exj = bi[j] * mx.invB, eyj = bi[j] * my.invB;
+          double pxj, cxj, Dqxj, pyj, cyj, Dqyj;
+          mcol(mx, exj - 1.0, Sx[j] - mx.A, pxj, cxj, Dqxj);
+          mcol(my, eyj - 1.0, Sy[j] - my.A, pyj, cyj, Dqyj);
+          const bool aj = (act >> j) & 1u;
+#pragma unroll
+          for (int i = j; i < NC; ++i) {
+            const bool ai = (act >> i) & 1u;
+            const double exi = bi[i] * mx.invB, eyi = bi[i] * my.invB;
+            const double uxi = fma(2.0, Sx[i], -mx.A * exi), uyi = fma(2.0, Sy[i], -my.A * eyi);
+            const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
+            const double Mx = fma(exi, pxj, cxj) - fma(Dqxj, uxi, mx.q2 * (Aij - Sx[i]));
+            const double My = fma(eyi, pyj, cyj) - fma(Dqyj, uyi, my.q2 * (Aij - Sy[i]));
+            double hij = fma(wx, Mx, wy * My) - itt;                                  // B.5b
+            if (i == j) hij += D[i] * (itt + es.eta);                                // + eta D (B.4a)
+            if (!(ai && aj)) hij = (i == j) ? 1.0 : 0.0;
+            Lm[tri(i, j)] = hij;
+          }
+        }
+        bool good = chol_packed<NC>(Lm, gt, st);
+        double sn = 0.0, sds = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          sn = fma(st[i], st[i], sn);
+          sds = fma(st[i] * st[i], D[i], sds);
+          if ((act >> i) & 1u) {
+            const double nv = nV[i] + st[i];
+            if (!(nv > 0.0) || !(nv < z[i])) good = false;
+          }
+        }
+        sn = sqrt(sn);
+        good = good && (sn <= Delta);
+        const double eta_used = es.eta;
+        if (es.feed(good, sn, Delta, kept_sn)) {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) s[i] = st[i];
+          snorm = sn;
+          double sg = 0.0;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) sg = fma(s[i], gt[i], sg);
+          pred = 0.5 * sg - 0.5 * eta_used * sds;
+          exact = (eta_used == 0.0);
+        }
+      }
+      if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; }
+      else {
+        double smax = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(s[i]));
+        if (exact && smax < o.tol_newton_step) {
+          finish = true;
+          fin_conv = true;
+          theta = 0.0;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) { nV[i] += s[i]; theta += nV[i]; }
+          const double it = 1.0 / theta, il = 1.0 / (1.0 - theta);
+#pragma unroll
+          for (int i = 0; i < NC; ++i) { y[i] = nV[i] * it; x[i] = (z[i] - nV[i]) * il; }
+        }
+      }
+    }
+    if (finish) {
+      double lnK[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log(y[i]) - log(x[i]) : 0.0;
+      store_split<NC>(io, w, n, z, fin_conv, false, theta, tr_it, status, x, y, lnK);
+      busy = false;
+    }
+  }
+}
+
+template <int NC, bool KIJ0>
+int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work& w, int sms, cudaStream_t st) {
+  const int threads = 128;
+  auto grid_for = [&](int64_t items) {
+    const int64_t need = (items + threads - 1) / threads;
+    const int64_t cap = (int64_t)sms * 16;
+    return (unsigned)(need < cap ? (need > 0 ? need : 1) : cap);
+  };
+  const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
+  const unsigned gP = (unsigned)(sms * 4);   // persistent refill kernels: a few CTAs per SM pull tickets
+  k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+  k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
+  k2_stab_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
+  k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+  k2_split_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
+  k_finalize_counters<<<1, 32, 0, st>>>(w);
+  return cudaGetLastError() == cudaSuccess ? 8 : -1;
+}
+
+// engine 1 entry
+template <int NC>
+int launch_stage2(const SysHost& hs, const Opt& o, const Io& io, void* workspace, cudaStream_t st) {
+  const Sys<NC> s = narrow<NC>(hs);
+  Work w;
+  carve_workspace(NC, io.N, (char*)workspace, &w);
+  if (cudaMemsetAsync(workspace, 0, align256(sizeof(StageCounters)) + align256(Q_COUNT * sizeof(int)), st) != cudaSuccess) return -1;
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  return hs.kij_zero ? launch_stage2_impl<NC, true>(s, o, io, w, sms, st) : launch_stage2_impl<NC, false>(s, o, io, w, sms, st);
+}
+
+}  // namespace ptf

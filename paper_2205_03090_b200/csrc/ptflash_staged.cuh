@@ -24,7 +24,7 @@
 
 namespace ptf {
 
-enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_COUNT = 8 };
+enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_COUNT = 8 };
 enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_ITER_SHIFT = 8 };
 
 struct Work {
@@ -37,6 +37,7 @@ struct Work {
   double *Zfeed, *tpdmin;  // [N]
   int* tflags;             // [2][N]
   int *status, *iters, *stabit;  // [N]
+  int* actmask;            // [N] bit i set <=> z_i > 0
 };
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -66,6 +67,7 @@ inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   p = take(n * 4); if (w) w->status = (int*)p;
   p = take(n * 4); if (w) w->iters = (int*)p;
   p = take(n * 4); if (w) w->stabit = (int*)p;
+  p = take(n * 4); if (w) w->actmask = (int*)p;
   return off;
 }
 
@@ -137,6 +139,12 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
       w.status[n] = status;
       w.iters[n] = 0;
       w.stabit[n] = 0;
+      {
+        int am = 0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) am |= (m.z[i] > 0.0) ? (1 << i) : 0;
+        w.actmask[n] = am;
+      }
       if (have0 && (fl & 1)) {
         dest = 2;
 #pragma unroll
