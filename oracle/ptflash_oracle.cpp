@@ -27,9 +27,14 @@
 #include <algorithm>
 #ifdef ORACLE_TRACE
 #include <cstdio>
-#define TRACE(...) std::fprintf(stderr, __VA_ARGS__)
+#define TRACE(...) ((void)0)
+#include <atomic>
+static std::atomic<long long> g_trace_attempts[64], g_trace_calls;
+#define TRACE_ATTEMPTS(n) do { g_trace_calls++; g_trace_attempts[(n) < 63 ? (n) : 63]++; } while (0)
+extern "C" void orc_trace_dump() { std::fprintf(stderr, "tr_subproblem calls %lld; attempts histogram:", (long long)g_trace_calls.load()); for (int i = 0; i < 64; ++i) if (g_trace_attempts[i].load()) std::fprintf(stderr, " %d:%lld", i, (long long)g_trace_attempts[i].load()); std::fprintf(stderr, "\n"); }
 #else
 #define TRACE(...) ((void)0)
+#define TRACE_ATTEMPTS(n) ((void)0)
 #endif
 
 #ifndef ORACLE_REAL
@@ -372,7 +377,9 @@ static bool tr_subproblem(int n, real (*H)[MAXC], const real* g, const real* D, 
   real Hh[MAXC][MAXC], neg[MAXC], st[MAXC];
   for (int a = 0; a < n; ++a) neg[a] = -g[a];
   real sn = 0;
+  int nattempt = 0;
   auto attempt = [&](real eta) -> bool {
+    ++nattempt;
     for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) Hh[a][b] = H[a][b] + ((a == b) ? eta * D[a] : (real)0);
     if (!chol_solve(n, Hh, neg, st)) return false;
     sn = 0;
@@ -385,7 +392,7 @@ static bool tr_subproblem(int n, real (*H)[MAXC], const real* g, const real* D, 
     return sn <= Delta;
   };
   auto keep = [&](real eta) { for (int a = 0; a < n; ++a) s[a] = st[a]; *eta_out = eta; *snorm_out = sn; };
-  if (attempt((real)0)) { keep((real)0); return true; }
+  if (attempt((real)0)) { keep((real)0); TRACE_ATTEMPTS(nattempt); return true; }
   real eta_lo = 0, eta_hi = 0, eta = eta0;
   bool found = false;
   for (int k = 0; k < 60; ++k) {
@@ -399,6 +406,8 @@ static bool tr_subproblem(int n, real (*H)[MAXC], const real* g, const real* D, 
     real mid = (eta_lo > (real)0) ? r_sqrt(eta_lo * eta_hi) : eta_hi / (real)8;
     if (attempt(mid)) { eta_hi = mid; keep(mid); } else eta_lo = mid;
   }
+  TRACE_ATTEMPTS(nattempt);
+  (void)nattempt;
   return true;
 }
 

@@ -10,6 +10,7 @@
 //   * symmetric nc x nc systems live in registers as a packed lower triangle with compile-time indices.
 #pragma once
 #include "ptflash_device.cuh"
+#include "ptflash_math.cuh"
 
 namespace ptf {
 
@@ -66,10 +67,10 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
     if (ra > B) { zmin = fmin(zmin, ra); zmax = fmax(zmax, ra); }
     if (rb > B) { zmin = fmin(zmin, rb); zmax = fmax(zmax, rb); }
   }
-  double lz = log(zmin - B), ll = log1p(B / zmin);
+  double lz = log_fast(zmin - B), ll = log1p_fast(B * rcp_fast(zmin));
   if (zmax != zmin) {
-    const double AoB = A / B;
-    const double lz2 = log(zmax - B), ll2 = log1p(B / zmax);
+    const double AoB = A * rcp_fast(B);
+    const double lz2 = log_fast(zmax - B), ll2 = log1p_fast(B * rcp_fast(zmax));
     const double gl = zmin - 1.0 - lz - AoB * ll;
     const double gv = zmax - 1.0 - lz2 - AoB * ll2;
     if (gv < gl) { zmin = zmax; lz = lz2; ll = ll2; }
@@ -116,7 +117,7 @@ __device__ __forceinline__ void lnphi_fast(const Sys<NC>& S, const double (&sa)[
   e.A = A;
   e.B = B;
   e.Z = pick_root_fast(A, B, e.Z, e.lnZmB, e.L);
-  const double invB = 1.0 / B;
+  const double invB = rcp_fast(B);
   e.q = e.L * invB;
   const double zm1 = e.Z - 1.0;
 #pragma unroll
@@ -198,7 +199,7 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     double f = 0.0, df = 0.0;
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
-      const double r = 1.0 / fma(km1[i], th, 1.0);
+      const double r = rcp_fast(fma(km1[i], th, 1.0));
       const double a = z[i] * km1[i] * r;
       f += a;
       df = fma(-a, km1[i] * r, df);

@@ -41,7 +41,7 @@ __device__ __forceinline__ bool split_iteration(const Sys<NC>& S, const double (
                                                 double& rk, bool update) {
   double K[NC], Sv[NC];
 #pragma unroll
-  for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+  for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
   if (!rr_fast<NC>(K, z, theta, x, y)) return false;
   if (!update) return true;
   Eos e;
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(128) k2_probe(const __grid_constant__ Sys<NC> 
       for (int it = 0; it < o.probe_iters; ++it) {
         double K[NC];
 #pragma unroll
-        for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+        for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
         if (!rr_fast<NC>(K, z, theta, x, y) || !(theta > 0.0) || !(theta < 1.0)) { pcase = 1; break; }
         Eos e;
         double Sv[NC];
@@ -104,8 +104,8 @@ __global__ void __launch_bounds__(128) k2_probe(const __grid_constant__ Sys<NC> 
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           const double di = w.d[(int64_t)i * io.N + n];
-          if (x[i] > 0.0) tx = fma(x[i], log(x[i]) + lpx[i] - di, tx);
-          if (y[i] > 0.0) ty = fma(y[i], log(y[i]) + lpy[i] - di, ty);
+          if (x[i] > 0.0) tx = fma(x[i], log_fast(x[i]) + lpx[i] - di, tx);
+          if (y[i] > 0.0) ty = fma(y[i], log_fast(y[i]) + lpy[i] - di, ty);
         }
         const double dG = (1.0 - theta) * tx + theta * ty;
         const double mn = fmin(dG, fmin(tx, ty));
@@ -165,8 +165,8 @@ __global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC
       auto eval = [&]() -> double {
         sumW = 0.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) { W[i] = ((act >> i) & 1u) ? exp(lnW[i]) : 0.0; sumW += W[i]; }
-        const double inv = 1.0 / sumW;
+        for (int i = 0; i < NC; ++i) { W[i] = ((act >> i) & 1u) ? exp_fast(lnW[i]) : 0.0; sumW += W[i]; }
+        const double inv = rcp_fast(sumW);
         double wn[NC];
 #pragma unroll
         for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
@@ -193,7 +193,9 @@ __global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC
       if (!converged && !o.use_newton) { eval(); capped = true; }
       need_newton = !converged && o.use_newton;
 #pragma unroll
-      for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = lnW[i];
+      for (int i = 0; i < NC; ++i)
+        w.lnW[((int64_t)sidx * NC + i) * N + n] =
+            need_newton ? (((act >> i) & 1u) ? 2.0 * exp_fast(0.5 * lnW[i]) : 0.0) : lnW[i];   // Newton works in beta = 2 sqrt(W) (B.1a)
       w.tm[(int64_t)sidx * N + n] = tm;
       w.sumW[(int64_t)sidx * N + n] = sumW;
       w.tflags[(int64_t)sidx * N + n] = (converged ? TF_CONVERGED : 0) | (capped ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
@@ -252,12 +254,14 @@ __global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sy
   const int total = w.qcount[Q_STAB_NEWTON];
   int* ticket = &w.qcount[Q_TICKET_STAB];
   // ---- lane state ----
-  bool busy = false, exhausted = false, first = true, reeval = false;
+  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
   int n = 0, sidx = 0, iters = 0, tr_it = 0;
   unsigned act = 0u;
   double spt = 0.0, sT = 0.0, pt = 0.0;   // sqrt(P)/T, sqrt(T), P/T: sqrt(A_i), B_i are rebuilt from constants
-  double beta[NC], s[NC];                 // accepted point (beta = 2 sqrt(W), B.1a) and pending step
-  double tm = 0.0, rmax_acc = 0.0, pred = 0.0, Delta = 1.0, Delta_cap = 8.0, snorm = 0.0, Zw = 0.0;
+  double beta[NC], s[NC];                 // accepted point (beta = 2 sqrt(W), B.1a) and pending / best-so-far step
+  double tm = 0.0, rmax_acc = 0.0, pred = 0.0, Delta = 1.0, Delta_cap = 8.0, snorm = 0.0, Zw = 0.0, kept_sn = 0.0;
+  EtaSearch es;
+  es.start(1.0e-3);
 #pragma unroll
   for (int i = 0; i < NC; ++i) { beta[i] = 0.0; s[i] = 0.0; }
 
@@ -278,13 +282,14 @@ __global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sy
           act = (unsigned)w.actmask[n];
 #pragma unroll
           for (int i = 0; i < NC; ++i) {
-            beta[i] = ((act >> i) & 1u) ? 2.0 * exp(0.5 * w.lnW[((int64_t)sidx * NC + i) * N + n]) : 0.0;
+            beta[i] = w.lnW[((int64_t)sidx * NC + i) * N + n];   // k2_stab_ss left beta = 2 sqrt(W) here
             s[i] = 0.0;
           }
           iters = w.tflags[(int64_t)sidx * N + n] >> TF_ITER_SHIFT;
           tr_it = 0;
           first = true;
           reeval = false;
+          searching = false;
           Zw = 0.0;
           busy = true;
         } else {
@@ -293,24 +298,28 @@ __global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sy
       }
     }
     if (!__any_sync(FULL, busy)) break;
-    if (!busy) continue;
 
-    // ---- evaluate tm and its gradient at the trial point beta + s ----
+    // The trip below is written WITHOUT early `continue`s and with explicit __syncwarp() joins: the factorisation
+    // block must be entered once per trip by all searching lanes together (a divergent entry makes the warp run
+    // the ~1500-instruction block twice with half the lanes each).
     double sa[NC], bi[NC], W[NC], lp[NC], Sv[NC], r[NC];
     double sumW = 0.0;
+    Eos e;
+    e.Z = Zw;
+    bool finish = false, fin_conv = false, fin_exact = false, fin_cap = false;
+    if (busy) {
+    // ---- evaluate tm and its gradient: at the trial point beta + s, or at beta while an eta search is pending ----
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
       sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));
       bi[i] = pt * S.wb[i];
-      const double h = 0.5 * (beta[i] + s[i]);
-      W[i] = h * h;                                          // B.1d
-      r[i] = ((act >> i) & 1u) ? 2.0 * log(h) : 0.0;         // ln W_i
+      const double h = 0.5 * (searching ? beta[i] : beta[i] + s[i]);
+      W[i] = h * h;                                              // B.1d
+      r[i] = ((act >> i) & 1u) ? 2.0 * log_fast(h) : 0.0;        // ln W_i
       sumW += W[i];
     }
-    Eos e;
-    e.Z = Zw;
     {
-      const double inv = 1.0 / sumW;
+      const double inv = rcp_fast(sumW);
       double wn[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
@@ -324,107 +333,110 @@ __global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sy
       rmax = fmax(rmax, fabs(r[i]));
       tm_new = fma(W[i], r[i] - 1.0, tm_new);
     }
-    // ---- accept / reject the pending step (B.3) ----
-    bool accepted = true;
-    if (first) {
-      double bn = 0.0;
+    if (!searching) {
+      // ---- accept / reject the pending step (B.3) ----
+      bool accepted = true;
+      if (first) {
+        double bn = 0.0;
 #pragma unroll
-      for (int i = 0; i < NC; ++i) bn = fma(beta[i], beta[i], bn);
-      Delta = fmax(1.0, 0.5 * sqrt(bn));
-      Delta_cap = 8.0 * Delta;
-    } else if (!reeval) {
-      const double act_red = tm_new - tm;
-      accepted = (act_red < 0.0) || (rmax < rmax_acc);
-      if (accepted) {
-        if (fabs(pred) > 1.0e-13) {
-          const double ratio = fabs(act_red / pred);
-          if (ratio <= 0.25) Delta *= 0.5;
-          else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
+        for (int i = 0; i < NC; ++i) bn = fma(beta[i], beta[i], bn);
+        Delta = fmax(1.0, 0.5 * sqrt(bn));
+        Delta_cap = 8.0 * Delta;
+      } else if (!reeval) {
+        const double act_red = tm_new - tm;
+        accepted = (act_red < 0.0) || (rmax < rmax_acc);
+        if (accepted) {
+          if (fabs(pred) > 1.0e-13) {
+            const double ratio = fabs(act_red / pred);
+            if (ratio <= 0.25) Delta *= 0.5;
+            else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
+          }
+        } else {
+          Delta = 0.5 * fmin(Delta, snorm);
+          reeval = true;   // next trip re-evaluates at the accepted point (s = 0) and continues from there
         }
+      }
+      if (!accepted) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) s[i] = 0.0;
       } else {
-        Delta = 0.5 * fmin(Delta, snorm);
-        reeval = true;   // next trip re-evaluates at the accepted point (s = 0) and continues from there
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { beta[i] += s[i]; s[i] = 0.0; }
+        tm = tm_new;
+        rmax_acc = rmax;
+        first = false;
+        reeval = false;
+        // ---- convergence / cap, else start the eta search of a new trust-region iteration ----
+        if (rmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+        else if (tr_it >= o.stab_tr_iters) { finish = true; fin_cap = true; }
+        else {
+          tr_it++;
+          iters++;
+          es.start(1.0e-3);
+          kept_sn = 0.0;
+          searching = true;
+        }
       }
     }
-    if (!accepted) {
-#pragma unroll
-      for (int i = 0; i < NC; ++i) s[i] = 0.0;
-      continue;
-    }
-#pragma unroll
-    for (int i = 0; i < NC; ++i) { beta[i] += s[i]; s[i] = 0.0; }
-    tm = tm_new;
-    rmax_acc = rmax;
-    first = false;
-    reeval = false;
-
-    // ---- convergence / cap, else one trust-region iteration ----
-    bool finish = false, fin_conv = false, fin_exact = false, fin_cap = false;
-    if (rmax < o.tol_newton_g) { finish = true; fin_conv = true; }
-    else if (tr_it >= o.stab_tr_iters) { finish = true; fin_cap = true; }
-    else {
-      tr_it++;
-      iters++;
+    }  // busy
+    __syncwarp();
+    if (busy && searching) {
+      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.1b): build H + eta I, factor, solve ----
       const MCoef mc = mcoef(e);
       const double isq = rsqrt(sumW);
       double g[NC], st[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) g[i] = 0.5 * beta[i] * r[i];   // B.2a
-      EtaSearch es;
-      es.start(1.0e-3);
-      double kept_sn = 0.0;
-#pragma unroll 1
-      while (es.phase < 3) {
-        double Lm[NT];
+      double Lm[NT];
 #pragma unroll
-        for (int j = 0; j < NC; ++j) {
-          const double ej = bi[j] * mc.invB;
-          double pj, cj, Dqj;
-          mcol(mc, ej - 1.0, Sv[j] - mc.A, pj, cj, Dqj);
-          const double hj = 0.5 * beta[j] * isq;
+      for (int j = 0; j < NC; ++j) {
+        const double ej = bi[j] * mc.invB;
+        double pj, cj, Dqj;
+        mcol(mc, ej - 1.0, Sv[j] - mc.A, pj, cj, Dqj);
+        const double hj = 0.5 * beta[j] * isq;
 #pragma unroll
-          for (int i = j; i < NC; ++i) {
-            const double ei = bi[i] * mc.invB;
-            const double ui = fma(2.0, Sv[i], -mc.A * ei);
-            const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
-            const double Mij = fma(ei, pj, cj) - fma(Dqj, ui, mc.q2 * (Aij - Sv[i]));
-            const double hi_ = 0.5 * beta[i] * isq;
-            double hij = hi_ * hj * Mij;                                   // B.2b
-            if (i == j) hij += 1.0 + 0.5 * r[i] + es.eta;
-            Lm[tri(i, j)] = hij;
-          }
-        }
-        bool good = chol_packed<NC>(Lm, g, st);
-        double sn = 0.0;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) {
-          sn = fma(st[i], st[i], sn);
-          if (((act >> i) & 1u) && !(beta[i] + st[i] > 0.0)) good = false;
-        }
-        sn = sqrt(sn);
-        good = good && (sn <= Delta);
-        const double eta_used = es.eta;
-        if (es.feed(good, sn, Delta, kept_sn)) {
-#pragma unroll
-          for (int i = 0; i < NC; ++i) s[i] = st[i];
-          snorm = sn;
-          // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
-          double sg = 0.0;
-#pragma unroll
-          for (int i = 0; i < NC; ++i) sg = fma(s[i], g[i], sg);
-          pred = 0.5 * sg - 0.5 * eta_used * sn * sn;
-          fin_exact = (eta_used == 0.0);
+        for (int i = j; i < NC; ++i) {
+          const double ei = bi[i] * mc.invB;
+          const double ui = fma(2.0, Sv[i], -mc.A * ei);
+          const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
+          const double Mij = fma(ei, pj, cj) - fma(Dqj, ui, mc.q2 * (Aij - Sv[i]));
+          const double hi_ = 0.5 * beta[i] * isq;
+          double hij = hi_ * hj * Mij;                                   // B.2b
+          if (i == j) hij += 1.0 + 0.5 * r[i] + es.eta;
+          Lm[tri(i, j)] = hij;
         }
       }
-      if (es.phase == 4) { finish = true; fin_cap = true; fin_exact = false; }
-      else {
+      bool good = chol_packed<NC>(Lm, g, st);
+      double sn = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        sn = fma(st[i], st[i], sn);
+        if (((act >> i) & 1u) && !(beta[i] + st[i] > 0.0)) good = false;
+      }
+      sn = sqrt(sn);
+      good = good && (sn <= Delta);
+      const double eta_used = es.eta;
+      if (es.feed(good, sn, Delta, kept_sn)) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) s[i] = st[i];
+        snorm = sn;
+        double sg = 0.0;   // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
+#pragma unroll
+        for (int i = 0; i < NC; ++i) sg = fma(s[i], g[i], sg);
+        pred = 0.5 * sg - 0.5 * eta_used * sn * sn;
+        exact = (eta_used == 0.0);
+      }
+      if (es.phase == 4) { finish = true; fin_cap = true; searching = false; }
+      else if (es.phase == 3) {
+        searching = false;
         double smax = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(s[i]));
-        if (fin_exact && smax < o.tol_newton_step) {
+        if (exact && smax < o.tol_newton_step) {
           // quadratic-convergence finish: apply the full Newton step and stop
           finish = true;
           fin_conv = true;
+          fin_exact = true;
           sumW = 0.0;
 #pragma unroll
           for (int i = 0; i < NC; ++i) {
@@ -432,22 +444,22 @@ __global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sy
             const double h = 0.5 * beta[i];
             sumW = fma(h, h, sumW);
           }
-        } else fin_exact = false;
+        }
       }
     }
+    __syncwarp();
     if (finish) {
+      // beta is stored; k_stab_decide turns it into ln W = 2 ln(beta/2) with all lanes active (TF_BETA)
 #pragma unroll
-      for (int i = 0; i < NC; ++i)
-        w.lnW[((int64_t)sidx * NC + i) * N + n] = ((act >> i) & 1u) ? 2.0 * log(0.5 * beta[i]) : 0.0;
+      for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = beta[i];
       w.tm[(int64_t)sidx * N + n] = tm;
       w.sumW[(int64_t)sidx * N + n] = sumW;
-      w.tflags[(int64_t)sidx * N + n] = (fin_conv ? TF_CONVERGED : 0) | ((fin_conv && fin_exact) ? TF_EXACT : 0) |
-                                        (fin_cap ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
+      w.tflags[(int64_t)sidx * N + n] = (fin_conv ? TF_CONVERGED : 0) | (fin_exact ? TF_EXACT : 0) |
+                                        (fin_cap ? TF_CAPPED : 0) | TF_BETA | (iters << TF_ITER_SHIFT);
       busy = false;
     }
   }
 }
-
 
 // ---- K5: phase-split SS ---------------------------------------------------------------------------
 template <int NC>
@@ -495,7 +507,7 @@ __global__ void __launch_bounds__(128) k2_split_ss(const __grid_constant__ Sys<N
         // Rachford-Rice first; the lnphi evaluations only if this is not the hand-over point
         double K[NC];
 #pragma unroll
-        for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+        for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
         if (!rr_fast<NC>(K, z, theta, x, y)) { failed = true; break; }
         if (last_rr && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
         if (k >= o.ss_cap) { status |= ST_SPLIT_CAP; break; }
@@ -523,7 +535,7 @@ __global__ void __launch_bounds__(128) k2_split_ss(const __grid_constant__ Sys<N
         r_prev = rk;
         if (conv) {
 #pragma unroll
-          for (int i = 0; i < NC; ++i) K[i] = exp(lnK[i]);
+          for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
           if (!rr_fast<NC>(K, z, theta, x, y)) failed = true; else converged = true;
           break;
         }
@@ -550,12 +562,14 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
   const int64_t N = io.N;
   const int total = w.qcount[Q_SPLIT_NEWTON];
   int* ticket = &w.qcount[Q_TICKET_SPLIT];
-  bool busy = false, exhausted = false, first = true, reeval = false;
+  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
   int n = 0, tr_it = 0, status = 0;
   unsigned act = 0u;
   double spt = 0.0, sT = 0.0, pt = 0.0;
-  double nV[NC], s[NC];   // accepted vapour mole numbers (B.4) and pending step
-  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, Zx = 0.0, Zy = 0.0;
+  double nV[NC], s[NC];   // accepted vapour mole numbers (B.4) and pending / best-so-far step
+  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, Zx = 0.0, Zy = 0.0, kept_sn = 0.0;
+  EtaSearch es;
+  es.start(1.0);
 #pragma unroll
   for (int i = 0; i < NC; ++i) { nV[i] = 0.0; s[i] = 0.0; }
 
@@ -575,7 +589,7 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
           double z[NC], K[NC], x[NC], y[NC];
           load_z<NC>(io, n, z);
 #pragma unroll
-          for (int i = 0; i < NC; ++i) K[i] = exp(w.lnK[(int64_t)i * N + n]);
+          for (int i = 0; i < NC; ++i) K[i] = exp_fast(w.lnK[(int64_t)i * N + n]);
           double theta = -1.0e300;
           rr_fast<NC>(K, z, theta, x, y);
 #pragma unroll
@@ -584,6 +598,7 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
           status = 0;
           first = true;
           reeval = false;
+          searching = false;
           Delta = 0.25;
           Zx = 0.0;
           Zy = 0.0;
@@ -594,24 +609,27 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
       }
     }
     if (!__any_sync(FULL, busy)) break;
-    if (!busy) continue;
 
-    // ---- evaluate G (eq. 8) and its gradient (B.5a) at the trial point n^V + s ----
     double sa[NC], bi[NC], z[NC], x[NC], y[NC], lp[NC], Sx[NC], Sy[NC], gt[NC];
-    load_z<NC>(io, n, z);
     double theta = 0.0;
+    Eos ex, ey;
+    bool finish = false, fin_conv = false;
+    if (busy) {
+    // ---- evaluate G (eq. 8) and its gradient (B.5a): at n^V + s, or at n^V while an eta search is pending ----
+    load_z<NC>(io, n, z);
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
       sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));
       bi[i] = pt * S.wb[i];
-      theta += nV[i] + s[i];
+      const double v = searching ? nV[i] : nV[i] + s[i];
+      y[i] = v;
+      theta += v;
     }
     {
-      const double it = 1.0 / theta, il = 1.0 / (1.0 - theta);
+      const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
 #pragma unroll
-      for (int i = 0; i < NC; ++i) { const double v = nV[i] + s[i]; y[i] = v * it; x[i] = (z[i] - v) * il; }
+      for (int i = 0; i < NC; ++i) { const double v = y[i]; y[i] = v * it; x[i] = (z[i] - v) * il; }
     }
-    Eos ex, ey;
     ex.Z = Zx;
     lnphi_fast<NC, KIJ0>(S, sa, bi, x, lp, Sx, ex);
     Zx = ex.Z;
@@ -619,7 +637,7 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
       double fx = 0.0;
-      if ((act >> i) & 1u) { fx = log(x[i]) + lp[i]; G_new = fma(z[i] - (nV[i] + s[i]), fx, G_new); }
+      if ((act >> i) & 1u) { fx = log_fast(x[i]) + lp[i]; G_new = fma(x[i] * (1.0 - theta), fx, G_new); }
       gt[i] = -fx;
     }
     ey.Z = Zy;
@@ -627,103 +645,105 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
     Zy = ey.Z;
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
-      if ((act >> i) & 1u) { const double fy = log(y[i]) + lp[i]; G_new = fma(nV[i] + s[i], fy, G_new); gt[i] += fy; }
+      if ((act >> i) & 1u) { const double fy = log_fast(y[i]) + lp[i]; G_new = fma(y[i] * theta, fy, G_new); gt[i] += fy; }
       gmax = fmax(gmax, fabs(gt[i]));
     }
-    // ---- accept / reject ----
-    bool accepted = true;
-    if (!first && !reeval) {
-      const double act_red = G_new - G;
-      accepted = (act_red < 0.0) || (gmax < gmax_acc);
-      if (accepted) {
-        if (fabs(pred) > 1.0e-13) {
-          const double ratio = fabs(act_red / pred);
-          if (ratio <= 0.25) Delta *= 0.5;
-          else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
+    if (!searching) {
+      // ---- accept / reject ----
+      bool accepted = true;
+      if (!first && !reeval) {
+        const double act_red = G_new - G;
+        accepted = (act_red < 0.0) || (gmax < gmax_acc);
+        if (accepted) {
+          if (fabs(pred) > 1.0e-13) {
+            const double ratio = fabs(act_red / pred);
+            if (ratio <= 0.25) Delta *= 0.5;
+            else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
+          }
+        } else {
+          Delta = 0.5 * fmin(Delta, snorm);
+          reeval = true;
         }
+      }
+      if (!accepted) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) s[i] = 0.0;
       } else {
-        Delta = 0.5 * fmin(Delta, snorm);
-        reeval = true;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { nV[i] += s[i]; s[i] = 0.0; }
+        G = G_new;
+        gmax_acc = gmax;
+        first = false;
+        reeval = false;
+        if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+        else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
+        else {
+          tr_it++;
+          es.start(1.0e-3 / (theta * (1.0 - theta)));
+          kept_sn = 0.0;
+          searching = true;
+        }
       }
     }
-    if (!accepted) {
-#pragma unroll
-      for (int i = 0; i < NC; ++i) s[i] = 0.0;
-      continue;
-    }
-#pragma unroll
-    for (int i = 0; i < NC; ++i) { nV[i] += s[i]; s[i] = 0.0; }
-    G = G_new;
-    gmax_acc = gmax;
-    first = false;
-    reeval = false;
-
-    bool finish = false, fin_conv = false;
-    if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
-    else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
-    else {
-      tr_it++;
+    }  // busy
+    __syncwarp();
+    if (busy && searching) {
+      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.4a) ----
       const MCoef mx = mcoef(ex), my = mcoef(ey);
       const double tt = theta * (1.0 - theta), itt = 1.0 / tt;
       const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
       double D[NC], st[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) D[i] = ((act >> i) & 1u) ? z[i] / (x[i] * y[i]) : 1.0;
-      EtaSearch es;
-      es.start(1.0e-3 * itt);
-      double kept_sn = 0.0;
-      bool exact = false;
-#pragma unroll 1
-      while (es.phase < 3) {
-        double Lm[NT];
+      double Lm[NT];
 #pragma unroll
-        for (int j = 0; j < NC; ++j) {
-          const double exj = bi[j] * mx.invB, eyj = bi[j] * my.invB;
-          double pxj, cxj, Dqxj, pyj, cyj, Dqyj;
-          mcol(mx, exj - 1.0, Sx[j] - mx.A, pxj, cxj, Dqxj);
-          mcol(my, eyj - 1.0, Sy[j] - my.A, pyj, cyj, Dqyj);
-          const bool aj = (act >> j) & 1u;
+      for (int j = 0; j < NC; ++j) {
+        const double exj = bi[j] * mx.invB, eyj = bi[j] * my.invB;
+        double pxj, cxj, Dqxj, pyj, cyj, Dqyj;
+        mcol(mx, exj - 1.0, Sx[j] - mx.A, pxj, cxj, Dqxj);
+        mcol(my, eyj - 1.0, Sy[j] - my.A, pyj, cyj, Dqyj);
+        const bool aj = (act >> j) & 1u;
 #pragma unroll
-          for (int i = j; i < NC; ++i) {
-            const bool ai = (act >> i) & 1u;
-            const double exi = bi[i] * mx.invB, eyi = bi[i] * my.invB;
-            const double uxi = fma(2.0, Sx[i], -mx.A * exi), uyi = fma(2.0, Sy[i], -my.A * eyi);
-            const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
-            const double Mx = fma(exi, pxj, cxj) - fma(Dqxj, uxi, mx.q2 * (Aij - Sx[i]));
-            const double My = fma(eyi, pyj, cyj) - fma(Dqyj, uyi, my.q2 * (Aij - Sy[i]));
-            double hij = fma(wx, Mx, wy * My) - itt;                                  // B.5b
-            if (i == j) hij += D[i] * (itt + es.eta);                                // + eta D (B.4a)
-            if (!(ai && aj)) hij = (i == j) ? 1.0 : 0.0;
-            Lm[tri(i, j)] = hij;
-          }
-        }
-        bool good = chol_packed<NC>(Lm, gt, st);
-        double sn = 0.0, sds = 0.0;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) {
-          sn = fma(st[i], st[i], sn);
-          sds = fma(st[i] * st[i], D[i], sds);
-          if ((act >> i) & 1u) {
-            const double nv = nV[i] + st[i];
-            if (!(nv > 0.0) || !(nv < z[i])) good = false;
-          }
-        }
-        sn = sqrt(sn);
-        good = good && (sn <= Delta);
-        const double eta_used = es.eta;
-        if (es.feed(good, sn, Delta, kept_sn)) {
-#pragma unroll
-          for (int i = 0; i < NC; ++i) s[i] = st[i];
-          snorm = sn;
-          double sg = 0.0;
-#pragma unroll
-          for (int i = 0; i < NC; ++i) sg = fma(s[i], gt[i], sg);
-          pred = 0.5 * sg - 0.5 * eta_used * sds;
-          exact = (eta_used == 0.0);
+        for (int i = j; i < NC; ++i) {
+          const bool ai = (act >> i) & 1u;
+          const double exi = bi[i] * mx.invB, eyi = bi[i] * my.invB;
+          const double uxi = fma(2.0, Sx[i], -mx.A * exi), uyi = fma(2.0, Sy[i], -my.A * eyi);
+          const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
+          const double Mx = fma(exi, pxj, cxj) - fma(Dqxj, uxi, mx.q2 * (Aij - Sx[i]));
+          const double My = fma(eyi, pyj, cyj) - fma(Dqyj, uyi, my.q2 * (Aij - Sy[i]));
+          double hij = fma(wx, Mx, wy * My) - itt;                                  // B.5b
+          if (i == j) hij += D[i] * (itt + es.eta);                                // + eta D (B.4a)
+          if (!(ai && aj)) hij = (i == j) ? 1.0 : 0.0;
+          Lm[tri(i, j)] = hij;
         }
       }
-      if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; }
-      else {
+      bool good = chol_packed<NC>(Lm, gt, st);
+      double sn = 0.0, sds = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        sn = fma(st[i], st[i], sn);
+        sds = fma(st[i] * st[i], D[i], sds);
+        if ((act >> i) & 1u) {
+          const double nv = nV[i] + st[i];
+          if (!(nv > 0.0) || !(nv < z[i])) good = false;
+        }
+      }
+      sn = sqrt(sn);
+      good = good && (sn <= Delta);
+      const double eta_used = es.eta;
+      if (es.feed(good, sn, Delta, kept_sn)) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) s[i] = st[i];
+        snorm = sn;
+        double sg = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) sg = fma(s[i], gt[i], sg);
+        pred = 0.5 * sg - 0.5 * eta_used * sds;
+        exact = (eta_used == 0.0);
+      }
+      if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
+      else if (es.phase == 3) {
+        searching = false;
         double smax = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(s[i]));
@@ -739,10 +759,11 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
         }
       }
     }
+    __syncwarp();
     if (finish) {
       double lnK[NC];
 #pragma unroll
-      for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log(y[i]) - log(x[i]) : 0.0;
+      for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
       store_split<NC>(io, w, n, z, fin_conv, false, theta, tr_it, status, x, y, lnK);
       busy = false;
     }

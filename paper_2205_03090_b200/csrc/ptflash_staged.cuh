@@ -21,11 +21,12 @@
 #pragma once
 #include "ptflash_flash.cuh"
 #include "ptflash_launch.h"
+#include "ptflash_math.cuh"
 
 namespace ptf {
 
 enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_COUNT = 8 };
-enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_ITER_SHIFT = 8 };
+enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_BETA = 8, TF_ITER_SHIFT = 8 + 0 };
 
 struct Work {
   StageCounters* ctr;
@@ -295,6 +296,15 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
 #pragma unroll
       for (int i = 0; i < NC; ++i) { sv.lnW[i] = w.lnW[(int64_t)i * N + n]; sl.lnW[i] = w.lnW[((int64_t)NC + i) * N + n]; }
       const int fv = w.tflags[n], fl_ = w.tflags[N + n];
+      // trials finished by the Newton stage come back as beta = 2 sqrt(W) (B.1a): ln W = 2 ln(beta / 2)
+      if (fv & TF_BETA) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) sv.lnW[i] = (m.z[i] > 0.0) ? 2.0 * log_fast(0.5 * sv.lnW[i]) : 0.0;
+      }
+      if (fl_ & TF_BETA) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) sl.lnW[i] = (m.z[i] > 0.0) ? 2.0 * log_fast(0.5 * sl.lnW[i]) : 0.0;
+      }
       sv.tm = w.tm[n]; sv.sumW = w.sumW[n]; sv.iters = fv >> TF_ITER_SHIFT;
       sv.converged = fv & TF_CONVERGED; sv.stationary_exact = fv & TF_EXACT; sv.capped = fv & TF_CAPPED;
       sl.tm = w.tm[N + n]; sl.sumW = w.sumW[N + n]; sl.iters = fl_ >> TF_ITER_SHIFT;
