@@ -127,6 +127,68 @@ __device__ __forceinline__ void lnphi_fast(const Sys<NC>& S, const double (&sa)[
   }
 }
 
+// Register-lean variant: sqrt(A_i) and B_i are rebuilt from three per-mixture scalars (sqrt(P)/T, sqrt(T), P/T)
+// and the per-component constants in the constant bank instead of living in 2 nc registers.
+template <int NC>
+struct PT3 { double spt, sT, pt; };
+template <int NC>
+__device__ __forceinline__ double sa_of(const Sys<NC>& S, const PT3<NC>& q, int i) { return q.spt * fabs(fma(-S.v[i], q.sT, S.u[i])); }
+template <int NC>
+__device__ __forceinline__ double bi_of(const Sys<NC>& S, const PT3<NC>& q, int i) { return q.pt * S.wb[i]; }
+
+template <int NC, bool KIJ0>
+__device__ __forceinline__ void lnphi_pt(const Sys<NC>& S, const PT3<NC>& q, const double (&c)[NC], double (&lp)[NC],
+                                         double (&Sv)[NC], Eos& e) {
+  double t[NC];
+  double B = 0.0;
+#pragma unroll
+  for (int j = 0; j < NC; ++j) { t[j] = sa_of<NC>(S, q, j) * c[j]; B = fma(c[j], bi_of<NC>(S, q, j), B); }
+  if (KIJ0) {
+    double sum = 0.0;
+#pragma unroll
+    for (int j = 0; j < NC; ++j) sum += t[j];
+#pragma unroll
+    for (int i = 0; i < NC; ++i) Sv[i] = sa_of<NC>(S, q, i) * sum;
+  } else {
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+      for (int j = 0; j < NC; j += 2) {
+        a0 = fma(S.omk[i * NC + j], t[j], a0);
+        if (j + 1 < NC) a1 = fma(S.omk[i * NC + j + 1], t[j + 1], a1);
+      }
+      Sv[i] = sa_of<NC>(S, q, i) * (a0 + a1);
+    }
+  }
+  double A0 = 0.0, A1 = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; i += 2) {
+    A0 = fma(c[i], Sv[i], A0);
+    if (i + 1 < NC) A1 = fma(c[i + 1], Sv[i + 1], A1);
+  }
+  const double A = A0 + A1;
+  e.A = A;
+  e.B = B;
+  e.Z = pick_root_fast(A, B, e.Z, e.lnZmB, e.L);
+  const double invB = rcp_fast(B);
+  e.q = e.L * invB;
+  const double zm1 = e.Z - 1.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    const double b = bi_of<NC>(S, q, i) * invB;
+    lp[i] = fma(b, zm1, -e.lnZmB) - e.q * fma(2.0, Sv[i], -A * b);
+  }
+}
+
+// Out-of-line copy for kernels that evaluate two phases per trip (x and y): one body instead of two keeps the
+// loop inside the instruction cache; the five small arrays travel through (L1-resident) local memory.
+template <int NC, bool KIJ0>
+__device__ __noinline__ void lnphi_call(const Sys<NC>& S, const double (&sa)[NC], const double (&bi)[NC],
+                                        const double (&c)[NC], double (&lp)[NC], double (&Sv)[NC], Eos& e) {
+  lnphi_fast<NC, KIJ0>(S, sa, bi, c, lp, Sv, e);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Coefficients of M_ij = n dlnphi_i/dn_j (unit total moles) in the form
 //   M_ij = e_i p_j + c_j - Dq_j u_i + 2q (S_i - A_ij),   e_i = B_i/B, u_i = 2 S_i - A e_i

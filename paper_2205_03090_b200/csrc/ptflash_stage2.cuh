@@ -127,9 +127,14 @@ __global__ void __launch_bounds__(128) k2_probe(const __grid_constant__ Sys<NC> 
 }
 
 // ---- K2: stability SS -----------------------------------------------------------------------------
+// Register-lean: the only per-component state kept across iterations is ln W; d is re-read from the workspace
+// (L1/L2 resident) and sqrt(A_i), B_i are rebuilt from three scalars, so four CTAs of 128 threads fit per SM.
+#ifndef PTF_SS_MINB
+#define PTF_SS_MINB 4
+#endif
 template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                  const __grid_constant__ Io io, const __grid_constant__ Work w) {
+__global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                               const __grid_constant__ Io io, const __grid_constant__ Work w) {
   const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
@@ -141,9 +146,12 @@ __global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC
       const int n = w.q_stab[idx >> 1];
       const int sidx = (int)(idx & 1);  // 0 vapour-like, 1 liquid-like
       item = (n << 1) | sidx;
-      double sa[NC], bi[NC], lnW[NC], d[NC], W[NC], lp[NC], Sv[NC];
-      double P, T;
-      load_pt<NC>(S, io, n, sa, bi, P, T);
+      double lnW[NC], W[NC], lp[NC], Sv[NC];
+      const double P = io.P[n], T = io.T[n];
+      PT3<NC> q;
+      q.sT = sqrt(T);
+      q.spt = sqrt(P) / T;
+      q.pt = P / T;
       const unsigned act = (unsigned)w.actmask[n];
       {
         int status = 0, fl = 0;
@@ -151,10 +159,7 @@ __global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC
         start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
         const double side = sidx ? -1.0 : 1.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) {
-          d[i] = w.d[(int64_t)i * N + n];
-          lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], w.lnz[(int64_t)i * N + n]) : 0.0;
-        }
+        for (int i = 0; i < NC; ++i) lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], w.lnz[(int64_t)i * N + n]) : 0.0;
       }
       Eos e;
       e.Z = 0.0;
@@ -162,35 +167,44 @@ __global__ void __launch_bounds__(128) k2_stab_ss(const __grid_constant__ Sys<NC
       bool converged = false, capped = false;
       int iters = 0;
       double tm = 0.0, sumW = 1.0;
-      auto eval = [&]() -> double {
+#pragma unroll 1
+      for (int k = 0; k <= ss_max; ++k) {
+        // evaluate the residual r = ln W + lnphi(w) - d at the current iterate
         sumW = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) { W[i] = ((act >> i) & 1u) ? exp_fast(lnW[i]) : 0.0; sumW += W[i]; }
-        const double inv = rcp_fast(sumW);
-        double wn[NC];
+        {
+          const double inv = rcp_fast(sumW);
+          double wn[NC];
 #pragma unroll
-        for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
-        lnphi_fast<NC, KIJ0>(S, sa, bi, wn, lp, Sv, e);
+          for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
+          lnphi_pt<NC, KIJ0>(S, q, wn, lp, Sv, e);
+        }
         double rmax = 0.0;
         tm = 1.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
-          const double r = ((act >> i) & 1u) ? lnW[i] + lp[i] - d[i] : 0.0;
+          // lp <- d - lnphi (the next iterate of eq. 5); r = ln W - (d - lnphi)
+          lp[i] = __ldg(&w.d[(int64_t)i * N + n]) - lp[i];
+          const double r = ((act >> i) & 1u) ? lnW[i] - lp[i] : 0.0;
           rmax = fmax(rmax, fabs(r));
           tm = fma(W[i], r - 1.0, tm);
         }
-        return rmax;
-      };
-#pragma unroll 1
-      for (int k = 0; k < ss_max; ++k) {
-        const double rmax = eval();
         if (rmax < o.tol_ss) { converged = true; break; }
+        if (k == ss_max) { capped = !o.use_newton; break; }   // the last pass only evaluates (pure-SS mode reports the cap)
+        if (k == ss_max - 1 && o.use_newton) {
+          // hand-over to the Newton stage after ss_max updates: no further evaluation needed here
+#pragma unroll
+          for (int i = 0; i < NC; ++i)
+            if ((act >> i) & 1u) lnW[i] = lp[i];
+          iters++;
+          break;
+        }
 #pragma unroll
         for (int i = 0; i < NC; ++i)
-          if ((act >> i) & 1u) lnW[i] = d[i] - lp[i];  // eq. 5
+          if ((act >> i) & 1u) lnW[i] = lp[i];  // eq. 5
         iters++;
       }
-      if (!converged && !o.use_newton) { eval(); capped = true; }
       need_newton = !converged && o.use_newton;
 #pragma unroll
       for (int i = 0; i < NC; ++i)
@@ -541,8 +555,9 @@ __global__ void __launch_bounds__(128) k2_split_ss(const __grid_constant__ Sys<N
         }
       }
       if (go_newton) {
+        // hand-over in the Newton variables: n^V_i = theta y_i (B.4)
 #pragma unroll
-        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = lnK[i];
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = fmin(theta * y[i], z[i]);
         w.iters[n] += k;
         w.status[n] |= status;
       } else {
@@ -585,15 +600,9 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
           spt = sqrt(P) / T;
           pt = P / T;
           act = (unsigned)w.actmask[n];
-          // the Rachford-Rice that ended the SS stage: n^V = theta y
-          double z[NC], K[NC], x[NC], y[NC];
-          load_z<NC>(io, n, z);
+          // k2_split_ss left n^V = theta y of its last Rachford-Rice here
 #pragma unroll
-          for (int i = 0; i < NC; ++i) K[i] = exp_fast(w.lnK[(int64_t)i * N + n]);
-          double theta = -1.0e300;
-          rr_fast<NC>(K, z, theta, x, y);
-#pragma unroll
-          for (int i = 0; i < NC; ++i) { nV[i] = fmin(theta * y[i], z[i]); s[i] = 0.0; }
+          for (int i = 0; i < NC; ++i) { nV[i] = w.lnK[(int64_t)i * N + n]; s[i] = 0.0; }
           tr_it = 0;
           status = 0;
           first = true;
@@ -631,7 +640,7 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
       for (int i = 0; i < NC; ++i) { const double v = y[i]; y[i] = v * it; x[i] = (z[i] - v) * il; }
     }
     ex.Z = Zx;
-    lnphi_fast<NC, KIJ0>(S, sa, bi, x, lp, Sx, ex);
+    lnphi_call<NC, KIJ0>(S, sa, bi, x, lp, Sx, ex);
     Zx = ex.Z;
     double G_new = 0.0, gmax = 0.0;
 #pragma unroll
@@ -641,7 +650,7 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
       gt[i] = -fx;
     }
     ey.Z = Zy;
-    lnphi_fast<NC, KIJ0>(S, sa, bi, y, lp, Sy, ey);
+    lnphi_call<NC, KIJ0>(S, sa, bi, y, lp, Sy, ey);
     Zy = ey.Z;
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
@@ -762,8 +771,13 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
     __syncwarp();
     if (finish) {
       double lnK[NC];
+      if (io.lnK) {
 #pragma unroll
-      for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
+        for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
+      } else {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
+      }
       store_split<NC>(io, w, n, z, fin_conv, false, theta, tr_it, status, x, y, lnK);
       busy = false;
     }
@@ -779,7 +793,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     return (unsigned)(need < cap ? (need > 0 ? need : 1) : cap);
   };
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
-  const unsigned gP = (unsigned)(sms * 4);   // persistent refill kernels: a few CTAs per SM pull tickets
+  const unsigned gP = (unsigned)(sms * 2);   // persistent refill kernels: a few CTAs per SM pull tickets
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
   k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
   k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
