@@ -24,12 +24,9 @@ __device__ __forceinline__ void load_pt(const Sys<NC>& S, const Io& io, int n, d
 }
 
 template <int NC>
-__device__ __forceinline__ void load_z(const Io& io, int n, double (&z)[NC]) {
-  double sz = 0.0;
+__device__ __forceinline__ void load_zn(const Io& io, const Work& w, int n, double (&z)[NC]) {
 #pragma unroll
-  for (int i = 0; i < NC; ++i) { z[i] = io.z[(int64_t)i * io.N + n]; sz += z[i]; }
-#pragma unroll
-  for (int i = 0; i < NC; ++i) z[i] = z[i] / sz;
+  for (int i = 0; i < NC; ++i) z[i] = __ldg(&w.zn[(int64_t)i * io.N + n]);   // normalised once by k_init
 }
 
 // one successive-substitution iteration of the phase split (Fig. 1): K = exp(lnK), RR, lnphi(x), lnphi(y),
@@ -59,9 +56,12 @@ __device__ __forceinline__ bool split_iteration(const Sys<NC>& S, const double (
 }
 
 // ---- K1b: probe -----------------------------------------------------------------------------------
+#ifndef PTF_SPLIT_MINB
+#define PTF_SPLIT_MINB 3
+#endif
 template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128) k2_probe(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
+__global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
   const int64_t cnt = w.qcount[Q_PROBE];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   PTF_GRID_STRIDE(idx, pad) {
@@ -69,41 +69,45 @@ __global__ void __launch_bounds__(128) k2_probe(const __grid_constant__ Sys<NC> 
     int pcase = 0, n = 0;
     if (in) {
       n = w.q_probe[idx];
-      double sa[NC], bi[NC], z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
-      double P, T;
-      load_pt<NC>(S, io, n, sa, bi, P, T);
-      load_z<NC>(io, n, z);
+      double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
+      const double P = io.P[n], T = io.T[n];
+      PT3<NC> q;
+      q.sT = sqrt(T);
+      q.spt = sqrt(P) / T;
+      q.pt = P / T;
+      load_zn<NC>(io, w, n, z);
       int status = 0, fl = 0;
       start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
-      double theta = -1.0e300, Zx = 0.0, Zy = 0.0, rk = 0.0;
+      double theta = -1.0e300, Zx = 0.0, Zy = 0.0;
       int iters = 0;
       pcase = 2;
 #pragma unroll 1
       for (int it = 0; it < o.probe_iters; ++it) {
-        double K[NC];
+        {
+          double K[NC];
 #pragma unroll
-        for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
-        if (!rr_fast<NC>(K, z, theta, x, y) || !(theta > 0.0) || !(theta < 1.0)) { pcase = 1; break; }
+          for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
+          if (!rr_fast<NC>(K, z, theta, x, y) || !(theta > 0.0) || !(theta < 1.0)) { pcase = 1; break; }
+        }
         Eos e;
         double Sv[NC];
         e.Z = Zx;
-        lnphi_fast<NC, KIJ0>(S, sa, bi, x, lpx, Sv, e);
+        lnphi_pt<NC, KIJ0>(S, q, x, lpx, Sv, e);
         Zx = e.Z;
         e.Z = Zy;
-        lnphi_fast<NC, KIJ0>(S, sa, bi, y, lpy, Sv, e);
+        lnphi_pt<NC, KIJ0>(S, q, y, lpy, Sv, e);
         Zy = e.Z;
 #pragma unroll
         for (int i = 0; i < NC; ++i)
           if (z[i] > 0.0) lnK[i] = lpx[i] - lpy[i];
         iters++;
       }
-      (void)rk;
       double tpd_min = 0.0;
       if (pcase == 2 && o.probe_iters > 0) {
         double tx = 0.0, ty = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
-          const double di = w.d[(int64_t)i * io.N + n];
+          const double di = __ldg(&w.d[(int64_t)i * io.N + n]);
           if (x[i] > 0.0) tx = fma(x[i], log_fast(x[i]) + lpx[i] - di, tx);
           if (y[i] > 0.0) ty = fma(y[i], log_fast(y[i]) + lpy[i] - di, ty);
         }
@@ -490,8 +494,8 @@ __device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, 
 }
 
 template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128) k2_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                   const __grid_constant__ Io io, const __grid_constant__ Work w) {
+__global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+                                                                   const __grid_constant__ Io io, const __grid_constant__ Work w) {
   const int64_t cnt = w.qcount[Q_SPLIT];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
@@ -501,58 +505,57 @@ __global__ void __launch_bounds__(128) k2_split_ss(const __grid_constant__ Sys<N
     int n = 0;
     if (in) {
       n = w.q_split[idx];
-      double sa[NC], bi[NC], z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
-      double P, T;
-      load_pt<NC>(S, io, n, sa, bi, P, T);
-      load_z<NC>(io, n, z);
+      double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
+      const double P = io.P[n], T = io.T[n];
+      PT3<NC> q;
+      q.sT = sqrt(T);
+      q.spt = sqrt(P) / T;
+      q.pt = P / T;
+      load_zn<NC>(io, w, n, z);
 #pragma unroll
       for (int i = 0; i < NC; ++i) lnK[i] = w.lnK[(int64_t)i * N + n];
-      double theta = -1.0e300, Zx = 0.0, Zy = 0.0, r_prev = -1.0, rk = 0.0;
-      bool converged = false, failed = false;
+      double theta = -1.0e300, Zx = 0.0, Zy = 0.0, r_prev = -1.0;
+      bool converged = false, failed = false, final_rr = false;
       int k = 0, status = 0;
+      // One copy of exp + Rachford-Rice + the two lnphi evaluations: the Rachford-Rice that makes x, y consistent with
+      // the converged lnK is the top of one more trip (final_rr).
 #pragma unroll 1
       while (true) {
         double mk = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i)
           if (z[i] > 0.0) mk = fmax(mk, fabs(lnK[i]));
-        if (mk < 1.0e-9) { failed = true; break; }
-        const bool last_rr = o.use_newton && k >= o.split_ss_iters;
-        // Rachford-Rice first; the lnphi evaluations only if this is not the hand-over point
-        double K[NC];
+        if (mk < 1.0e-9) { failed = true; break; }   // trivial collapse
+        {
+          double K[NC];
 #pragma unroll
-        for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
-        if (!rr_fast<NC>(K, z, theta, x, y)) { failed = true; break; }
-        if (last_rr && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
+          for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
+          if (!rr_fast<NC>(K, z, theta, x, y)) { failed = true; break; }
+        }
+        if (final_rr) { converged = true; break; }
+        if (o.use_newton && k >= o.split_ss_iters && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
         if (k >= o.ss_cap) { status |= ST_SPLIT_CAP; break; }
         {
           Eos e;
           double Sv[NC];
           e.Z = Zx;
-          lnphi_fast<NC, KIJ0>(S, sa, bi, x, lpx, Sv, e);
+          lnphi_pt<NC, KIJ0>(S, q, x, lpx, Sv, e);
           Zx = e.Z;
           e.Z = Zy;
-          lnphi_fast<NC, KIJ0>(S, sa, bi, y, lpy, Sv, e);
+          lnphi_pt<NC, KIJ0>(S, q, y, lpy, Sv, e);
           Zy = e.Z;
         }
-        rk = 0.0;
+        double rk = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i)
           if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = fmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
         ++k;
-        bool conv = false;
-        if (rk < 1.0e-14) conv = true;
+        if (rk < 1.0e-14) final_rr = true;
         else if (r_prev > 0.0 && rk < o.tol_ss) {
-          const double rho = rk / r_prev;
-          if (rho < 1.0 && rk * rho / (1.0 - rho) < o.tol_ss) conv = true;
+          const double rho = rk / r_prev;   // linear-convergence error estimate eps = r rho / (1 - rho)
+          if (rho < 1.0 && rk * rho / (1.0 - rho) < o.tol_ss) final_rr = true;
         }
         r_prev = rk;
-        if (conv) {
-#pragma unroll
-          for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
-          if (!rr_fast<NC>(K, z, theta, x, y)) failed = true; else converged = true;
-          break;
-        }
       }
       if (go_newton) {
         // hand-over in the Newton variables: n^V_i = theta y_i (B.4)
@@ -625,7 +628,7 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
     bool finish = false, fin_conv = false;
     if (busy) {
     // ---- evaluate G (eq. 8) and its gradient (B.5a): at n^V + s, or at n^V while an eta search is pending ----
-    load_z<NC>(io, n, z);
+    load_zn<NC>(io, w, n, z);
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
       sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));

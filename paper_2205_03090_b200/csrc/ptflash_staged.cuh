@@ -33,6 +33,7 @@ struct Work {
   int* qcount;  // [Q_COUNT]
   int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton;
   double *lnz, *d, *lnK;   // [NC][N]
+  double* zn;              // [NC][N] normalised feed z / sum z (written once by k_init)
   double* lnW;             // [2][NC][N]
   double *tm, *sumW;       // [2][N]
   double *Zfeed, *tpdmin;  // [N]
@@ -59,6 +60,7 @@ inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   p = take(c * n * 8); if (w) w->lnz = (double*)p;
   p = take(c * n * 8); if (w) w->d = (double*)p;
   p = take(c * n * 8); if (w) w->lnK = (double*)p;
+  p = take(c * n * 8); if (w) w->zn = (double*)p;
   p = take(2 * c * n * 8); if (w) w->lnW = (double*)p;
   p = take(2 * n * 8); if (w) w->tm = (double*)p;
   p = take(2 * n * 8); if (w) w->sumW = (double*)p;
@@ -135,6 +137,7 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
       for (int i = 0; i < NC; ++i) {
         w.lnz[(int64_t)i * io.N + n] = m.lnz[i];
         w.d[(int64_t)i * io.N + n] = m.d[i];
+        w.zn[(int64_t)i * io.N + n] = m.z[i];
       }
       w.Zfeed[n] = Zf;
       w.status[n] = status;
