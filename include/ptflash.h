@@ -48,6 +48,7 @@ typedef struct ptflash_handle_s* ptflash_handle_t;
 #define PTFLASH_ST_BAND 4          /* 0 < |tpd_min| < band (1e-9): label decided inside the near-zero TPD band */
 #define PTFLASH_ST_SPLIT_FAILED 8  /* "unstable" verdict but the split ended trivial or with beta outside (0,1): reported as single phase */
 #define PTFLASH_ST_LNK0_REJECTED 32 /* caller-supplied lnK0 non-finite or |lnK0| > 700: Wilson used instead */
+#define PTFLASH_ST_WARM_RESTART 64  /* PTFLASH_FLAG_SKIP_STABILITY split did not reach two phases: hint dropped, mixture re-flashed from Wilson with the full stability analysis */
 
 /* flags[n] bits for ptflash_flash_ex (interface effect of the paper's classifier/initializer, section 4.3
  * caller-supplied K estimates and a "known unstable" verdict) */

@@ -27,7 +27,11 @@
 #include <algorithm>
 #ifdef ORACLE_TRACE
 #include <cstdio>
+#ifdef ORACLE_TRACE_PRINT
+#define TRACE(...) std::fprintf(stderr, __VA_ARGS__)
+#else
 #define TRACE(...) ((void)0)
+#endif
 #include <atomic>
 static std::atomic<long long> g_trace_attempts[64], g_trace_calls;
 #define TRACE_ATTEMPTS(n) do { g_trace_calls++; g_trace_attempts[(n) < 63 ? (n) : 63]++; } while (0)
@@ -82,7 +86,7 @@ static Opts opts_from(const double* p) {
 }
 
 // status bits (same meaning as include/ptflash.h but defined independently)
-enum { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_RR = 16 };
+enum { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_RR = 16, ST_WARM_RESTART = 64 };
 
 // ------------------------------------------------------------------------------------------------
 // O1 Setup: dimensionless SRK groups.  PAPER.md:412-434 (A.2a-g, A.3).  R never appears:
@@ -687,6 +691,10 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
     }
     if (!converged) { if (gmax < (real)o.tol_newton_g) converged = true; else out.status |= ST_SPLIT_CAP; }
     for (int i = 0; i < nc; ++i) lnK[i] = (z[i] > (real)0) ? r_log(y[i]) - r_log(x[i]) : lnK[i];
+    // the Newton iteration can also slide into the trivial solution x = y (G is flat there): same test as in the SS loop
+    real mkn = 0;
+    for (int i = 0; i < nc; ++i) if (z[i] > (real)0) mkn = std::max(mkn, r_abs(lnK[i]));
+    if (mkn < (real)1e-9) failed = true;
   }
 
   out.theta = theta;
@@ -808,6 +816,17 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
       out.phase = 2; out.beta = sp.theta;
       for (int i = 0; i < nc; ++i) { out.x[i] = sp.x[i]; out.y[i] = sp.y[i]; out.lnK[i] = sp.lnK[i]; }
     } else if (!(sp.status & ST_SPLIT_FAILED)) out.status |= ST_SPLIT_FAILED;
+  }
+  if (!two && skip_stab) {
+    // The caller's "known unstable + lnK0" hint did not lead to a two-phase solution (trivial collapse, theta outside
+    // (0,1) or an iteration cap -- cf. the initializer-only failure reported at PAPER.md:363).  The hint is dropped and
+    // the mixture is flashed again from Wilson with the full stability analysis; the restart is reported (reading C21).
+    FlashOut cold;
+    flash_one(nc, Tc, Pc, omega, kij, P, T, z_in, nullptr, 0, o, cold);
+    cold.iters += out.iters;
+    cold.status |= ST_WARM_RESTART;
+    out = cold;
+    return;
   }
   if (!two) {
     // single phase: x = y = z, beta = 1 iff Z_feed > 1/3 (convention)

@@ -50,7 +50,8 @@ struct Io {
   int32_t *status, *stab_iters;
 };
 
-enum : int { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_LNK0_REJECTED = 32 };
+enum : int { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_LNK0_REJECTED = 32, ST_WARM_RESTART = 64,
+              ST_INTERNAL_SKIPPED = 128 /* workspace only: mixture entered the split through PTFLASH_FLAG_SKIP_STABILITY */ };
 
 struct Eos {
   double A, B, Z, L, q, lnZmB;

@@ -386,9 +386,11 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
     }
   }
   if (!converged) { if (gmax < o.tol_newton_g) converged = true; else st.status |= ST_SPLIT_CAP; }
+  double mkn = 0.0;
 #pragma unroll
   for (int i = 0; i < NC; ++i)
-    if (act[i]) st.lnK[i] = log(y[i]) - log(x[i]);
+    if (act[i]) { st.lnK[i] = log(y[i]) - log(x[i]); mkn = fmax(mkn, fabs(st.lnK[i])); }
+  if (mkn < 1.0e-9) st.failed = true;   // Newton slid into the trivial solution x = y
   st.converged = converged;
   st.theta = theta;
 }
@@ -459,6 +461,7 @@ __device__ __forceinline__ bool start_lnK(const Sys<NC>& S, const Io& io, int64_
                                           int& fl, int& status) {
   wilson_lnK<NC>(S, P, T, lnKs);
   fl = (io.flags && io.lnK0) ? io.flags[n] : 0;
+  if (status & ST_WARM_RESTART) fl = 0;   // the caller's hint was dropped for this mixture
   if (!(fl & 3)) return false;
   double l0[NC];
   bool have0 = true;
@@ -578,44 +581,52 @@ __device__ void flash_one(const Sys<NC>& S, const Opt& o, const Io& io, int64_t 
   if (!load_feed<NC>(io, n, m.z, P, T)) { store_invalid<NC>(io, n); return; }
   feed_reference<NC>(S, P, T, m, Zf);
   const double nan = __longlong_as_double(0x7ff8000000000000LL);
-  int status = 0, iters = 0, stab_iters = 0, fl = 0;
-
-  double lnKs[NC], lnK[NC];
-  const bool have0 = start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
-  const bool skip_stab = have0 && (fl & 1);
-#pragma unroll
-  for (int i = 0; i < NC; ++i) lnK[i] = lnKs[i];
-
-  bool unstable = false;
-  double tpd_min = 0.0;
-  if (!skip_stab) {
-    const int pcase = probe<NC>(S, o, m, lnK, tpd_min, iters);
-    if (pcase == 3) unstable = true;
-    else {
-      // stability with the Wilson / caller K (reading C19), both starts
-      double lnWv[NC], lnWl[NC];
-      StabRes sv, sl;
-      stab_trial<NC>(S, o, m, lnKs, +1.0, lnWv, sv);
-      stab_trial<NC>(S, o, m, lnKs, -1.0, lnWl, sl);
-      stab_iters = sv.iters + sl.iters;
-      unstable = stab_decide<NC>(o, m, sv, sl, lnWv, lnWl, lnK, tpd_min, status);
-    }
-  } else {
-    unstable = true;
-    tpd_min = nan;
-  }
-
+  int status = 0, iters = 0, stab_iters = 0;
   bool two = false;
-  double theta = 0.0;
-  double x[NC], y[NC];
-  if (unstable) {
-    SplitRes sp;
-    phase_split<NC>(S, o, m, lnK, x, y, sp);
-    iters += sp.iters;
-    status |= sp.status;
-    two = sp.two_phase;
-    theta = sp.theta;
-    if (!two) status |= ST_SPLIT_FAILED;
+  double theta = 0.0, tpd_min = 0.0;
+  double x[NC], y[NC], lnK[NC];
+  // attempt 0 honours the caller's lnK0 / skip-stability hint; attempt 1 (only after a failed skip-stability split)
+  // is the plain cold flash (status ST_WARM_RESTART makes start_lnK ignore the hint)
+#pragma unroll 1
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    int fl = 0, it_probe = 0;
+    double lnKs[NC];
+    const bool have0 = start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
+    const bool skip_stab = have0 && (fl & 1);
+#pragma unroll
+    for (int i = 0; i < NC; ++i) lnK[i] = lnKs[i];
+    bool unstable = false;
+    tpd_min = 0.0;
+    if (!skip_stab) {
+      const int pcase = probe<NC>(S, o, m, lnK, tpd_min, it_probe);
+      iters += it_probe;
+      if (pcase == 3) unstable = true;
+      else {
+        // stability with the Wilson / caller K (reading C19), both starts
+        double lnWv[NC], lnWl[NC];
+        StabRes sv, sl;
+        stab_trial<NC>(S, o, m, lnKs, +1.0, lnWv, sv);
+        stab_trial<NC>(S, o, m, lnKs, -1.0, lnWl, sl);
+        stab_iters = sv.iters + sl.iters;
+        unstable = stab_decide<NC>(o, m, sv, sl, lnWv, lnWl, lnK, tpd_min, status);
+      }
+    } else {
+      unstable = true;
+      tpd_min = nan;
+    }
+    int split_status = 0;
+    if (unstable) {
+      SplitRes sp;
+      phase_split<NC>(S, o, m, lnK, x, y, sp);
+      iters += sp.iters;
+      split_status = sp.status;
+      two = sp.two_phase;
+      theta = sp.theta;
+      if (!two) split_status |= ST_SPLIT_FAILED;
+    }
+    if (!two && skip_stab) { status |= ST_WARM_RESTART; continue; }   // drop the hint, flash again from Wilson
+    status |= split_status;
+    break;
   }
   store_result<NC>(io, n, two, theta, m.z, x, y, lnK, Zf, iters, status, tpd_min, stab_iters);
 }

@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
       q.spt = sqrt(P) / T;
       q.pt = P / T;
       load_zn<NC>(io, w, n, z);
-      int status = 0, fl = 0;
+      int status = w.status[n] & ST_WARM_RESTART, fl = 0;
       start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
       double theta = -1.0e300, Zx = 0.0, Zy = 0.0;
       int iters = 0;
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
         const double mn = fmin(dG, fmin(tx, ty));
         if (mn < -o.probe_margin) { tpd_min = mn; pcase = 3; }
       }
-      w.iters[n] = iters;
+      w.iters[n] += iters;
       if (pcase == 3) {
 #pragma unroll
         for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnK[i];
@@ -158,7 +158,7 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
       q.pt = P / T;
       const unsigned act = (unsigned)w.actmask[n];
       {
-        int status = 0, fl = 0;
+        int status = w.status[n] & ST_WARM_RESTART, fl = 0;
         double lnKs[NC];
         start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
         const double side = sidx ? -1.0 : 1.0;
@@ -484,13 +484,8 @@ template <int NC>
 __device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, const double (&z)[NC], bool converged,
                                             bool failed, double theta, int st_iters, int st_status, const double (&x)[NC],
                                             const double (&y)[NC], const double (&lnK)[NC]) {
-  int status = w.status[n] | st_status;
-  bool two = false;
-  if (failed) status |= ST_SPLIT_FAILED;
-  else if (converged && theta > 0.0 && theta < 1.0) two = true;
-  else status |= ST_SPLIT_FAILED;
-  store_result<NC>(io, n, two, theta, z, x, y, lnK, w.Zfeed[n], w.iters[n] + st_iters, status, w.tpdmin[n], w.stabit[n]);
-  count_add(two, &w.ctr->n_two_phase);
+  const bool two = !failed && converged && theta > 0.0 && theta < 1.0;
+  finish_common<NC>(io, w, n, z, two, theta, st_iters, st_status, x, y, lnK);
 }
 
 template <int NC, bool KIJ0>
@@ -774,6 +769,12 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
     __syncwarp();
     if (finish) {
       double lnK[NC];
+      // trivial collapse x = y (max |ln K| < 1e-9): |y/x - 1| is the same test to first order and needs no logarithm
+      double mkn = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+        if ((act >> i) & 1u) mkn = fmax(mkn, fabs(y[i] - x[i]) * rcp_fast(x[i]));
+      const bool trivial = mkn < 1.0e-9;
       if (io.lnK) {
 #pragma unroll
         for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
@@ -781,14 +782,14 @@ __global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ S
 #pragma unroll
         for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
       }
-      store_split<NC>(io, w, n, z, fin_conv, false, theta, tr_it, status, x, y, lnK);
+      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK);
       busy = false;
     }
   }
 }
 
 template <int NC, bool KIJ0>
-int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work& w, int sms, cudaStream_t st) {
+int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work& w_in, int sms, cudaStream_t st) {
   const int threads = 128;
   auto grid_for = [&](int64_t items) {
     const int64_t need = (items + threads - 1) / threads;
@@ -797,15 +798,23 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   };
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
   const unsigned gP = (unsigned)(sms * 2);   // persistent refill kernels: a few CTAs per SM pull tickets
+  Work w = w_in;
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
-  k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
-  k2_stab_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
-  k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
-  k2_split_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
-  k_finalize_counters<<<1, 32, 0, st>>>(w);
-  return cudaGetLastError() == cudaSuccess ? 8 : -1;
+  int launches = 1;
+  const int passes = (io.flags && io.lnK0) ? 2 : 1;   // pass 1: cold re-flash of mixtures whose skip-stability hint failed
+  for (int pass = 0; pass < passes; ++pass) {
+    w.pass = pass;
+    if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
+    k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+    k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
+    k2_stab_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
+    k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+    k2_split_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
+    k_finalize_counters<<<1, 32, 0, st>>>(w);
+    launches += 7;
+  }
+  return cudaGetLastError() == cudaSuccess ? launches : -1;
 }
 
 // engine 1 entry

@@ -25,13 +25,14 @@
 
 namespace ptf {
 
-enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_COUNT = 8 };
+enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_RETRY = 7, Q_COUNT = 8 };
 enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_BETA = 8, TF_ITER_SHIFT = 8 + 0 };
 
 struct Work {
   StageCounters* ctr;
   int* qcount;  // [Q_COUNT]
-  int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton;
+  int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton, *q_retry;
+  int pass;  // 0: first pass; 1: re-flash of mixtures whose skip-stability hint failed (ST_WARM_RESTART)
   double *lnz, *d, *lnK;   // [NC][N]
   double* zn;              // [NC][N] normalised feed z / sum z (written once by k_init)
   double* lnW;             // [2][NC][N]
@@ -57,6 +58,8 @@ inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   p = take(2 * n * 4); if (w) w->q_stab_newton = (int*)p;
   p = take(n * 4); if (w) w->q_split = (int*)p;
   p = take(n * 4); if (w) w->q_split_newton = (int*)p;
+  p = take(n * 4); if (w) w->q_retry = (int*)p;
+  if (w) w->pass = 0;
   p = take(c * n * 8); if (w) w->lnz = (double*)p;
   p = take(c * n * 8); if (w) w->d = (double*)p;
   p = take(c * n * 8); if (w) w->lnK = (double*)p;
@@ -151,6 +154,7 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
       }
       if (have0 && (fl & 1)) {
         dest = 2;
+        w.status[n] = status | ST_INTERNAL_SKIPPED;
 #pragma unroll
         for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnKs[i];
         w.tpdmin[n] = __longlong_as_double(0x7ff8000000000000LL);
@@ -193,12 +197,12 @@ __global__ void __launch_bounds__(128) k_probe(const __grid_constant__ Sys<NC> S
       MixCtx<NC> m;
       double P, T;
       reload_ctx<NC>(S, io, w, n, true, m, P, T);
-      int status = 0, fl = 0, iters = 0;
+      int status = w.status[n] & ST_WARM_RESTART, fl = 0, iters = 0;
       double lnK[NC];
       start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
       double tpd_min = 0.0;
       pcase = probe<NC>(S, o, m, lnK, tpd_min, iters);
-      w.iters[n] = iters;
+      w.iters[n] += iters;
       if (pcase == 3) {
 #pragma unroll
         for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnK[i];
@@ -241,7 +245,7 @@ __global__ void __launch_bounds__(128) k_stab_ss(const __grid_constant__ Sys<NC>
       MixCtx<NC> m;
       double P, T;
       reload_ctx<NC>(S, io, w, n, true, m, P, T);
-      int status = 0, fl = 0;
+      int status = w.status[n] & ST_WARM_RESTART, fl = 0;
       double lnKs[NC];
       start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
       StabState<NC> st;
@@ -325,7 +329,7 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
         w.status[n] = status;
         w.stabit[n] = stab_iters;
       } else {
-        store_result<NC>(io, n, false, 0.0, m.z, m.z, m.z, lnK, w.Zfeed[n], w.iters[n], status, tpd_min, stab_iters);
+        store_result<NC>(io, n, false, 0.0, m.z, m.z, m.z, lnK, w.Zfeed[n], w.iters[n], status & ~ST_INTERNAL_SKIPPED, tpd_min, stab_iters);
       }
     }
     queue_push(unstable, &w.qcount[Q_SPLIT], w.q_split, n);
@@ -333,16 +337,32 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
 }
 
 // ---- K5 / K6 --------------------------------------------------------------------------------------
+// Final store of a mixture that went through the split -- or, if its skip-stability hint did not lead to two phases,
+// hand it to the second pass (hint dropped, full cold flash; reported as ST_WARM_RESTART).
+template <int NC>
+__device__ __forceinline__ void finish_common(const Io& io, const Work& w, int n, const double (&z)[NC], bool two, double theta,
+                                              int st_iters, int st_status, const double (&x)[NC], const double (&y)[NC],
+                                              const double (&lnK)[NC]) {
+  const int ws = w.status[n];
+  const bool retry = (w.pass == 0) && (ws & ST_INTERNAL_SKIPPED) && !two;
+  if (retry) {
+    w.status[n] = (ws & ST_LNK0_REJECTED) | ST_WARM_RESTART;
+    w.iters[n] += st_iters;
+  } else {
+    int status = (ws | st_status) & ~ST_INTERNAL_SKIPPED;
+    if (!two) status |= ST_SPLIT_FAILED;
+    store_result<NC>(io, n, two, theta, z, x, y, lnK, w.Zfeed[n], w.iters[n] + st_iters, status, w.tpdmin[n], w.stabit[n]);
+  }
+  count_add(two, &w.ctr->n_two_phase);
+  queue_push(retry, &w.qcount[Q_RETRY], w.q_retry, n);
+}
+
 template <int NC>
 __device__ __forceinline__ void finish_split(const Io& io, const Work& w, int n, const MixCtx<NC>& m, const SplitState<NC>& st,
                                              const double (&x)[NC], const double (&y)[NC]) {
   SplitRes sp;
   split_finish<NC>(st, sp);
-  int status = w.status[n] | sp.status;
-  if (!sp.two_phase) status |= ST_SPLIT_FAILED;
-  store_result<NC>(io, n, sp.two_phase, sp.theta, m.z, x, y, st.lnK, w.Zfeed[n], w.iters[n] + sp.iters, status, w.tpdmin[n],
-                   w.stabit[n]);
-  count_add(sp.two_phase, &w.ctr->n_two_phase);
+  finish_common<NC>(io, w, n, m.z, sp.two_phase, sp.theta, sp.iters, sp.status & ~ST_SPLIT_FAILED, x, y, st.lnK);
 }
 
 template <int NC>
@@ -398,13 +418,26 @@ __global__ void __launch_bounds__(128) k_split_newton(const __grid_constant__ Sy
   }
 }
 
-// counters that are simply queue lengths
+// counters that are simply queue lengths (accumulated over the passes)
 static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
-    w.ctr->n_stab = w.qcount[Q_STAB];
-    w.ctr->n_stab_newton = w.qcount[Q_STAB_NEWTON];
-    w.ctr->n_split = w.qcount[Q_SPLIT];
-    w.ctr->n_split_newton = w.qcount[Q_SPLIT_NEWTON];
+    w.ctr->n_stab += w.qcount[Q_STAB];
+    w.ctr->n_stab_newton += w.qcount[Q_STAB_NEWTON];
+    w.ctr->n_split += w.qcount[Q_SPLIT];
+    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON];
+  }
+}
+
+// second pass: the retry queue becomes the probe queue, every other queue and ticket restarts from zero
+static __global__ void k_begin_pass2(const __grid_constant__ Work w) {
+  const int cnt = w.qcount[Q_RETRY];
+  for (int i = threadIdx.x; i < cnt; i += blockDim.x) w.q_probe[i] = w.q_retry[i];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    w.qcount[Q_PROBE] = cnt;
+    w.qcount[Q_STAB] = 0; w.qcount[Q_STAB_NEWTON] = 0; w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0;
+    w.qcount[Q_TICKET_STAB] = 0; w.qcount[Q_TICKET_SPLIT] = 0; w.qcount[Q_RETRY] = 0;
+    w.ctr->reserved[0] = cnt;   // number of warm restarts
   }
 }
 
@@ -425,14 +458,21 @@ int launch_staged(const SysHost& hs, const Opt& o, const Io& io, void* workspace
   };
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k_probe<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k_stab_ss<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
-  k_stab_newton<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
-  k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k_split_ss<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k_split_newton<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  k_finalize_counters<<<1, 32, 0, st>>>(w);
-  return cudaGetLastError() == cudaSuccess ? 8 : -1;
+  int launches = 1;
+  const int passes = (io.flags && io.lnK0) ? 2 : 1;
+  for (int pass = 0; pass < passes; ++pass) {
+    w.pass = pass;
+    if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
+    k_probe<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    k_stab_ss<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
+    k_stab_newton<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
+    k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    k_split_ss<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    k_split_newton<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    k_finalize_counters<<<1, 32, 0, st>>>(w);
+    launches += 7;
+  }
+  return cudaGetLastError() == cudaSuccess ? launches : -1;
 }
 
 }  // namespace ptf
