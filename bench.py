@@ -33,7 +33,7 @@ UNIT = "flashes/s"
 WORKLOAD = "config3: 10-component CO2-rich SRK flash (8 n-alkanes + CO2 + N2, kij per BASELINE.json), z=0.6*Dir(1)+0.4*e_CO2, T~U[220,500]K, P~U[5,300]bar, seed 2205030903"
 # Algorithmic FP64 work per flash on this workload: thread-level predicated-on DADD + DMUL + 2*DFMA of
 # all stage kernels, counted by ncu on the committed build (profiles/), per mixture.
-FLOPS_PER_FLASH = float(os.environ.get("PTFLASH_FLOPS_PER_FLASH", "7.37e4"))
+FLOPS_PER_FLASH = float(os.environ.get("PTFLASH_FLOPS_PER_FLASH", "4.56e4"))
 BYTES_PER_FLASH_NC10 = 272.0   # 8(nc+2) in + 8(2nc+1)+8 out, SURVEY.md section 8(d)
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # SMs x DFMA lanes/clk x 2 flop x max SM clock
 
