@@ -222,6 +222,9 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
   }
 }
 
+#ifndef PTF_NEWTON_MINB
+#define PTF_NEWTON_MINB 2
+#endif
 // ---- lane refill ----------------------------------------------------------------------------------
 // Lanes with want == true take consecutive tickets; returns the ticket (>= total means the queue is exhausted).
 __device__ __forceinline__ int64_t take_ticket(bool want, int* __restrict__ ticket) {
@@ -264,7 +267,7 @@ struct EtaSearch {
 
 // ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
 template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128) k2_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+__global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                       const __grid_constant__ Io io, const __grid_constant__ Work w) {
   constexpr int NT = NC * (NC + 1) / 2;
   constexpr unsigned FULL = 0xffffffffu;
@@ -568,7 +571,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
 
 // ---- K6: phase-split trust-region Newton on G (B.4-B.5), persistent warps with lane refill --------
 template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128) k2_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+__global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                        const __grid_constant__ Io io, const __grid_constant__ Work w) {
   constexpr int NT = NC * (NC + 1) / 2;
   constexpr unsigned FULL = 0xffffffffu;
@@ -797,7 +800,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     return (unsigned)(need < cap ? (need > 0 ? need : 1) : cap);
   };
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
-  const unsigned gP = (unsigned)(sms * 2);   // persistent refill kernels: a few CTAs per SM pull tickets
+  const unsigned gP = (unsigned)(sms * PTF_NEWTON_MINB);   // persistent refill kernels: a few CTAs per SM pull tickets
   Work w = w_in;
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
   int launches = 1;
