@@ -815,6 +815,17 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
       two = true;
       out.phase = 2; out.beta = sp.theta;
       for (int i = 0; i < nc; ++i) { out.x[i] = sp.x[i]; out.y[i] = sp.y[i]; out.lnK[i] = sp.lnK[i]; }
+      // Phase identity (reading C23): the phase with the larger compressibility factor is
+      // reported as the vapour y ("smallest root ... liquid phase ... largest ... vapor").  Without this
+      // the identity follows the sign of the K that seeded the split, and when both stability starts reach the SAME
+      // stationary point (tm^L = tm^V up to rounding) the paper's rule "tm^L < tm^V" is decided by noise.
+      real lpt[MAXC], Zx, Zy;
+      lnphi(s, sp.x, lpt, &Zx, nullptr);
+      lnphi(s, sp.y, lpt, &Zy, nullptr);
+      if (Zy < Zx) {
+        out.beta = (real)1 - sp.theta;
+        for (int i = 0; i < nc; ++i) { out.x[i] = sp.y[i]; out.y[i] = sp.x[i]; out.lnK[i] = -sp.lnK[i]; }
+      }
     } else if (!(sp.status & ST_SPLIT_FAILED)) out.status |= ST_SPLIT_FAILED;
   }
   if (!two && skip_stab) {

@@ -29,7 +29,7 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
 #pragma unroll 1
     for (int k = 0; k < 4; ++k) {
       const double df = cub_df(Z, r1);
-      const double dz = cub_f(Z, r1, r0) / df;
+      const double dz = cub_f(Z, r1, r0) * rcp_nr1(df);
       const double Zn = Z - dz;
       if (!(Zn > B) || !(Zn < 2.0 + B)) break;   // also catches NaN / df == 0
       Z = Zn;
@@ -38,7 +38,7 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
     if (ok) {
       // one more guarded step brings the root to rounding (and detects a linear-rate, i.e. nearly double, root)
       const double df = cub_df(Z, r1);
-      const double dz = cub_f(Z, r1, r0) / df;
+      const double dz = cub_f(Z, r1, r0) * rcp_nr1(df);
       if (fabs(dz) <= 1.0e-13 * Z) Z -= dz; else ok = false;
     }
   }
@@ -50,7 +50,7 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
     for (int k = 0; k < 100; ++k) {
       const double df = cub_df(Z, r1);
       if (!(df > 0.0)) break;
-      const double Zn = Z - cub_f(Z, r1, r0) / df;
+      const double Zn = Z - cub_f(Z, r1, r0) * rcp_nr1(df);
       if (up ? !(Zn > Z) : !(Zn < Z)) break;
       Z = Zn;
     }
@@ -59,9 +59,9 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
   const double p = Z - 1.0, q = fma(p, Z, r1);
   const double disc = fma(p, p, -4.0 * q);
   if (disc >= 0.0) {
-    const double sq = sqrt(disc);
+    const double sq = sqrt_fast(disc);
     const double t = (p >= 0.0) ? -0.5 * (p + sq) : 0.5 * (sq - p);
-    double ra = t, rb = (t != 0.0) ? q / t : -p - t;
+    double ra = t, rb = (t != 0.0) ? div_fast(q, t) : -p - t;
     ra = cub_polish(ra, r1, r0);
     rb = cub_polish(rb, r1, r0);
     if (ra > B) { zmin = fmin(zmin, ra); zmax = fmax(zmax, ra); }
@@ -201,18 +201,18 @@ __device__ __forceinline__ MCoef mcoef(const Eos& e) {
   MCoef m;
   const double A = e.A, B = e.B, Z = e.Z;
   const double FZ = fma(fma(3.0, Z, -2.0), Z, A - B - B * B);
-  const double iFZ = 1.0 / FZ;
+  const double iFZ = rcp_fast(FZ);
   const double ZA = -(Z - B) * iFZ;
   const double ZB = fma(1.0 + 2.0 * B, Z, A) * iFZ;
-  const double iZZB = 1.0 / (Z * (Z + B));
-  m.invB = 1.0 / B;
+  const double iZZB = rcp_fast(Z * (Z + B));
+  m.invB = rcp_fast(B);
   m.A = A; m.B = B; m.q = e.q;
   m.q2 = 2.0 * e.q;
   m.zA2 = 2.0 * ZA;
   m.zBB = ZB * B;
   m.zm1 = Z - 1.0;
   m.qA = e.q * A;
-  m.invZmB = 1.0 / (Z - B);
+  m.invZmB = rcp_fast(Z - B);
   m.cL1 = (Z - ZB * B) * iZZB;   // DL_j / B = cL1 eps_j - cL2 sig_j
   m.cL2 = 2.0 * ZA * iZZB;
   return m;
@@ -248,10 +248,10 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     f1 = fma(z[i] * km1[i], rcp_fast(K[i]), f1);
   }
   if (!(Kmax > 1.0) || !(Kmin < 1.0)) return false;
-  const double al = 1.0 / (1.0 - Kmax), ar = 1.0 / (1.0 - Kmin);
+  const double al = div_fast(1.0, 1.0 - Kmax), ar = div_fast(1.0, 1.0 - Kmin);
   double lo = al, hi = ar, th;
   if (f0 > 0.0) {
-    if (f1 < 0.0) { lo = 0.0; hi = 1.0; th = f0 / (f0 - f1); }
+    if (f1 < 0.0) { lo = 0.0; hi = 1.0; th = f0 * rcp_fast(f0 - f1); }
     else if (f1 == 0.0) { lo = hi = 1.0; th = 1.0; }
     else { lo = 1.0; th = fmin(1.0 + 0.5 * (ar - 1.0), 2.0); }
   } else if (f0 < 0.0) { hi = 0.0; th = fmax(0.5 * al, -1.0); }
@@ -277,7 +277,7 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     const double u = th - al, w = ar - th;
     const double h = u * w * f;
     const double dh = (w - u) * f + u * w * df;
-    double tn = th - h / dh;
+    double tn = th - h * rcp_fast(dh);
     const bool inside = (tn > lo && tn < hi);
     if (!inside) tn = 0.5 * (lo + hi);
     const double step = fabs(tn - th);
@@ -315,7 +315,7 @@ __device__ __forceinline__ bool chol_packed(double (&Lm)[NC * (NC + 1) / 2], con
 #pragma unroll
     for (int k = 0; k < j; ++k) acc = fma(-Lm[tri(j, k)], Lm[tri(j, k)], acc);
     pd = pd && (acc > 0.0);
-    const double inv = rsqrt(acc);
+    const double inv = rsqrt_fast(acc);
     Lm[tri(j, j)] = inv;
 #pragma unroll
     for (int i = j + 1; i < NC; ++i) {

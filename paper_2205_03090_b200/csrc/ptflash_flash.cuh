@@ -552,18 +552,31 @@ __device__ __forceinline__ void store_invalid(const Io& io, int64_t n) {
   if (io.stab_iters) io.stab_iters[n] = 0;
 }
 
+// Phase identity of a converged split (reading C23): true if the "y" phase has the smaller Z and must be reported as x.
+template <int NC>
+__device__ __noinline__ bool phase_swap_by_Z(const Sys<NC>& S, const MixCtx<NC>& m, const double (&x)[NC], const double (&y)[NC]) {
+  double lp[NC], Sv[NC];
+  Eos ex, ey;
+  lnphi_eval<NC>(S, m.sa, m.bi, x, lp, Sv, ex);
+  lnphi_eval<NC>(S, m.sa, m.bi, y, lp, Sv, ey);
+  return ey.Z < ex.Z;
+}
+
 // Final store.  two == false: single phase, x = y = z, beta = 1 iff Z_feed > 1/3 (convention).
 template <int NC>
 __device__ __forceinline__ void store_result(const Io& io, int64_t n, bool two, double theta, const double (&z)[NC],
                                              const double (&x)[NC], const double (&y)[NC], const double (&lnK)[NC],
-                                             double Zfeed, int iters, int status, double tpd_min, int stab_iters) {
-  io.beta[n] = two ? theta : ((Zfeed > 1.0 / 3.0) ? 1.0 : 0.0);
+                                             double Zfeed, int iters, int status, double tpd_min, int stab_iters,
+                                             bool swap) {
+  // swap: the split's "y" phase has the smaller compressibility factor, so it is reported as the liquid x
+  // (phase identity by Z, reading C23: PAPER.md:445 assigns the smallest root to the liquid, the largest to the vapour)
+  io.beta[n] = two ? (swap ? 1.0 - theta : theta) : ((Zfeed > 1.0 / 3.0) ? 1.0 : 0.0);
   io.phase[n] = two ? 2 : 1;
 #pragma unroll
   for (int i = 0; i < NC; ++i) {
-    io.x[(int64_t)i * io.N + n] = two ? x[i] : z[i];
-    io.y[(int64_t)i * io.N + n] = two ? y[i] : z[i];
-    if (io.lnK) io.lnK[(int64_t)i * io.N + n] = two ? lnK[i] : 0.0;
+    io.x[(int64_t)i * io.N + n] = two ? (swap ? y[i] : x[i]) : z[i];
+    io.y[(int64_t)i * io.N + n] = two ? (swap ? x[i] : y[i]) : z[i];
+    if (io.lnK) io.lnK[(int64_t)i * io.N + n] = two ? (swap ? -lnK[i] : lnK[i]) : 0.0;
   }
   if (io.iters) io.iters[n] = iters;
   if (io.tpd_min) io.tpd_min[n] = tpd_min;
@@ -628,7 +641,8 @@ __device__ void flash_one(const Sys<NC>& S, const Opt& o, const Io& io, int64_t 
     status |= split_status;
     break;
   }
-  store_result<NC>(io, n, two, theta, m.z, x, y, lnK, Zf, iters, status, tpd_min, stab_iters);
+  const bool swap = two && phase_swap_by_Z<NC>(S, m, x, y);
+  store_result<NC>(io, n, two, theta, m.z, x, y, lnK, Zf, iters, status, tpd_min, stab_iters, swap);
 }
 
 template <int NC>

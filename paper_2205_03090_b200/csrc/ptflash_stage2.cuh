@@ -72,9 +72,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
       double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
       const double P = io.P[n], T = io.T[n];
       PT3<NC> q;
-      q.sT = sqrt(T);
-      q.spt = sqrt(P) / T;
-      q.pt = P / T;
+      { const double iT = rcp_fast(T); q.sT = sqrt_fast(T); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
       load_zn<NC>(io, w, n, z);
       int status = w.status[n] & ST_WARM_RESTART, fl = 0;
       start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
@@ -120,6 +118,8 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
 #pragma unroll
         for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnK[i];
         w.tpdmin[n] = tpd_min;
+        w.Zxy[n] = Zx;
+        w.Zxy[io.N + n] = Zy;
       }
     }
     count_add(pcase == 1, &w.ctr->n_case1);
@@ -153,9 +153,7 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
       double lnW[NC], W[NC], lp[NC], Sv[NC];
       const double P = io.P[n], T = io.T[n];
       PT3<NC> q;
-      q.sT = sqrt(T);
-      q.spt = sqrt(P) / T;
-      q.pt = P / T;
+      { const double iT = rcp_fast(T); q.sT = sqrt_fast(T); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
       const unsigned act = (unsigned)w.actmask[n];
       {
         int status = w.status[n] & ST_WARM_RESTART, fl = 0;
@@ -217,6 +215,7 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
       w.tm[(int64_t)sidx * N + n] = tm;
       w.sumW[(int64_t)sidx * N + n] = sumW;
       w.tflags[(int64_t)sidx * N + n] = (converged ? TF_CONVERGED : 0) | (capped ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
+      if (need_newton) w.Zw[(int64_t)sidx * N + n] = e.Z;
     }
     queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
   }
@@ -259,7 +258,7 @@ struct EtaSearch {
     }
     if (phase == 2) {
       if (kept_sn >= 0.5 * Delta || (eta_lo > 0.0 && eta_hi / eta_lo < 1.5) || k >= 12) phase = 3;
-      else eta = (eta_lo > 0.0) ? sqrt(eta_lo * eta_hi) : eta_hi * 0.125;
+      else eta = (eta_lo > 0.0) ? sqrt_fast(eta_lo * eta_hi) : eta_hi * 0.125;
     }
     return keep;
   }
@@ -297,9 +296,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
           n = item >> 1;
           sidx = item & 1;
           const double P = io.P[n], T = io.T[n];
-          sT = sqrt(T);
-          spt = sqrt(P) / T;
-          pt = P / T;
+          { const double iT = rcp_fast(T); sT = sqrt_fast(T); spt = sqrt_fast(P) * iT; pt = P * iT; }
           act = (unsigned)w.actmask[n];
 #pragma unroll
           for (int i = 0; i < NC; ++i) {
@@ -311,7 +308,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
           first = true;
           reeval = false;
           searching = false;
-          Zw = 0.0;
+          Zw = w.Zw[(int64_t)sidx * N + n];
           busy = true;
         } else {
           exhausted = true;
@@ -361,14 +358,14 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
         double bn = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) bn = fma(beta[i], beta[i], bn);
-        Delta = fmax(1.0, 0.5 * sqrt(bn));
+        Delta = fmax(1.0, 0.5 * sqrt_fast(bn));
         Delta_cap = 8.0 * Delta;
       } else if (!reeval) {
         const double act_red = tm_new - tm;
         accepted = (act_red < 0.0) || (rmax < rmax_acc);
         if (accepted) {
           if (fabs(pred) > 1.0e-13) {
-            const double ratio = fabs(act_red / pred);
+            const double ratio = fabs(act_red * rcp_fast(pred));
             if (ratio <= 0.25) Delta *= 0.5;
             else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
           }
@@ -404,7 +401,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
     if (busy && searching) {
       // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.1b): build H + eta I, factor, solve ----
       const MCoef mc = mcoef(e);
-      const double isq = rsqrt(sumW);
+      const double isq = rsqrt_fast(sumW);
       double g[NC], st[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) g[i] = 0.5 * beta[i] * r[i];   // B.2a
@@ -434,7 +431,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
         sn = fma(st[i], st[i], sn);
         if (((act >> i) & 1u) && !(beta[i] + st[i] > 0.0)) good = false;
       }
-      sn = sqrt(sn);
+      sn = sqrt_fast(sn);
       good = good && (sn <= Delta);
       const double eta_used = es.eta;
       if (es.feed(good, sn, Delta, kept_sn)) {
@@ -486,9 +483,9 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
 template <int NC>
 __device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, const double (&z)[NC], bool converged,
                                             bool failed, double theta, int st_iters, int st_status, const double (&x)[NC],
-                                            const double (&y)[NC], const double (&lnK)[NC]) {
+                                            const double (&y)[NC], const double (&lnK)[NC], double Zx, double Zy) {
   const bool two = !failed && converged && theta > 0.0 && theta < 1.0;
-  finish_common<NC>(io, w, n, z, two, theta, st_iters, st_status, x, y, lnK);
+  finish_common<NC>(io, w, n, z, two, theta, st_iters, st_status, x, y, lnK, two && (Zy < Zx));   // phase identity by Z (C23)
 }
 
 template <int NC, bool KIJ0>
@@ -506,13 +503,12 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
       double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
       const double P = io.P[n], T = io.T[n];
       PT3<NC> q;
-      q.sT = sqrt(T);
-      q.spt = sqrt(P) / T;
-      q.pt = P / T;
+      { const double iT = rcp_fast(T); q.sT = sqrt_fast(T); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
       load_zn<NC>(io, w, n, z);
 #pragma unroll
       for (int i = 0; i < NC; ++i) lnK[i] = w.lnK[(int64_t)i * N + n];
-      double theta = -1.0e300, Zx = 0.0, Zy = 0.0, r_prev = -1.0;
+      double theta = -1.0e300, r_prev = -1.0;
+      double Zx = w.Zxy[n], Zy = w.Zxy[N + n];   // roots of the stage that produced lnK (0: none)
       bool converged = false, failed = false, final_rr = false;
       int k = 0, status = 0;
       // One copy of exp + Rachford-Rice + the two lnphi evaluations: the Rachford-Rice that makes x, y consistent with
@@ -550,19 +546,25 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         ++k;
         if (rk < 1.0e-14) final_rr = true;
         else if (r_prev > 0.0 && rk < o.tol_ss) {
-          const double rho = rk / r_prev;   // linear-convergence error estimate eps = r rho / (1 - rho)
-          if (rho < 1.0 && rk * rho / (1.0 - rho) < o.tol_ss) final_rr = true;
+          const double rho = rk * rcp_fast(r_prev);   // linear-convergence error estimate eps = r rho / (1 - rho)
+          if (rho < 1.0 && rk * rho < o.tol_ss * (1.0 - rho)) final_rr = true;
         }
         r_prev = rk;
       }
       if (go_newton) {
         // hand-over in the Newton variables: n^V_i = theta y_i (B.4)
+        // ... of the MINORITY phase: for theta > 1/2 the roles of the two phases are exchanged (n^L = (1 - theta) x is
+        // handed over as "n^V"), so that the majority composition (z - n)/(1 - sum n) is formed without cancellation; G
+        // and its stationary point are the same, and the final store restores the phase identity by Z (C23).
+        const bool mirror = theta > 0.5;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = fmin(theta * y[i], z[i]);
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = fmin(mirror ? (1.0 - theta) * x[i] : theta * y[i], z[i]);
         w.iters[n] += k;
         w.status[n] |= status;
+        w.Zxy[n] = mirror ? Zy : Zx;
+        w.Zxy[N + n] = mirror ? Zx : Zy;
       } else {
-        store_split<NC>(io, w, n, z, converged, failed, theta, k, status, x, y, lnK);
+        store_split<NC>(io, w, n, z, converged, failed, theta, k, status, x, y, lnK, Zx, Zy);
       }
     }
     queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
@@ -597,9 +599,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
         if (tk < total) {
           n = w.q_split_newton[tk];
           const double P = io.P[n], T = io.T[n];
-          sT = sqrt(T);
-          spt = sqrt(P) / T;
-          pt = P / T;
+          { const double iT = rcp_fast(T); sT = sqrt_fast(T); spt = sqrt_fast(P) * iT; pt = P * iT; }
           act = (unsigned)w.actmask[n];
           // k2_split_ss left n^V = theta y of its last Rachford-Rice here
 #pragma unroll
@@ -610,8 +610,8 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
           reeval = false;
           searching = false;
           Delta = 0.25;
-          Zx = 0.0;
-          Zy = 0.0;
+          Zx = w.Zxy[n];
+          Zy = w.Zxy[N + n];
           busy = true;
         } else {
           exhausted = true;
@@ -666,7 +666,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
         accepted = (act_red < 0.0) || (gmax < gmax_acc);
         if (accepted) {
           if (fabs(pred) > 1.0e-13) {
-            const double ratio = fabs(act_red / pred);
+            const double ratio = fabs(act_red * rcp_fast(pred));
             if (ratio <= 0.25) Delta *= 0.5;
             else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
           }
@@ -689,7 +689,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
         else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
         else {
           tr_it++;
-          es.start(1.0e-3 / (theta * (1.0 - theta)));
+          es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
           kept_sn = 0.0;
           searching = true;
         }
@@ -700,11 +700,11 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
     if (busy && searching) {
       // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.4a) ----
       const MCoef mx = mcoef(ex), my = mcoef(ey);
-      const double tt = theta * (1.0 - theta), itt = 1.0 / tt;
+      const double tt = theta * (1.0 - theta), itt = rcp_fast(tt);
       const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
       double D[NC], st[NC];
 #pragma unroll
-      for (int i = 0; i < NC; ++i) D[i] = ((act >> i) & 1u) ? z[i] / (x[i] * y[i]) : 1.0;
+      for (int i = 0; i < NC; ++i) D[i] = ((act >> i) & 1u) ? z[i] * rcp_fast(x[i] * y[i]) : 1.0;
       double Lm[NT];
 #pragma unroll
       for (int j = 0; j < NC; ++j) {
@@ -738,7 +738,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
           if (!(nv > 0.0) || !(nv < z[i])) good = false;
         }
       }
-      sn = sqrt(sn);
+      sn = sqrt_fast(sn);
       good = good && (sn <= Delta);
       const double eta_used = es.eta;
       if (es.feed(good, sn, Delta, kept_sn)) {
@@ -763,7 +763,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
           theta = 0.0;
 #pragma unroll
           for (int i = 0; i < NC; ++i) { nV[i] += s[i]; theta += nV[i]; }
-          const double it = 1.0 / theta, il = 1.0 / (1.0 - theta);
+          const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
 #pragma unroll
           for (int i = 0; i < NC; ++i) { y[i] = nV[i] * it; x[i] = (z[i] - nV[i]) * il; }
         }
@@ -785,7 +785,7 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
 #pragma unroll
         for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
       }
-      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK);
+      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, Zx, Zy);
       busy = false;
     }
   }

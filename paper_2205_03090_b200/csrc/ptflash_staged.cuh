@@ -38,6 +38,7 @@ struct Work {
   double* lnW;             // [2][NC][N]
   double *tm, *sumW;       // [2][N]
   double *Zfeed, *tpdmin;  // [N]
+  double *Zw, *Zxy;        // [2][N] cubic roots handed from an SS stage to its Newton stage (warm starts)
   int* tflags;             // [2][N]
   int *status, *iters, *stabit;  // [N]
   int* actmask;            // [N] bit i set <=> z_i > 0
@@ -69,6 +70,8 @@ inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   p = take(2 * n * 8); if (w) w->sumW = (double*)p;
   p = take(n * 8); if (w) w->Zfeed = (double*)p;
   p = take(n * 8); if (w) w->tpdmin = (double*)p;
+  p = take(2 * n * 8); if (w) w->Zw = (double*)p;
+  p = take(2 * n * 8); if (w) w->Zxy = (double*)p;
   p = take(2 * n * 4); if (w) w->tflags = (int*)p;
   p = take(n * 4); if (w) w->status = (int*)p;
   p = take(n * 4); if (w) w->iters = (int*)p;
@@ -143,6 +146,8 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
         w.zn[(int64_t)i * io.N + n] = m.z[i];
       }
       w.Zfeed[n] = Zf;
+      w.Zxy[n] = 0.0;
+      w.Zxy[io.N + n] = 0.0;
       w.status[n] = status;
       w.iters[n] = 0;
       w.stabit[n] = 0;
@@ -329,7 +334,7 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
         w.status[n] = status;
         w.stabit[n] = stab_iters;
       } else {
-        store_result<NC>(io, n, false, 0.0, m.z, m.z, m.z, lnK, w.Zfeed[n], w.iters[n], status & ~ST_INTERNAL_SKIPPED, tpd_min, stab_iters);
+        store_result<NC>(io, n, false, 0.0, m.z, m.z, m.z, lnK, w.Zfeed[n], w.iters[n], status & ~ST_INTERNAL_SKIPPED, tpd_min, stab_iters, false);
       }
     }
     queue_push(unstable, &w.qcount[Q_SPLIT], w.q_split, n);
@@ -342,7 +347,7 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
 template <int NC>
 __device__ __forceinline__ void finish_common(const Io& io, const Work& w, int n, const double (&z)[NC], bool two, double theta,
                                               int st_iters, int st_status, const double (&x)[NC], const double (&y)[NC],
-                                              const double (&lnK)[NC]) {
+                                              const double (&lnK)[NC], bool swap) {
   const int ws = w.status[n];
   const bool retry = (w.pass == 0) && (ws & ST_INTERNAL_SKIPPED) && !two;
   if (retry) {
@@ -351,18 +356,19 @@ __device__ __forceinline__ void finish_common(const Io& io, const Work& w, int n
   } else {
     int status = (ws | st_status) & ~ST_INTERNAL_SKIPPED;
     if (!two) status |= ST_SPLIT_FAILED;
-    store_result<NC>(io, n, two, theta, z, x, y, lnK, w.Zfeed[n], w.iters[n] + st_iters, status, w.tpdmin[n], w.stabit[n]);
+    store_result<NC>(io, n, two, theta, z, x, y, lnK, w.Zfeed[n], w.iters[n] + st_iters, status, w.tpdmin[n], w.stabit[n], swap);
   }
   count_add(two, &w.ctr->n_two_phase);
   queue_push(retry, &w.qcount[Q_RETRY], w.q_retry, n);
 }
 
 template <int NC>
-__device__ __forceinline__ void finish_split(const Io& io, const Work& w, int n, const MixCtx<NC>& m, const SplitState<NC>& st,
-                                             const double (&x)[NC], const double (&y)[NC]) {
+__device__ __forceinline__ void finish_split(const Sys<NC>& S, const Io& io, const Work& w, int n, const MixCtx<NC>& m,
+                                             const SplitState<NC>& st, const double (&x)[NC], const double (&y)[NC]) {
   SplitRes sp;
   split_finish<NC>(st, sp);
-  finish_common<NC>(io, w, n, m.z, sp.two_phase, sp.theta, sp.iters, sp.status & ~ST_SPLIT_FAILED, x, y, st.lnK);
+  const bool swap = sp.two_phase && phase_swap_by_Z<NC>(S, m, x, y);
+  finish_common<NC>(io, w, n, m.z, sp.two_phase, sp.theta, sp.iters, sp.status & ~ST_SPLIT_FAILED, x, y, st.lnK, swap);
 }
 
 template <int NC>
@@ -391,7 +397,7 @@ __global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC
         w.iters[n] += st.iters;
         w.status[n] |= st.status;
       } else {
-        finish_split<NC>(io, w, n, m, st, x, y);
+        finish_split<NC>(S, io, w, n, m, st, x, y);
       }
     }
     queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
@@ -414,7 +420,7 @@ __global__ void __launch_bounds__(128) k_split_newton(const __grid_constant__ Sy
     st.iters = 0; st.status = 0; st.converged = false; st.failed = false; st.go_newton = true;
     rr_solve<NC>(K, m.z, st.theta, x, y);  // the same Rachford-Rice that ended the SS stage
     split_newton<NC>(S, o, m, st, x, y);
-    finish_split<NC>(io, w, n, m, st, x, y);
+    finish_split<NC>(S, io, w, n, m, st, x, y);
   }
 }
 

@@ -95,14 +95,10 @@ def test_parity_config5_warm_start(oracle_mod):
         rep_c = check(w, g_cold, o_cold)
         two = (g_warm["phase"] == 2) & (g_cold["phase"] == 2)
         assert two.sum() > 2000
-        # warm and cold starts reach the same split wherever both report two phases -- up to the liquid/vapour labels:
-        # a noisy lnK0 with the wrong sign near a critical point returns the same two phases with x and y exchanged
-        # (beta -> 1 - beta), which satisfies (1a), (1b), (2) equally ("phase identity")
+        # warm and cold starts reach the same split wherever both report two phases, liquid/vapour labels included:
+        # the identity no longer follows the sign of the supplied lnK0 but the compressibility factors (reading C23)
         db = np.abs(g_warm["beta"] - g_cold["beta"])[two]
-        dbs = np.abs(g_warm["beta"] - (1.0 - g_cold["beta"]))[two]
-        dxs = np.abs(g_warm["x"] - g_cold["y"]).max(0)[two]
-        swapped = (db > 1e-8) & (dbs < 1e-8) & (dxs < 1e-8)
-        assert np.all((db < 1e-8) | swapped) and swapped.mean() < 0.02
+        assert np.all(db < 1e-8)
         restarted = (g_warm["status"] & 64) != 0
         assert np.all(g_warm["stab_iters"][(flags == 1) & ~restarted] == 0)   # stability skipped where the caller said so
         # a failed skip-stability hint is dropped and reported (ST_WARM_RESTART), on both sides for the same mixtures

@@ -506,3 +506,33 @@ def test_warm_start_and_skip_stability(sys10):
     assert np.abs(warm["beta"] - cold["beta"])[two].max() < 1e-8
     assert warm["iters"][two].mean() < cold["iters"][two].mean()
     assert np.all(warm["stab_iters"][two] == 0)
+
+
+def test_phase_identity_by_compressibility(oracle_mod, sys10):
+    # Reading C23 (smallest root -> liquid, largest -> vapour): y is the phase with the larger Z.
+    # (a) invariant on a workload; (b) independence of the sign of the K that seeds the split -- the two phases a
+    # split finds from lnK and from -lnK are the same, and so is their reported identity; (c) the tie cases of
+    # config 3 in which both stability starts reach the same stationary point (tm^L = tm^V to rounding, so that
+    # "tm^L < tm^V", is decided by noise): the double and the long double build now report the same
+    # identity (they did not before C23: mixtures 320255 and 730360).
+    w = W.config3(3000)
+    r = sys10.flash(w.z, w.P, w.T, nthreads=8)
+    two = np.where(r["phase"] == 2)[0]
+    assert len(two) > 500
+    for n in two[:200]:
+        _, Zx = sys10.lnphi(w.P[n], w.T[n], r["x"][:, n])
+        _, Zy = sys10.lnphi(w.P[n], w.T[n], r["y"][:, n])
+        assert Zy > Zx
+    flags = np.where(r["phase"] == 2, 1, 0).astype(np.uint8)
+    rneg = sys10.flash(w.z, w.P, w.T, lnK0=-r["lnK"], flags=flags, nthreads=8)
+    ok = (rneg["status"][two] & 64) == 0          # not restarted
+    assert ok.mean() > 0.9
+    assert np.abs(rneg["beta"] - r["beta"])[two][ok].max() < 1e-8
+    assert np.abs(rneg["y"] - r["y"])[:, two[ok]].max() < 1e-8
+    ld = oracle_mod.Oracle.from_system(W.system_co2_10(), real="long double")
+    for n in (320255, 616425, 693344, 730360, 813246):
+        wn = W.config3(1, offset=n)
+        a = sys10.flash(wn.z, wn.P, wn.T, nthreads=1)
+        b = ld.flash(wn.z, wn.P, wn.T, nthreads=1)
+        assert a["phase"][0] == 2 and b["phase"][0] == 2
+        assert abs(a["beta"][0] - b["beta"][0]) < 1e-9 and np.abs(a["x"] - b["x"]).max() < 1e-9
