@@ -123,7 +123,8 @@ enum {
   PTFLASH_OPT_USE_NEWTON = 11,     /* [1]; 0 = pure successive substitution */
   PTFLASH_OPT_SS_CAP = 12,         /* [100000]: SS cap when Newton is off or theta stays outside (0,1) */
   PTFLASH_OPT_ENGINE = 13,         /* [1] 1 = staged persistent kernels with work queues; 0 = single run-to-completion kernel */
-  PTFLASH_NUM_OPTS = 14
+  PTFLASH_OPT_STAGE_PROFILE = 14,  /* [0] 1 = record a CUDA event between the stage kernels (engine 1), see ptflash_get_stage_ms */
+  PTFLASH_NUM_OPTS = 15
 };
 int ptflash_set_option(ptflash_handle_t h, int key, double value);
 int ptflash_get_option(ptflash_handle_t h, int key, double* value);
@@ -141,6 +142,14 @@ typedef struct ptflash_stats {
   int64_t kernel_launches;  /* kernels launched by the last call */
 } ptflash_stats_t;
 int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out);
+
+/* Stage times of the last call made with PTFLASH_OPT_STAGE_PROFILE = 1 (engine 1), measured with CUDA events recorded
+ * on the call's stream between the stage kernels -- the per-stage "time" row of the paper's profiler (Table 4
+ * PAPER.md:332-345).  Order (first pass): init, probe, stab_ss, stab_newton, stab_decide, split_ss, split_newton;
+ * a second pass (warm restarts) appends its six stages.  Writes up to `cap` values (milliseconds) to HOST array `ms`,
+ * returns the number written (0 if profiling was off), or PTFLASH_EINVAL / PTFLASH_ECUDA.  Synchronises the stream. */
+#define PTFLASH_NUM_STAGES 7
+int ptflash_get_stage_ms(ptflash_handle_t h, float* ms, int cap);
 
 /* FP64 roofline probe: runs an unrolled independent-DFMA kernel on every SM for `iters` iterations and returns
  * the achieved FP64 FLOP/s (used by bench.py as the measured denominator of the ALU roofline). */

@@ -17,9 +17,9 @@ PTFLASH_OK, PTFLASH_EINVAL, PTFLASH_ECUDA = 0, -1, -2
 ST_STAB_CAP, ST_SPLIT_CAP, ST_BAND, ST_SPLIT_FAILED, ST_LNK0_REJECTED = 1, 2, 4, 8, 32
 FLAG_SKIP_STABILITY, FLAG_USE_LNK0 = 1, 2
 OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band", "probe_iters",
-           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine"]
+           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile"]
 EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
-           "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_fp64_peak",
+           "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_get_stage_ms", "ptflash_fp64_peak",
            "ptflash_last_error", "ptflash_version"]
 
 
@@ -69,6 +69,8 @@ def load_library():
     L.ptflash_get_option.argtypes = [vp, C.c_int, dp]
     L.ptflash_get_stats.restype = C.c_int
     L.ptflash_get_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.ptflash_get_stage_ms.restype = C.c_int
+    L.ptflash_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
     L.ptflash_fp64_peak.restype = C.c_int
     L.ptflash_fp64_peak.argtypes = [C.c_int, dp, dp, vp]
     L.ptflash_last_error.restype = C.c_char_p
@@ -159,6 +161,18 @@ def ptflash_get_stats(h) -> dict:
     return s.as_dict()
 
 
+STAGE_NAMES = ["init", "probe", "stab_ss", "stab_newton", "stab_decide", "split_ss", "split_newton"]
+
+
+def ptflash_get_stage_ms(h) -> list:
+    """Stage times (ms) of the last call made with the stage_profile option on; [] if it was off."""
+    buf = (C.c_float * 24)()
+    n = load_library().ptflash_get_stage_ms(h, buf, 24)
+    if n < 0:
+        _check(n, "ptflash_get_stage_ms")
+    return [float(buf[i]) for i in range(n)]
+
+
 def ptflash_fp64_peak(iters=4096, stream=None):
     """Measured FP64 FLOP/s of an independent-DFMA kernel on the current device -> (flops_per_s, ms)."""
     f, ms = C.c_double(0), C.c_double(0)
@@ -189,6 +203,9 @@ class PTFlash:
 
     def stats(self):
         return ptflash_get_stats(self.h)
+
+    def stage_ms(self):
+        return ptflash_get_stage_ms(self.h)
 
     def flash(self, z, P, T, lnK0=None, flags=None, extended=True, stream=None):
         """z [nc, N], P [N], T [N]: CUDA float64 tensors -> dict of CUDA tensors."""

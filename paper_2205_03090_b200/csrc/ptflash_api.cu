@@ -20,7 +20,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 
-const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1};
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0};
 
 }  // namespace
 
@@ -40,6 +40,10 @@ struct ptflash_handle_s {
   ptf::StageCounters* counters_host;  // pinned
   int64_t last_N;
   int last_launches;
+  // stage profiling (PTFLASH_OPT_STAGE_PROFILE): events recorded between the stage kernels of the last call
+  cudaEvent_t events[PTF_MAX_STAGE_EVENTS];
+  bool events_made;
+  int n_events;
 };
 
 namespace {
@@ -59,6 +63,8 @@ ptf::Opt make_opt(const double* o) {
   r.split_tr_iters = (int)o[PTFLASH_OPT_SPLIT_TR_ITERS];
   r.use_newton = (int)o[PTFLASH_OPT_USE_NEWTON];
   r.ss_cap = (int)o[PTFLASH_OPT_SS_CAP];
+  r.prof_events = nullptr;
+  r.prof_count = nullptr;
   return r;
 }
 
@@ -151,6 +157,8 @@ int ptflash_destroy(ptflash_handle_t h) {
   if (h->ws) cudaFree(h->ws);
   if (h->stage) cudaFree(h->stage);
   if (h->counters_host) cudaFreeHost(h->counters_host);
+  if (h->events_made)
+    for (int i = 0; i < PTF_MAX_STAGE_EVENTS; ++i) cudaEventDestroy(h->events[i]);
   delete h;
   return rc;
 }
@@ -191,7 +199,17 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
     const size_t need = ptf::staged_workspace_bytes(h->sys.nc, io->N);
     if (!ensure(&h->ws, &h->ws_bytes, need, st, "cudaMalloc(workspace)")) return PTFLASH_ECUDA;
   }
-  const ptf::Opt o = make_opt(h->opts);
+  ptf::Opt o = make_opt(h->opts);
+  h->n_events = 0;
+  if ((int)h->opts[PTFLASH_OPT_STAGE_PROFILE] && engine) {
+    if (!h->events_made) {
+      for (int i = 0; i < PTF_MAX_STAGE_EVENTS; ++i)
+        if (!cuda_ok(cudaEventCreate(&h->events[i]), "cudaEventCreate")) return PTFLASH_ECUDA;
+      h->events_made = true;
+    }
+    o.prof_events = h->events;
+    o.prof_count = &h->n_events;
+  }
   const int launches = fn(h->sys, o, d, h->ws, st);
   if (launches < 0) { cuda_ok(cudaGetLastError(), "kernel launch"); if (g_err.empty()) set_err("kernel launch failed"); return PTFLASH_ECUDA; }
   if (engine) {
@@ -271,6 +289,16 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
     out->n_two_phase = c.n_two_phase;
   }
   return PTFLASH_OK;
+}
+
+int ptflash_get_stage_ms(ptflash_handle_t h, float* ms, int cap) {
+  if (!h || !ms || cap < 0) { set_err("ptflash_get_stage_ms: bad argument"); return PTFLASH_EINVAL; }
+  if (!h->used || h->n_events < 2) return 0;
+  if (!cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
+  int n = 0;
+  for (int i = 0; i + 1 < h->n_events && n < cap; ++i, ++n)
+    if (!cuda_ok(cudaEventElapsedTime(&ms[n], h->events[i], h->events[i + 1]), "cudaEventElapsedTime")) return PTFLASH_ECUDA;
+  return n;
 }
 
 int ptflash_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, void* stream) {

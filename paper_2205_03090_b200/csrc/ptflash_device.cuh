@@ -26,7 +26,11 @@ namespace ptf {
 struct Opt {
   double tol_ss, tol_newton_g, tol_newton_step, probe_margin, trivial_tol, band;
   int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap;
+  // host only: cudaEvent_t[PTF_MAX_STAGE_EVENTS] recorded between the stage kernels when stage profiling is on (else null)
+  void* prof_events;
+  int* prof_count;   // host only: number of events recorded by the last launch
 };
+#define PTF_MAX_STAGE_EVENTS 24
 
 // Per-system constants, precomputed on the host in ptflash_create:
 //   sqrt(A_i) = sqrt(P)/T * |u_i - v_i sqrt(T)|,  u_i = sqrt(0.42748/Pc_i) Tc_i (1+m_i),  v_i = sqrt(0.42748/Pc_i) sqrt(Tc_i) m_i

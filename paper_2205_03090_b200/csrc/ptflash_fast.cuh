@@ -306,8 +306,16 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
 // (L L^T) s = -g.  On exit Lm holds L with the INVERSE diagonal on the diagonal.  Returns false if not
 // positive definite.
 // ------------------------------------------------------------------------------------------------
-template <int NC>
-__device__ __forceinline__ bool chol_packed(double (&Lm)[NC * (NC + 1) / 2], const double (&g)[NC], double (&s)[NC]) {
+// Packed triangle in shared memory: element k of thread t at base[k * STRIDE + t] (conflict-free: the 32 lanes of a
+// warp read 32 consecutive doubles), compile-time k -> immediate offsets.
+template <int STRIDE>
+struct TriSmem {
+  double* p;
+  __device__ __forceinline__ double& operator[](int k) const { return p[k * STRIDE]; }
+};
+
+template <int NC, class Mat>
+__device__ __forceinline__ bool chol_packed(Mat& Lm, const double (&g)[NC], double (&s)[NC]) {
   bool pd = true;
 #pragma unroll
   for (int j = 0; j < NC; ++j) {

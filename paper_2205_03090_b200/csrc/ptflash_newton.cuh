@@ -1,0 +1,593 @@
+// ptflash_newton.cuh -- trust-region Newton stages of engine 1 (B.1-B.3 stability, B.4-B.5 phase split),
+// third generation: matrix-free Hessian rows + row-wise Cholesky with the factor in shared memory.
+//
+// Why: the second-generation kernels (k2_*_newton) kept the packed nc x nc Hessian in registers (110 registers at
+// nc = 10) next to the lane state of the refill loop; at 255 registers they spilled to local memory (the split kernel
+// moved 3.7 GB through DRAM for 2.3 GFLOP of work) and ran two warps per scheduler.  Here
+//   * the Hessian is never stored: M = n dlnphi/dn is a bilinear form in the basis F_i = (1, B_i, S_i),
+//         M_ij = sum_ab F_ia C_ab F_jb - 2 q A_ij          (C: 3 x 3 from the scalars of the cubic, mc3() below),
+//     so row i of H is generated in registers from C F_i (9 FMAs) and four per-component vectors, 5-6 FMAs per entry;
+//   * the Cholesky is row-wise (Banachiewicz): the current row lives in registers, finished rows L[j][.] are read from
+//     shared memory (one LDS per FMA, conflict-free: element k of thread t at [k * 128 + t]), the forward substitution
+//     is fused into the row loop, the inverse diagonal stays in registers;
+//   * the lane state that must survive a trip (accepted point, pending step) is parked in shared memory, so the
+//     register file only holds what the current phase of the trip needs.
+// The trust-region logic (EtaSearch, acceptance rule, B.3 radius update, lane refill from a ticket) is unchanged.
+#pragma once
+#include "ptflash_fast.cuh"
+#include "ptflash_staged.cuh"
+
+namespace ptf {
+
+constexpr int NEWTON_THREADS = 128;
+
+// Coefficients of M_ij = sum_ab F_ia C[a][b] F_jb - q2 A_ij with F_i = (1, B_i, S_i) (B_i, not B_i/B).
+// Derivation: DESIGN.md section 2 (M_ij = e_i p_j + c_j - Dq_j u_i + 2q(S_i - A_ij) with p, c, Dq affine in
+// e_j - 1 and S_j - A, u_i = 2 S_i - A e_i, e_i = B_i/B).
+struct MC3 {
+  double c00, c01, c02, c10, c11, c12, c20, c21, c22, q2;
+};
+__device__ __forceinline__ MC3 mc3(const Eos& e) {
+  const double A = e.A, B = e.B, Z = e.Z, q = e.q;
+  const double FZ = fma(fma(3.0, Z, -2.0), Z, A - B - B * B);
+  const double iFZ = rcp_fast(FZ);
+  const double ZA = -(Z - B) * iFZ;
+  const double ZB = fma(1.0 + 2.0 * B, Z, A) * iFZ;
+  const double iZZB = rcp_fast(Z * (Z + B));
+  const double invB = rcp_fast(B);
+  const double invZmB = rcp_fast(Z - B);
+  const double q2 = 2.0 * q;
+  const double zA2 = 2.0 * ZA, zBB = ZB * B;
+  const double p1 = zBB - (Z - 1.0) - q * A, p2 = zA2 + q2, p0 = -p1 - p2 * A;
+  const double c1 = -(zBB - B) * invZmB, c2 = -zA2 * invZmB, c0 = -c1 - c2 * A;
+  const double d1 = (Z - zBB) * iZZB - q, d2 = -zA2 * iZZB, d0 = -d1 - d2 * A;
+  MC3 m;
+  m.q2 = q2;
+  m.c00 = c0;
+  m.c01 = c1 * invB;
+  m.c02 = c2;
+  m.c10 = fma(A, d0, p0) * invB;
+  m.c11 = fma(A, d1, p1) * invB * invB;
+  m.c12 = fma(A, d2, p2) * invB;
+  m.c20 = q2 - 2.0 * d0;
+  m.c21 = -2.0 * d1 * invB;
+  m.c22 = -2.0 * d2;
+  return m;
+}
+
+// strict lower triangle of the Cholesky factor, one column of shared memory per thread
+template <int NC>
+struct LRows {
+  double* p;
+  __device__ __forceinline__ double& at(int i, int j) const { return p[(i * (i - 1) / 2 + j) * NEWTON_THREADS]; }
+};
+
+// Eliminate row i of a row-wise Cholesky.  On entry row[0..i] = H[i][0..i]; on exit row[j < i] = L[i][j] (also stored
+// to shared memory), invd[i] = 1 / L[i][i], yv[i] = forward substitution of rhs.  `i` is a compile-time constant
+// after unrolling, so every j < i / k < j test disappears.
+template <int NC>
+__device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const LRows<NC>& L, double (&invd)[NC],
+                                         double (&yv)[NC], const double rhs, bool& pd) {
+#pragma unroll
+  for (int j = 0; j < NC; ++j) {
+    if (j < i) {
+      double acc = row[j];
+#pragma unroll
+      for (int k = 0; k < NC; ++k)
+        if (k < j) acc = fma(-row[k], L.at(j, k), acc);
+      row[j] = acc * invd[j];
+    }
+  }
+  double acc = row[i], a = rhs;
+#pragma unroll
+  for (int k = 0; k < NC; ++k)
+    if (k < i) { acc = fma(-row[k], row[k], acc); a = fma(-row[k], yv[k], a); }
+  pd = pd && (acc > 0.0);
+  const double inv = rsqrt_fast(acc);
+  invd[i] = inv;
+  yv[i] = a * inv;
+#pragma unroll
+  for (int j = 0; j < NC; ++j)
+    if (j < i) L.at(i, j) = row[j];
+}
+
+// back substitution L^T s = yv
+template <int NC>
+__device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&invd)[NC], const double (&yv)[NC], double (&s)[NC]) {
+#pragma unroll
+  for (int i = NC - 1; i >= 0; --i) {
+    double acc = yv[i];
+#pragma unroll
+    for (int k = 0; k < NC; ++k)
+      if (k > i) acc = fma(-L.at(k, i), s[k], acc);
+    s[i] = acc * invd[i];
+  }
+}
+
+#ifndef PTF_STABN_MINB
+#define PTF_STABN_MINB 2
+#endif
+#ifndef PTF_SPLITN_MINB
+#define PTF_SPLITN_MINB 2
+#endif
+
+template <int NC>
+constexpr int stabn_smem_doubles() { return NC * (NC - 1) / 2 + 2 * NC; }   // per thread: L, beta, pending step
+template <int NC>
+constexpr int splitn_smem_doubles() { return NC * (NC - 1) / 2 + 5 * NC; }  // per thread: L, n^V, pending step, z, g, D
+
+// ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(NEWTON_THREADS, PTF_STABN_MINB)
+k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o, const __grid_constant__ Io io,
+               const __grid_constant__ Work w) {
+  constexpr int NL = NC * (NC - 1) / 2;
+  constexpr unsigned FULL = 0xffffffffu;
+  extern __shared__ double ptf_smem[];
+  double* const sm = ptf_smem + threadIdx.x;
+  const LRows<NC> L{sm};
+  double* const sb = sm + NL * NEWTON_THREADS;   // accepted point beta = 2 sqrt(W) (B.1a)
+  double* const sp = sb + NC * NEWTON_THREADS;   // pending / best-so-far step
+  const int64_t N = io.N;
+  const int total = w.qcount[Q_STAB_NEWTON];
+  int* ticket = &w.qcount[Q_TICKET_STAB];
+  // ---- lane state (scalars only) ----
+  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
+  int n = 0, sidx = 0, iters = 0, tr_it = 0;
+  unsigned act = 0u;
+  PT3<NC> q;
+  q.spt = 0.0; q.sT = 0.0; q.pt = 0.0;
+  double tm = 0.0, rmax_acc = 0.0, pred = 0.0, Delta = 1.0, Delta_cap = 8.0, snorm = 0.0, Zw = 0.0, kept_sn = 0.0;
+  EtaSearch es;
+  es.start(1.0e-3);
+
+#pragma unroll 1
+  while (true) {
+    // ---- refill idle lanes from the ticket ----
+    if (__any_sync(FULL, !busy && !exhausted)) {
+      const int64_t tk = take_ticket(!busy && !exhausted, ticket);
+      if (tk >= 0) {
+        if (tk < total) {
+          const int item = w.q_stab_newton[tk];
+          n = item >> 1;
+          sidx = item & 1;
+          const double P = io.P[n], T = io.T[n];
+          { const double iT = rcp_fast(T); q.sT = sqrt_fast(T); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
+          act = (unsigned)w.actmask[n];
+#pragma unroll
+          for (int i = 0; i < NC; ++i) {
+            sb[i * NEWTON_THREADS] = w.lnW[((int64_t)sidx * NC + i) * N + n];   // k2_stab_ss left beta = 2 sqrt(W) here
+            sp[i * NEWTON_THREADS] = 0.0;
+          }
+          iters = w.tflags[(int64_t)sidx * N + n] >> TF_ITER_SHIFT;
+          tr_it = 0;
+          first = true;
+          reeval = false;
+          searching = false;
+          Zw = w.Zw[(int64_t)sidx * N + n];
+          busy = true;
+        } else {
+          exhausted = true;
+        }
+      }
+    }
+    if (!__any_sync(FULL, busy)) break;
+
+    double r[NC], Sv[NC];
+    double sumW = 0.0;
+    Eos e;
+    e.Z = Zw;
+    bool finish = false, fin_conv = false, fin_exact = false, fin_cap = false;
+    if (busy) {
+      // ---- evaluate tm and its gradient: at the trial point beta + s, or at beta while an eta search is pending ----
+      double W[NC], lp[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const double b = sb[i * NEWTON_THREADS], s = sp[i * NEWTON_THREADS];
+        const double h = 0.5 * (searching ? b : b + s);
+        W[i] = h * h;                                              // B.1d
+        r[i] = ((act >> i) & 1u) ? 2.0 * log_fast(h) : 0.0;        // ln W_i
+        sumW += W[i];
+      }
+      {
+        const double inv = rcp_fast(sumW);
+        double wn[NC];
+#pragma unroll
+        for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
+        lnphi_pt<NC, KIJ0>(S, q, wn, lp, Sv, e);
+      }
+      Zw = e.Z;
+      double rmax = 0.0, tm_new = 1.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - __ldg(&w.d[(int64_t)i * N + n]) : 0.0;
+        rmax = fmax(rmax, fabs(r[i]));
+        tm_new = fma(W[i], r[i] - 1.0, tm_new);
+      }
+      if (!searching) {
+        // ---- accept / reject the pending step (B.3) ----
+        bool accepted = true;
+        if (first) {
+          double bn = 0.0;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) bn = fma(W[i], 4.0, bn);   // |beta|^2 = 4 sum W
+          Delta = fmax(1.0, 0.5 * sqrt_fast(bn));
+          Delta_cap = 8.0 * Delta;
+        } else if (!reeval) {
+          const double act_red = tm_new - tm;
+          accepted = (act_red < 0.0) || (rmax < rmax_acc);
+          if (accepted) {
+            if (fabs(pred) > 1.0e-13) {
+              const double ratio = fabs(act_red * rcp_fast(pred));
+              if (ratio <= 0.25) Delta *= 0.5;
+              else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
+            }
+          } else {
+            Delta = 0.5 * fmin(Delta, snorm);
+            reeval = true;   // next trip re-evaluates at the accepted point (s = 0) and continues from there
+          }
+        }
+        if (!accepted) {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) sp[i * NEWTON_THREADS] = 0.0;
+        } else {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) { sb[i * NEWTON_THREADS] += sp[i * NEWTON_THREADS]; sp[i * NEWTON_THREADS] = 0.0; }
+          tm = tm_new;
+          rmax_acc = rmax;
+          first = false;
+          reeval = false;
+          // ---- convergence / cap, else start the eta search of a new trust-region iteration ----
+          if (rmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+          else if (tr_it >= o.stab_tr_iters) { finish = true; fin_cap = true; }
+          else {
+            tr_it++;
+            iters++;
+            es.start(1.0e-3);
+            kept_sn = 0.0;
+            searching = true;
+          }
+        }
+      }
+    }  // busy
+    __syncwarp();
+    if (busy && searching) {
+      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.1b): rows of H + eta I generated on the fly ----
+      const MC3 mc = mc3(e);
+      const double isq = rsqrt_fast(sumW);
+      const double sqW = sumW * isq;
+      const double c01p = mc.c01 * q.pt, c10p = mc.c10 * q.pt, c11p = mc.c11 * q.pt * q.pt, c12p = mc.c12 * q.pt, c21p = mc.c21 * q.pt;
+      double h[NC], hS[NC], hsa[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        h[i] = 0.5 * sb[i * NEWTON_THREADS] * isq;      // sqrt(w_i); B.2b: H_ij = sqrt(w_i w_j) M_ij + delta_ij (1 + r_i / 2)
+        hS[i] = h[i] * Sv[i];
+        hsa[i] = h[i] * sa_of<NC>(S, q, i);
+      }
+      double invd[NC], yv[NC], st[NC];
+      bool good = true;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        // G = C^T-contracted basis vector of row i: H_ij = G0 h_j + G1 (h_j wb_j) + G2 hS_j - q2 hsa_i omk_ij hsa_j
+        const double hb = h[i] * S.wb[i];
+        const double G0 = fma(hS[i], mc.c20, fma(hb, c10p, h[i] * mc.c00));
+        const double G1 = fma(hS[i], c21p, fma(hb, c11p, h[i] * c01p));
+        const double G2 = fma(hS[i], mc.c22, fma(hb, c12p, h[i] * mc.c02));
+        const double qs = mc.q2 * hsa[i];
+        double row[NC];
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+          if (j <= i) {
+            double a = fma(G2, hS[j], fma(G1, h[j] * S.wb[j], G0 * h[j]));
+            a = fma(-(KIJ0 ? qs : qs * S.omk[i * NC + j]), hsa[j], a);
+            row[j] = a;
+          }
+        }
+        row[i] += 1.0 + 0.5 * r[i] + es.eta;
+        chol_row<NC>(i, row, L, invd, yv, -h[i] * r[i] * sqW, good);   // rhs = -g_i = -beta_i r_i / 2 (B.2a)
+      }
+      chol_back<NC>(L, invd, yv, st);
+      double sn = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        sn = fma(st[i], st[i], sn);
+        if (((act >> i) & 1u) && !(sb[i * NEWTON_THREADS] + st[i] > 0.0)) good = false;
+      }
+      sn = sqrt_fast(sn);
+      good = good && (sn <= Delta);
+      const double eta_used = es.eta;
+      if (es.feed(good, sn, Delta, kept_sn)) {
+        double sg = 0.0;   // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { sp[i * NEWTON_THREADS] = st[i]; sg = fma(st[i], h[i] * r[i], sg); }
+        snorm = sn;
+        pred = 0.5 * sg * sqW - 0.5 * eta_used * sn * sn;
+        exact = (eta_used == 0.0);
+      }
+      if (es.phase == 4) { finish = true; fin_cap = true; searching = false; }
+      else if (es.phase == 3) {
+        searching = false;
+        double smax = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * NEWTON_THREADS]));
+        if (exact && smax < o.tol_newton_step) {
+          // quadratic-convergence finish: apply the full Newton step and stop
+          finish = true;
+          fin_conv = true;
+          fin_exact = true;
+          sumW = 0.0;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) {
+            const double b = sb[i * NEWTON_THREADS] + sp[i * NEWTON_THREADS];
+            sb[i * NEWTON_THREADS] = b;
+            sumW = fma(0.5 * b, 0.5 * b, sumW);
+          }
+        }
+      }
+    }
+    __syncwarp();
+    if (finish) {
+      // beta is stored; k_stab_decide turns it into ln W = 2 ln(beta/2) with all lanes active (TF_BETA)
+#pragma unroll
+      for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = sb[i * NEWTON_THREADS];
+      w.tm[(int64_t)sidx * N + n] = tm;
+      w.sumW[(int64_t)sidx * N + n] = sumW;
+      w.tflags[(int64_t)sidx * N + n] = (fin_conv ? TF_CONVERGED : 0) | (fin_exact ? TF_EXACT : 0) |
+                                        (fin_cap ? TF_CAPPED : 0) | TF_BETA | (iters << TF_ITER_SHIFT);
+      busy = false;
+    }
+  }
+}
+
+// ---- K6: phase-split trust-region Newton on G (B.4-B.5), persistent warps with lane refill --------
+// Variables n^V (B.4); H~ = theta_L^-1 ... in the code's normalisation: H_ij = wx Mx_ij + wy My_ij - 1/tt + delta_ij D_i (1/tt + eta),
+// tt = theta (1 - theta), wx = 1/(1 - theta), wy = 1/theta, D_i = z_i / (x_i y_i) (B.5b with the unit-total-mole M, reading C18).
+// Basis F_i = (1, B_i, Sx_i, Sy_i); the 4 x 4 coefficient matrix is wx Cx (+) wy Cy - E_00 / tt.
+template <int NC, bool KIJ0>
+__global__ void __launch_bounds__(NEWTON_THREADS, PTF_SPLITN_MINB)
+k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o, const __grid_constant__ Io io,
+                const __grid_constant__ Work w) {
+  constexpr int NL = NC * (NC - 1) / 2;
+  constexpr unsigned FULL = 0xffffffffu;
+  extern __shared__ double ptf_smem[];
+  double* const sm = ptf_smem + threadIdx.x;
+  const LRows<NC> L{sm};
+  double* const sn = sm + NL * NEWTON_THREADS;   // accepted n^V (of the minority phase, see k2_split_ss)
+  double* const sp = sn + NC * NEWTON_THREADS;   // pending / best-so-far step
+  double* const sz = sp + NC * NEWTON_THREADS;   // feed
+  double* const sg = sz + NC * NEWTON_THREADS;   // gradient (B.5a) at the evaluated point
+  double* const sD = sg + NC * NEWTON_THREADS;   // D_i = z_i / (x_i y_i)
+  const int64_t N = io.N;
+  const int total = w.qcount[Q_SPLIT_NEWTON];
+  int* ticket = &w.qcount[Q_TICKET_SPLIT];
+  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
+  int n = 0, tr_it = 0, status = 0;
+  unsigned act = 0u;
+  PT3<NC> q;
+  q.spt = 0.0; q.sT = 0.0; q.pt = 0.0;
+  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, Zx = 0.0, Zy = 0.0, kept_sn = 0.0;
+  EtaSearch es;
+  es.start(1.0);
+
+#pragma unroll 1
+  while (true) {
+    if (__any_sync(FULL, !busy && !exhausted)) {
+      const int64_t tk = take_ticket(!busy && !exhausted, ticket);
+      if (tk >= 0) {
+        if (tk < total) {
+          n = w.q_split_newton[tk];
+          const double P = io.P[n], T = io.T[n];
+          { const double iT = rcp_fast(T); q.sT = sqrt_fast(T); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
+          act = (unsigned)w.actmask[n];
+#pragma unroll
+          for (int i = 0; i < NC; ++i) {
+            sn[i * NEWTON_THREADS] = w.lnK[(int64_t)i * N + n];   // k2_split_ss left n^V here
+            sp[i * NEWTON_THREADS] = 0.0;
+            sz[i * NEWTON_THREADS] = __ldg(&w.zn[(int64_t)i * N + n]);
+          }
+          tr_it = 0;
+          status = 0;
+          first = true;
+          reeval = false;
+          searching = false;
+          Delta = 0.25;
+          Zx = w.Zxy[n];
+          Zy = w.Zxy[N + n];
+          busy = true;
+        } else {
+          exhausted = true;
+        }
+      }
+    }
+    if (!__any_sync(FULL, busy)) break;
+
+    double Sx[NC], Sy[NC];
+    double theta = 0.0;
+    Eos ex, ey;
+    bool finish = false, fin_conv = false;
+    if (busy) {
+      // ---- evaluate G (eq. 8) and its gradient (B.5a): at n^V + s, or at n^V while an eta search is pending ----
+      double x[NC], y[NC], lp[NC], gt[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const double v = searching ? sn[i * NEWTON_THREADS] : sn[i * NEWTON_THREADS] + sp[i * NEWTON_THREADS];
+        y[i] = v;
+        theta += v;
+      }
+      {
+        const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { const double v = y[i]; y[i] = v * it; x[i] = (sz[i * NEWTON_THREADS] - v) * il; }
+      }
+      ex.Z = Zx;
+      lnphi_pt<NC, KIJ0>(S, q, x, lp, Sx, ex);
+      Zx = ex.Z;
+      double G_new = 0.0, gmax = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        double fx = 0.0;
+        if ((act >> i) & 1u) { fx = log_fast(x[i]) + lp[i]; G_new = fma(x[i] * (1.0 - theta), fx, G_new); }
+        gt[i] = -fx;
+      }
+      ey.Z = Zy;
+      lnphi_pt<NC, KIJ0>(S, q, y, lp, Sy, ey);
+      Zy = ey.Z;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const bool a = (act >> i) & 1u;
+        if (a) { const double fy = log_fast(y[i]) + lp[i]; G_new = fma(y[i] * theta, fy, G_new); gt[i] += fy; }
+        gmax = fmax(gmax, fabs(gt[i]));
+        sg[i * NEWTON_THREADS] = gt[i];
+        sD[i * NEWTON_THREADS] = a ? sz[i * NEWTON_THREADS] * rcp_fast(x[i] * y[i]) : 1.0;
+        if (!a) { Sx[i] = 0.0; Sy[i] = 0.0; }
+      }
+      if (!searching) {
+        // ---- accept / reject ----
+        bool accepted = true;
+        if (!first && !reeval) {
+          const double act_red = G_new - G;
+          accepted = (act_red < 0.0) || (gmax < gmax_acc);
+          if (accepted) {
+            if (fabs(pred) > 1.0e-13) {
+              const double ratio = fabs(act_red * rcp_fast(pred));
+              if (ratio <= 0.25) Delta *= 0.5;
+              else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
+            }
+          } else {
+            Delta = 0.5 * fmin(Delta, snorm);
+            reeval = true;
+          }
+        }
+        if (!accepted) {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) sp[i * NEWTON_THREADS] = 0.0;
+        } else {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) { sn[i * NEWTON_THREADS] += sp[i * NEWTON_THREADS]; sp[i * NEWTON_THREADS] = 0.0; }
+          G = G_new;
+          gmax_acc = gmax;
+          first = false;
+          reeval = false;
+          if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+          else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
+          else {
+            tr_it++;
+            es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
+            kept_sn = 0.0;
+            searching = true;
+          }
+        }
+      }
+    }  // busy
+    __syncwarp();
+    if (busy && searching) {
+      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.4a) ----
+      const MC3 mx = mc3(ex), my = mc3(ey);
+      const double tt = theta * (1.0 - theta), itt = rcp_fast(tt);
+      const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
+      const double pt = q.pt;
+      // 4 x 4 coefficients in the basis (1, wb_i, Sx_i, Sy_i) (pt folded into the wb rows / columns)
+      const double c00 = fma(wx, mx.c00, wy * my.c00) - itt;
+      const double c01 = fma(wx, mx.c01, wy * my.c01) * pt, c10 = fma(wx, mx.c10, wy * my.c10) * pt;
+      const double c11 = fma(wx, mx.c11, wy * my.c11) * pt * pt;
+      const double c02 = wx * mx.c02, c20 = wx * mx.c20, c12 = wx * mx.c12 * pt, c21 = wx * mx.c21 * pt, c22 = wx * mx.c22;
+      const double c03 = wy * my.c02, c30 = wy * my.c20, c13 = wy * my.c12 * pt, c31 = wy * my.c21 * pt, c33 = wy * my.c22;
+      const double qa = fma(wx, mx.q2, wy * my.q2);
+      const double deta = itt + es.eta;
+      double one[NC], sa[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const bool a = (act >> i) & 1u;
+        one[i] = a ? 1.0 : 0.0;
+        sa[i] = a ? sa_of<NC>(S, q, i) : 0.0;
+      }
+      double invd[NC], yv[NC], st[NC];
+      bool good = true;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const double ob = one[i] * S.wb[i];
+        const double G0 = fma(Sy[i], c30, fma(Sx[i], c20, fma(ob, c10, one[i] * c00)));
+        const double G1 = fma(Sy[i], c31, fma(Sx[i], c21, fma(ob, c11, one[i] * c01)));
+        const double G2 = fma(Sx[i], c22, fma(ob, c12, one[i] * c02));
+        const double G3 = fma(Sy[i], c33, fma(ob, c13, one[i] * c03));
+        const double qs = qa * sa[i];
+        double row[NC];
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+          if (j <= i) {
+            double a = fma(G3, Sy[j], fma(G2, Sx[j], fma(G1, one[j] * S.wb[j], G0 * one[j])));
+            a = fma(-(KIJ0 ? qs : qs * S.omk[i * NC + j]), sa[j], a);
+            row[j] = a;
+          }
+        }
+        row[i] = fma(sD[i * NEWTON_THREADS], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
+        chol_row<NC>(i, row, L, invd, yv, -sg[i * NEWTON_THREADS], good);
+      }
+      chol_back<NC>(L, invd, yv, st);
+      double snrm = 0.0, sds = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        snrm = fma(st[i], st[i], snrm);
+        sds = fma(st[i] * st[i], sD[i * NEWTON_THREADS], sds);
+        if ((act >> i) & 1u) {
+          const double nv = sn[i * NEWTON_THREADS] + st[i];
+          if (!(nv > 0.0) || !(nv < sz[i * NEWTON_THREADS])) good = false;
+        }
+      }
+      snrm = sqrt_fast(snrm);
+      good = good && (snrm <= Delta);
+      const double eta_used = es.eta;
+      if (es.feed(good, snrm, Delta, kept_sn)) {
+        double sgd = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { sp[i * NEWTON_THREADS] = st[i]; sgd = fma(st[i], sg[i * NEWTON_THREADS], sgd); }
+        snorm = snrm;
+        pred = 0.5 * sgd - 0.5 * eta_used * sds;
+        exact = (eta_used == 0.0);
+      }
+      if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
+      else if (es.phase == 3) {
+        searching = false;
+        double smax = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * NEWTON_THREADS]));
+        if (exact && smax < o.tol_newton_step) {
+          finish = true;
+          fin_conv = true;
+#pragma unroll
+          for (int i = 0; i < NC; ++i) sn[i * NEWTON_THREADS] += sp[i * NEWTON_THREADS];
+        }
+      }
+    }
+    __syncwarp();
+    if (finish) {
+      // compositions of the accepted point
+      double z[NC], x[NC], y[NC], lnK[NC];
+      theta = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) { z[i] = sz[i * NEWTON_THREADS]; y[i] = sn[i * NEWTON_THREADS]; theta += y[i]; }
+      {
+        const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { const double v = y[i]; y[i] = v * it; x[i] = (z[i] - v) * il; }
+      }
+      // trivial collapse x = y (max |ln K| < 1e-9): |y/x - 1| is the same test to first order and needs no logarithm
+      double mkn = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+        if ((act >> i) & 1u) mkn = fmax(mkn, fabs(y[i] - x[i]) * rcp_fast(x[i]));
+      const bool trivial = mkn < 1.0e-9;
+      if (io.lnK) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
+      } else {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
+      }
+      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, Zx, Zy);
+      busy = false;
+    }
+  }
+}
+
+}  // namespace ptf

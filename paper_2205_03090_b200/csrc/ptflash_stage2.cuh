@@ -221,8 +221,11 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
   }
 }
 
+#ifndef PTF_TRI_SMEM
+#define PTF_TRI_SMEM 1   // packed Newton matrices in shared memory (440 B per thread at nc = 10) instead of registers
+#endif
 #ifndef PTF_NEWTON_MINB
-#define PTF_NEWTON_MINB 2
+#define PTF_NEWTON_MINB 3
 #endif
 // ---- lane refill ----------------------------------------------------------------------------------
 // Lanes with want == true take consecutive tickets; returns the ticket (>= total means the queue is exhausted).
@@ -405,7 +408,12 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __g
       double g[NC], st[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) g[i] = 0.5 * beta[i] * r[i];   // B.2a
+#if PTF_TRI_SMEM
+      extern __shared__ double ptf_smem[];
+      TriSmem<128> Lm{ptf_smem + threadIdx.x};
+#else
       double Lm[NT];
+#endif
 #pragma unroll
       for (int j = 0; j < NC; ++j) {
         const double ej = bi[j] * mc.invB;
@@ -705,7 +713,12 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
       double D[NC], st[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) D[i] = ((act >> i) & 1u) ? z[i] * rcp_fast(x[i] * y[i]) : 1.0;
+#if PTF_TRI_SMEM
+      extern __shared__ double ptf_smem[];
+      TriSmem<128> Lm{ptf_smem + threadIdx.x};
+#else
       double Lm[NT];
+#endif
 #pragma unroll
       for (int j = 0; j < NC; ++j) {
         const double exj = bi[j] * mx.invB, eyj = bi[j] * my.invB;
@@ -791,6 +804,14 @@ __global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __
   }
 }
 
+}  // namespace ptf
+#include "ptflash_newton.cuh"
+namespace ptf {
+
+#ifndef PTF_NEWTON_V3
+#define PTF_NEWTON_V3 1   // 1: matrix-free rows + shared-memory Cholesky (ptflash_newton.cuh); 0: register-resident k2_* kernels
+#endif
+
 template <int NC, bool KIJ0>
 int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work& w_in, int sms, cudaStream_t st) {
   const int threads = 128;
@@ -802,21 +823,62 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
   const unsigned gP = (unsigned)(sms * PTF_NEWTON_MINB);   // persistent refill kernels: a few CTAs per SM pull tickets
   Work w = w_in;
+  const size_t tri_bytes = PTF_TRI_SMEM ? (size_t)(NC * (NC + 1) / 2) * threads * sizeof(double) : 0;
+  if (tri_bytes > 48 * 1024) {
+    cudaFuncSetAttribute(k2_stab_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tri_bytes);
+    cudaFuncSetAttribute(k2_split_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tri_bytes);
+  }
+#if PTF_NEWTON_V3
+  // persistent refill kernels: as many CTAs per SM as registers and shared memory allow (queried once per instantiation)
+  const size_t stab_bytes = (size_t)stabn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
+  const size_t split_bytes = (size_t)splitn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
+  static int stab_cta = 0, split_cta = 0;
+  if (stab_cta == 0) {
+    cudaFuncSetAttribute(k3_stab_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stab_bytes);
+    cudaFuncSetAttribute(k3_split_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)split_bytes);
+    int a = 0, b = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k3_stab_newton<NC, KIJ0>, NEWTON_THREADS, stab_bytes);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k3_split_newton<NC, KIJ0>, NEWTON_THREADS, split_bytes);
+    stab_cta = a > 0 ? a : 1;
+    split_cta = b > 0 ? b : 1;
+  }
+#endif
+  // optional stage profiling: one event before the first kernel and one after every stage kernel
+  cudaEvent_t* ev = (cudaEvent_t*)o.prof_events;
+  int nev = 0;
+  auto mark = [&]() { if (ev && nev < PTF_MAX_STAGE_EVENTS) cudaEventRecord(ev[nev++], st); };
+  mark();
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  mark();
   int launches = 1;
   const int passes = (io.flags && io.lnK0) ? 2 : 1;   // pass 1: cold re-flash of mixtures whose skip-stability hint failed
   for (int pass = 0; pass < passes; ++pass) {
     w.pass = pass;
     if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
     k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+    mark();
     k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
-    k2_stab_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
+    mark();
+#if PTF_NEWTON_V3
+    k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), threads, stab_bytes, st>>>(s, o, io, w);
+#else
+    k2_stab_newton<NC, KIJ0><<<gP, threads, tri_bytes, st>>>(s, o, io, w);
+#endif
+    mark();
     k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    mark();
     k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
-    k2_split_newton<NC, KIJ0><<<gP, threads, 0, st>>>(s, o, io, w);
+    mark();
+#if PTF_NEWTON_V3
+    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), threads, split_bytes, st>>>(s, o, io, w);
+#else
+    k2_split_newton<NC, KIJ0><<<gP, threads, tri_bytes, st>>>(s, o, io, w);
+#endif
     k_finalize_counters<<<1, 32, 0, st>>>(w);
+    mark();
     launches += 7;
   }
+  if (o.prof_count) *o.prof_count = nev;
   return cudaGetLastError() == cudaSuccess ? launches : -1;
 }
 
