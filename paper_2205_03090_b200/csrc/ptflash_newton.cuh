@@ -21,6 +21,16 @@ namespace ptf {
 
 constexpr int NEWTON_THREADS = 128;
 
+#ifndef PTF_NEWTON_CTA_SYNC
+#define PTF_NEWTON_CTA_SYNC 1
+#endif
+#ifdef PTF_DEBUG_COUNT
+__device__ unsigned long long g_dbg[16];
+#define PTF_DBG(k, v) atomicAdd(&g_dbg[k], (unsigned long long)(v))
+#else
+#define PTF_DBG(k, v)
+#endif
+
 // Coefficients of M_ij = sum_ab F_ia C[a][b] F_jb - q2 A_ij with F_i = (1, B_i, S_i) (B_i, not B_i/B).
 // Derivation: DESIGN.md section 2 (M_ij = e_i p_j + c_j - Dq_j u_i + 2q(S_i - A_ij) with p, c, Dq affine in
 // e_j - 1 and S_j - A, u_i = 2 S_i - A e_i, e_i = B_i/B).
@@ -114,7 +124,7 @@ __device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&inv
 template <int NC>
 constexpr int stabn_smem_doubles() { return NC * (NC - 1) / 2 + 2 * NC; }   // per thread: L, beta, pending step
 template <int NC>
-constexpr int splitn_smem_doubles() { return NC * (NC - 1) / 2 + 5 * NC; }  // per thread: L, n^V, pending step, z, g, D
+constexpr int splitn_smem_doubles() { return NC * (NC - 1) / 2 + 6 * NC; }  // per thread: L, n^V, pending step, g, D, S(x), S(y)
 
 // ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
 template <int NC, bool KIJ0>
@@ -171,7 +181,13 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         }
       }
     }
+#if PTF_NEWTON_CTA_SYNC
+    // CTA-wide trip alignment: the four warps of a CTA walk the (larger than the instruction cache) trip body together,
+    // so one instruction fetch serves all of them
+    if (!__syncthreads_or(busy)) break;
+#else
     if (!__any_sync(FULL, busy)) break;
+#endif
 
     double r[NC], Sv[NC];
     double sumW = 0.0;
@@ -340,23 +356,27 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
 }
 
 // ---- K6: phase-split trust-region Newton on G (B.4-B.5), persistent warps with lane refill --------
-// Variables n^V (B.4); H~ = theta_L^-1 ... in the code's normalisation: H_ij = wx Mx_ij + wy My_ij - 1/tt + delta_ij D_i (1/tt + eta),
-// tt = theta (1 - theta), wx = 1/(1 - theta), wy = 1/theta, D_i = z_i / (x_i y_i) (B.5b with the unit-total-mole M, reading C18).
-// Basis F_i = (1, B_i, Sx_i, Sy_i); the 4 x 4 coefficient matrix is wx Cx (+) wy Cy - E_00 / tt.
+// Variables n^V (B.4).  In the code's normalisation H_ij = wx Mx_ij + wy My_ij - 1/tt + delta_ij D_i (1/tt + eta),
+// tt = theta (1 - theta), wx = 1/(1 - theta), wy = 1/theta, D_i = z_i / (x_i y_i) (B.5b with the unit-total-mole M,
+// reading C18).  Basis F_i = (1, B_i, Sx_i, Sy_i); the 4 x 4 coefficient matrix is wx Cx (+) wy Cy - E_00 / tt.
+//
+// The evaluation of a trip (two lnphi, one code copy looped over the phases) leaves S(x), S(y), the gradient and D in
+// shared memory, so a lane that has to retry with a larger eta does not evaluate again.
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(NEWTON_THREADS, PTF_SPLITN_MINB)
 k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o, const __grid_constant__ Io io,
                 const __grid_constant__ Work w) {
   constexpr int NL = NC * (NC - 1) / 2;
+  constexpr int T = NEWTON_THREADS;
   constexpr unsigned FULL = 0xffffffffu;
   extern __shared__ double ptf_smem[];
   double* const sm = ptf_smem + threadIdx.x;
   const LRows<NC> L{sm};
-  double* const sn = sm + NL * NEWTON_THREADS;   // accepted n^V (of the minority phase, see k2_split_ss)
-  double* const sp = sn + NC * NEWTON_THREADS;   // pending / best-so-far step
-  double* const sz = sp + NC * NEWTON_THREADS;   // feed
-  double* const sg = sz + NC * NEWTON_THREADS;   // gradient (B.5a) at the evaluated point
-  double* const sD = sg + NC * NEWTON_THREADS;   // D_i = z_i / (x_i y_i)
+  double* const sn = sm + NL * T;    // accepted n^V (of the minority phase, see k2_split_ss)
+  double* const sp = sn + NC * T;    // pending step
+  double* const sg = sp + NC * T;    // gradient (B.5a) at the evaluated point
+  double* const sD = sg + NC * T;    // D_i = z_i / (x_i y_i)
+  double* const sS = sD + NC * T;    // S(x) [NC], S(y) [NC]
   const int64_t N = io.N;
   const int total = w.qcount[Q_SPLIT_NEWTON];
   int* ticket = &w.qcount[Q_TICKET_SPLIT];
@@ -365,9 +385,12 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   unsigned act = 0u;
   PT3<NC> q;
   q.spt = 0.0; q.sT = 0.0; q.pt = 0.0;
-  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, Zx = 0.0, Zy = 0.0, kept_sn = 0.0;
+  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, kept_sn = 0.0, theta = 0.5;
   EtaSearch es;
   es.start(1.0);
+  Eos ex, ey;   // cubic scalars of the two phases at the evaluated point (Z doubles as the warm start)
+  ex.A = ex.B = ex.Z = ex.q = ex.L = ex.lnZmB = 0.0;
+  ey = ex;
 
 #pragma unroll 1
   while (true) {
@@ -376,14 +399,13 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       if (tk >= 0) {
         if (tk < total) {
           n = w.q_split_newton[tk];
-          const double P = io.P[n], T = io.T[n];
-          { const double iT = rcp_fast(T); q.sT = sqrt_fast(T); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
+          const double P = io.P[n], Tk = io.T[n];
+          { const double iT = rcp_fast(Tk); q.sT = sqrt_fast(Tk); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
           act = (unsigned)w.actmask[n];
 #pragma unroll
           for (int i = 0; i < NC; ++i) {
-            sn[i * NEWTON_THREADS] = w.lnK[(int64_t)i * N + n];   // k2_split_ss left n^V here
-            sp[i * NEWTON_THREADS] = 0.0;
-            sz[i * NEWTON_THREADS] = __ldg(&w.zn[(int64_t)i * N + n]);
+            sn[i * T] = w.lnK[(int64_t)i * N + n];   // k2_split_ss left n^V here
+            sp[i * T] = 0.0;
           }
           tr_it = 0;
           status = 0;
@@ -391,97 +413,102 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           reeval = false;
           searching = false;
           Delta = 0.25;
-          Zx = w.Zxy[n];
-          Zy = w.Zxy[N + n];
+          ex.Z = w.Zxy[n];
+          ey.Z = w.Zxy[N + n];
           busy = true;
         } else {
           exhausted = true;
         }
       }
     }
+#if PTF_NEWTON_CTA_SYNC
+    // CTA-wide trip alignment: the four warps of a CTA walk the (larger than the instruction cache) trip body together,
+    // so one instruction fetch serves all of them
+    if (!__syncthreads_or(busy)) break;
+#else
     if (!__any_sync(FULL, busy)) break;
+#endif
 
-    double Sx[NC], Sy[NC];
-    double theta = 0.0;
-    Eos ex, ey;
     bool finish = false, fin_conv = false;
-    if (busy) {
-      // ---- evaluate G (eq. 8) and its gradient (B.5a): at n^V + s, or at n^V while an eta search is pending ----
-      double x[NC], y[NC], lp[NC], gt[NC];
+    if (busy && !searching) {
+      // ---- evaluate G (eq. 8) and its gradient (B.5a) at n^V + s ----
+      PTF_DBG(0, 1);
+      theta = 0.0;
 #pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        const double v = searching ? sn[i * NEWTON_THREADS] : sn[i * NEWTON_THREADS] + sp[i * NEWTON_THREADS];
-        y[i] = v;
-        theta += v;
-      }
-      {
-        const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
-#pragma unroll
-        for (int i = 0; i < NC; ++i) { const double v = y[i]; y[i] = v * it; x[i] = (sz[i * NEWTON_THREADS] - v) * il; }
-      }
-      ex.Z = Zx;
-      lnphi_pt<NC, KIJ0>(S, q, x, lp, Sx, ex);
-      Zx = ex.Z;
+      for (int i = 0; i < NC; ++i) theta += sn[i * T] + sp[i * T];
+      const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
       double G_new = 0.0, gmax = 0.0;
+#pragma unroll 1
+      for (int ph = 0; ph < 2; ++ph) {
+        double c[NC], lp[NC], Sv[NC];
 #pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        double fx = 0.0;
-        if ((act >> i) & 1u) { fx = log_fast(x[i]) + lp[i]; G_new = fma(x[i] * (1.0 - theta), fx, G_new); }
-        gt[i] = -fx;
-      }
-      ey.Z = Zy;
-      lnphi_pt<NC, KIJ0>(S, q, y, lp, Sy, ey);
-      Zy = ey.Z;
+        for (int i = 0; i < NC; ++i) {
+          const double v = sn[i * T] + sp[i * T];
+          c[i] = ph ? v * it : (__ldg(&w.zn[(int64_t)i * N + n]) - v) * il;
+        }
+        Eos e;
+        e.Z = ph ? ey.Z : ex.Z;
+        lnphi_pt<NC, KIJ0>(S, q, c, lp, Sv, e);
+        if (ph) ey = e; else ex = e;
+        const double wph = ph ? theta : 1.0 - theta;
 #pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        const bool a = (act >> i) & 1u;
-        if (a) { const double fy = log_fast(y[i]) + lp[i]; G_new = fma(y[i] * theta, fy, G_new); gt[i] += fy; }
-        gmax = fmax(gmax, fabs(gt[i]));
-        sg[i * NEWTON_THREADS] = gt[i];
-        sD[i * NEWTON_THREADS] = a ? sz[i * NEWTON_THREADS] * rcp_fast(x[i] * y[i]) : 1.0;
-        if (!a) { Sx[i] = 0.0; Sy[i] = 0.0; }
-      }
-      if (!searching) {
-        // ---- accept / reject ----
-        bool accepted = true;
-        if (!first && !reeval) {
-          const double act_red = G_new - G;
-          accepted = (act_red < 0.0) || (gmax < gmax_acc);
-          if (accepted) {
-            if (fabs(pred) > 1.0e-13) {
-              const double ratio = fabs(act_red * rcp_fast(pred));
-              if (ratio <= 0.25) Delta *= 0.5;
-              else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
-            }
+        for (int i = 0; i < NC; ++i) {
+          const bool a = (act >> i) & 1u;
+          const double f = a ? log_fast(c[i]) + lp[i] : 0.0;
+          G_new = fma(c[i] * wph, f, G_new);
+          sS[(ph * NC + i) * T] = a ? Sv[i] : 0.0;
+          if (ph == 0) {
+            sg[i * T] = -f;
+            sD[i * T] = c[i];
           } else {
-            Delta = 0.5 * fmin(Delta, snorm);
-            reeval = true;
-          }
-        }
-        if (!accepted) {
-#pragma unroll
-          for (int i = 0; i < NC; ++i) sp[i * NEWTON_THREADS] = 0.0;
-        } else {
-#pragma unroll
-          for (int i = 0; i < NC; ++i) { sn[i * NEWTON_THREADS] += sp[i * NEWTON_THREADS]; sp[i * NEWTON_THREADS] = 0.0; }
-          G = G_new;
-          gmax_acc = gmax;
-          first = false;
-          reeval = false;
-          if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
-          else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
-          else {
-            tr_it++;
-            es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
-            kept_sn = 0.0;
-            searching = true;
+            const double g = sg[i * T] + f;
+            sg[i * T] = g;
+            gmax = fmax(gmax, fabs(g));
+            sD[i * T] = a ? __ldg(&w.zn[(int64_t)i * N + n]) * rcp_fast(sD[i * T] * c[i]) : 1.0;
           }
         }
       }
-    }  // busy
+      // ---- accept / reject ----
+      bool accepted = true;
+      if (!first && !reeval) {
+        const double act_red = G_new - G;
+        accepted = (act_red < 0.0) || (gmax < gmax_acc);
+        if (accepted) {
+          if (fabs(pred) > 1.0e-13) {
+            const double ratio = fabs(act_red * rcp_fast(pred));
+            if (ratio <= 0.25) Delta *= 0.5;
+            else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
+          }
+        } else {
+          Delta = 0.5 * fmin(Delta, snorm);
+          reeval = true;
+          PTF_DBG(1, 1);
+        }
+      }
+      if (!accepted) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) sp[i * T] = 0.0;
+      } else {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) { sn[i * T] += sp[i * T]; sp[i * T] = 0.0; }
+        G = G_new;
+        gmax_acc = gmax;
+        first = false;
+        reeval = false;
+        if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
+        else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
+        else {
+          tr_it++;
+          es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
+          kept_sn = 0.0;
+          searching = true;
+        }
+      }
+    }
     __syncwarp();
     if (busy && searching) {
-      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.4a) ----
+      // ---- ONE attempt of the restricted-step sub-problem at eta (B.4a) ----
+      PTF_DBG(2, 1);
       const MC3 mx = mc3(ex), my = mc3(ey);
       const double tt = theta * (1.0 - theta), itt = rcp_fast(tt);
       const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
@@ -494,15 +521,17 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       const double c03 = wy * my.c02, c30 = wy * my.c20, c13 = wy * my.c12 * pt, c31 = wy * my.c21 * pt, c33 = wy * my.c22;
       const double qa = fma(wx, mx.q2, wy * my.q2);
       const double deta = itt + es.eta;
-      double one[NC], sa[NC];
+      double one[NC], sa[NC], Sx[NC], Sy[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
         const bool a = (act >> i) & 1u;
         one[i] = a ? 1.0 : 0.0;
         sa[i] = a ? sa_of<NC>(S, q, i) : 0.0;
+        Sx[i] = sS[i * T];
+        Sy[i] = sS[(NC + i) * T];
       }
       double invd[NC], yv[NC], st[NC];
-      bool good = true;
+      bool pd = true;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
         const double ob = one[i] * S.wb[i];
@@ -520,42 +549,44 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
             row[j] = a;
           }
         }
-        row[i] = fma(sD[i * NEWTON_THREADS], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
-        chol_row<NC>(i, row, L, invd, yv, -sg[i * NEWTON_THREADS], good);
+        row[i] = fma(sD[i * T], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
+        chol_row<NC>(i, row, L, invd, yv, -sg[i * T], pd);
       }
       chol_back<NC>(L, invd, yv, st);
-      double snrm = 0.0, sds = 0.0;
+      bool good = pd;
+      double s2 = 0.0, sds = 0.0, sgd = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
-        snrm = fma(st[i], st[i], snrm);
-        sds = fma(st[i] * st[i], sD[i * NEWTON_THREADS], sds);
+        s2 = fma(st[i], st[i], s2);
+        sds = fma(st[i] * st[i], sD[i * T], sds);
+        sgd = fma(st[i], sg[i * T], sgd);
         if ((act >> i) & 1u) {
-          const double nv = sn[i * NEWTON_THREADS] + st[i];
-          if (!(nv > 0.0) || !(nv < sz[i * NEWTON_THREADS])) good = false;
+          const double nv = sn[i * T] + st[i];
+          if (!(nv > 0.0) || !(nv < __ldg(&w.zn[(int64_t)i * N + n]))) good = false;
         }
       }
-      snrm = sqrt_fast(snrm);
-      good = good && (snrm <= Delta);
+      const double sl = sqrt_fast(s2);
+      good = good && (sl <= Delta);
       const double eta_used = es.eta;
-      if (es.feed(good, snrm, Delta, kept_sn)) {
-        double sgd = 0.0;
+      if (es.feed(good, sl, Delta, kept_sn)) {
 #pragma unroll
-        for (int i = 0; i < NC; ++i) { sp[i * NEWTON_THREADS] = st[i]; sgd = fma(st[i], sg[i * NEWTON_THREADS], sgd); }
-        snorm = snrm;
+        for (int i = 0; i < NC; ++i) sp[i * T] = st[i];
+        snorm = sl;
         pred = 0.5 * sgd - 0.5 * eta_used * sds;
         exact = (eta_used == 0.0);
       }
+      if (!good) PTF_DBG(5, 1);
       if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
       else if (es.phase == 3) {
         searching = false;
         double smax = 0.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * NEWTON_THREADS]));
+        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * T]));
         if (exact && smax < o.tol_newton_step) {
           finish = true;
           fin_conv = true;
 #pragma unroll
-          for (int i = 0; i < NC; ++i) sn[i * NEWTON_THREADS] += sp[i * NEWTON_THREADS];
+          for (int i = 0; i < NC; ++i) sn[i * T] += sp[i * T];
         }
       }
     }
@@ -565,7 +596,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       double z[NC], x[NC], y[NC], lnK[NC];
       theta = 0.0;
 #pragma unroll
-      for (int i = 0; i < NC; ++i) { z[i] = sz[i * NEWTON_THREADS]; y[i] = sn[i * NEWTON_THREADS]; theta += y[i]; }
+      for (int i = 0; i < NC; ++i) { z[i] = __ldg(&w.zn[(int64_t)i * N + n]); y[i] = sn[i * T]; theta += y[i]; }
       {
         const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
 #pragma unroll
@@ -584,7 +615,11 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
 #pragma unroll
         for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
       }
-      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, Zx, Zy);
+      PTF_DBG(6, 1);
+      PTF_DBG(7, fin_conv ? 0 : 1);
+      PTF_DBG(8, trivial ? 1 : 0);
+      PTF_DBG(9, tr_it);
+      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, ex.Z, ey.Z);
       busy = false;
     }
   }
