@@ -111,7 +111,10 @@ int ptflash_destroy(ptflash_handle_t h);
 enum {
   PTFLASH_OPT_TOL_SS = 0,          /* SS residual target, stability and split [1e-10] */
   PTFLASH_OPT_TOL_NEWTON_G = 1,    /* Newton gradient target [1e-12] */
-  PTFLASH_OPT_TOL_NEWTON_STEP = 2, /* Newton step below which the full step is applied and iteration stops [1e-10] */
+  PTFLASH_OPT_TOL_NEWTON_STEP = 2, /* phase-split Newton: a full (eta = 0) step with max_i |s_i| / min(n^V_i, n^L_i) below this is
+                                      applied and the iteration stops; the error left behind is second order [1e-7, relative:
+                                      next to a phase boundary the mole numbers of the incipient phase are themselves ~1e-9,
+                                      so an absolute threshold would stop on an unconverged point] */
   PTFLASH_OPT_PROBE_MARGIN = 3,    /* probe: "negative" means < -margin [1e-8] */
   PTFLASH_OPT_TRIVIAL_TOL = 4,     /* trivial stability solution: max|lnW - lnz| < tol [1e-6] */
   PTFLASH_OPT_BAND = 5,            /* near-zero TPD band [1e-9] */
@@ -124,7 +127,9 @@ enum {
   PTFLASH_OPT_SS_CAP = 12,         /* [100000]: SS cap when Newton is off or theta stays outside (0,1) */
   PTFLASH_OPT_ENGINE = 13,         /* [1] 1 = staged persistent kernels with work queues; 0 = single run-to-completion kernel */
   PTFLASH_OPT_STAGE_PROFILE = 14,  /* [0] 1 = record a CUDA event between the stage kernels (engine 1), see ptflash_get_stage_ms */
-  PTFLASH_NUM_OPTS = 15
+  PTFLASH_OPT_TOL_NEWTON_STEP_STAB = 15, /* the same for the stability Newton, whose result enters only through tm (itself
+                                            second order in the error of W) and the K seed [1e-6] */
+  PTFLASH_NUM_OPTS = 16
 };
 int ptflash_set_option(ptflash_handle_t h, int key, double value);
 int ptflash_get_option(ptflash_handle_t h, int key, double* value);

@@ -20,7 +20,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 
-const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0};
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6};
 
 }  // namespace
 
@@ -53,6 +53,7 @@ ptf::Opt make_opt(const double* o) {
   r.tol_ss = o[PTFLASH_OPT_TOL_SS];
   r.tol_newton_g = o[PTFLASH_OPT_TOL_NEWTON_G];
   r.tol_newton_step = o[PTFLASH_OPT_TOL_NEWTON_STEP];
+  r.tol_newton_step_stab = o[PTFLASH_OPT_TOL_NEWTON_STEP_STAB];
   r.probe_margin = o[PTFLASH_OPT_PROBE_MARGIN];
   r.trivial_tol = o[PTFLASH_OPT_TRIVIAL_TOL];
   r.band = o[PTFLASH_OPT_BAND];

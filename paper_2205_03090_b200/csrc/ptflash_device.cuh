@@ -24,7 +24,7 @@ namespace ptf {
 // parameter blocks
 // ------------------------------------------------------------------------------------------------
 struct Opt {
-  double tol_ss, tol_newton_g, tol_newton_step, probe_margin, trivial_tol, band;
+  double tol_ss, tol_newton_g, tol_newton_step, tol_newton_step_stab, probe_margin, trivial_tol, band;
   int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap;
   // host only: cudaEvent_t[PTF_MAX_STAGE_EVENTS] recorded between the stage kernels when stage profiling is on (else null)
   void* prof_events;

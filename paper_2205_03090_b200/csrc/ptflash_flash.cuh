@@ -139,7 +139,7 @@ __device__ __noinline__ void stab_newton(const Sys<NC>& S, const Opt& o, const M
     double smax = 0.0;
 #pragma unroll
     for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sstep[i]));
-    if (eta == 0.0 && smax < o.tol_newton_step) {
+    if (eta == 0.0 && smax < o.tol_newton_step_stab) {
       // quadratic-convergence finish: apply the full Newton step and stop
       double sumW = 0.0;
 #pragma unroll
@@ -344,9 +344,10 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
     }
     double eta = 0.0, snorm = 0.0;
     if (!tr_subproblem<NC>(H, gt, D, Delta, 1.0e-3 * itt, nV, m.z, act, sstep, eta, snorm, Lc)) { st.status |= ST_SPLIT_CAP; break; }
-    double smax = 0.0;
+    double smax = 0.0;   // largest step relative to the smaller of the two mole numbers n^V_i, n^L_i = z_i - n^V_i
 #pragma unroll
-    for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sstep[i]));
+    for (int i = 0; i < NC; ++i)
+      if (act[i]) smax = fmax(smax, fabs(sstep[i]) / fmin(nV[i], m.z[i] - nV[i]));
     if (eta == 0.0 && smax < o.tol_newton_step) {
       theta = 0.0;
 #pragma unroll

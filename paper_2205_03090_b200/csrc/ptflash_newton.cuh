@@ -66,18 +66,21 @@ __device__ __forceinline__ MC3 mc3(const Eos& e) {
 }
 
 // strict lower triangle of the Cholesky factor, one column of shared memory per thread
+// (volatile: without it the compiler forwards every stored L[i][j] to its later loads -- all indices are compile-time --
+// and the factor is back in registers, 255 of them plus spills)
 template <int NC>
 struct LRows {
-  double* p;
-  __device__ __forceinline__ double& at(int i, int j) const { return p[(i * (i - 1) / 2 + j) * NEWTON_THREADS]; }
+  volatile double* p;
+  __device__ __forceinline__ volatile double& at(int i, int j) const { return p[(i * (i - 1) / 2 + j) * NEWTON_THREADS]; }
 };
 
-// Eliminate row i of a row-wise Cholesky.  On entry row[0..i] = H[i][0..i]; on exit row[j < i] = L[i][j] (also stored
-// to shared memory), invd[i] = 1 / L[i][i], yv[i] = forward substitution of rhs.  `i` is a compile-time constant
-// after unrolling, so every j < i / k < j test disappears.
+// Eliminate row i of a row-wise Cholesky.  On entry row[0..i] = H[i][0..i]; on exit row[j < i] = L[i][j], invd[i] = 1 / L[i][i],
+// yv[i] = forward substitution of rhs.  Rows 1 .. NC-2 are stored to shared memory; the LAST row is never read by a later
+// row, so it stays in registers and the first step of the back substitution is taken right here (s[NC-1], yv updated).
+// `i` is a compile-time constant after unrolling, so every j < i / k < j test disappears.
 template <int NC>
 __device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const LRows<NC>& L, double (&invd)[NC],
-                                         double (&yv)[NC], const double rhs, bool& pd) {
+                                         double (&yv)[NC], double (&s)[NC], const double rhs, bool& pd) {
 #pragma unroll
   for (int j = 0; j < NC; ++j) {
     if (j < i) {
@@ -96,19 +99,27 @@ __device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const L
   const double inv = rsqrt_fast(acc);
   invd[i] = inv;
   yv[i] = a * inv;
+  if (i < NC - 1) {
 #pragma unroll
-  for (int j = 0; j < NC; ++j)
-    if (j < i) L.at(i, j) = row[j];
+    for (int j = 0; j < NC; ++j)
+      if (j < i) L.at(i, j) = row[j];
+  } else {
+    const double sl = yv[i] * inv;
+    s[i] = sl;
+#pragma unroll
+    for (int k = 0; k < NC; ++k)
+      if (k < i) yv[k] = fma(-row[k], sl, yv[k]);
+  }
 }
 
-// back substitution L^T s = yv
+// back substitution L^T s = yv for rows NC-2 .. 0 (row NC-1 was done by chol_row)
 template <int NC>
 __device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&invd)[NC], const double (&yv)[NC], double (&s)[NC]) {
 #pragma unroll
-  for (int i = NC - 1; i >= 0; --i) {
+  for (int i = NC - 2; i >= 0; --i) {
     double acc = yv[i];
 #pragma unroll
-    for (int k = 0; k < NC; ++k)
+    for (int k = 0; k < NC - 1; ++k)
       if (k > i) acc = fma(-L.at(k, i), s[k], acc);
     s[i] = acc * invd[i];
   }
@@ -122,22 +133,25 @@ __device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&inv
 #endif
 
 template <int NC>
-constexpr int stabn_smem_doubles() { return NC * (NC - 1) / 2 + 2 * NC; }   // per thread: L, beta, pending step
+constexpr int newton_lrows() { return (NC - 1) * (NC - 2) / 2; }            // rows 1 .. NC-2 of the strict lower triangle
 template <int NC>
-constexpr int splitn_smem_doubles() { return NC * (NC - 1) / 2 + 6 * NC; }  // per thread: L, n^V, pending step, g, D, S(x), S(y)
+constexpr int stabn_smem_doubles() { return newton_lrows<NC>() + 3 * NC; }   // per thread: L, beta, pending step, residual r
+template <int NC>
+constexpr int splitn_smem_doubles() { return newton_lrows<NC>() + 6 * NC; }  // per thread: L, n^V, pending step, g, D, S(x), S(y)
 
 // ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(NEWTON_THREADS, PTF_STABN_MINB)
 k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o, const __grid_constant__ Io io,
                const __grid_constant__ Work w) {
-  constexpr int NL = NC * (NC - 1) / 2;
+  constexpr int NL = newton_lrows<NC>();
   constexpr unsigned FULL = 0xffffffffu;
   extern __shared__ double ptf_smem[];
   double* const sm = ptf_smem + threadIdx.x;
   const LRows<NC> L{sm};
   double* const sb = sm + NL * NEWTON_THREADS;   // accepted point beta = 2 sqrt(W) (B.1a)
   double* const sp = sb + NC * NEWTON_THREADS;   // pending / best-so-far step
+  double* const sr = sp + NC * NEWTON_THREADS;   // residual r_i = ln W_i + lnphi_i(w) - d_i at the evaluated point
   const int64_t N = io.N;
   const int total = w.qcount[Q_STAB_NEWTON];
   int* ticket = &w.qcount[Q_TICKET_STAB];
@@ -189,14 +203,14 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
     if (!__any_sync(FULL, busy)) break;
 #endif
 
-    double r[NC], Sv[NC];
+    double Sv[NC];
     double sumW = 0.0;
     Eos e;
     e.Z = Zw;
     bool finish = false, fin_conv = false, fin_exact = false, fin_cap = false;
     if (busy) {
       // ---- evaluate tm and its gradient: at the trial point beta + s, or at beta while an eta search is pending ----
-      double W[NC], lp[NC];
+      double W[NC], lp[NC], r[NC];
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
         const double b = sb[i * NEWTON_THREADS], s = sp[i * NEWTON_THREADS];
@@ -219,6 +233,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - __ldg(&w.d[(int64_t)i * N + n]) : 0.0;
         rmax = fmax(rmax, fabs(r[i]));
         tm_new = fma(W[i], r[i] - 1.0, tm_new);
+        sr[i * NEWTON_THREADS] = r[i];
       }
       if (!searching) {
         // ---- accept / reject the pending step (B.3) ----
@@ -268,56 +283,56 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
     }  // busy
     __syncwarp();
     if (busy && searching) {
-      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.1b): rows of H + eta I generated on the fly ----
+      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.1b) ----
+      // B.2b: H_ij = sqrt(w_i w_j) M_ij + delta_ij (1 + r_i / 2) = h_i h_j Mt_ij with h_i = sqrt(w_i) and
+      // Mt = M + diag((1 + r_i / 2 + eta) / w_i): the congruent matrix Mt is factored instead (same inertia), so the rows
+      // need only S_j, sqrt(A_j) and constants; H s = -g becomes Mt u = -g / h = -r sqrt(sum W), s_i = u_i / h_i.
+      // A component with z_i = 0 gets the diagonal 1e300, which decouples it (its step is masked to zero).
       const MC3 mc = mc3(e);
       const double isq = rsqrt_fast(sumW);
       const double sqW = sumW * isq;
       const double c01p = mc.c01 * q.pt, c10p = mc.c10 * q.pt, c11p = mc.c11 * q.pt * q.pt, c12p = mc.c12 * q.pt, c21p = mc.c21 * q.pt;
-      double h[NC], hS[NC], hsa[NC];
+      double sa[NC];
 #pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        h[i] = 0.5 * sb[i * NEWTON_THREADS] * isq;      // sqrt(w_i); B.2b: H_ij = sqrt(w_i w_j) M_ij + delta_ij (1 + r_i / 2)
-        hS[i] = h[i] * Sv[i];
-        hsa[i] = h[i] * sa_of<NC>(S, q, i);
-      }
+      for (int i = 0; i < NC; ++i) sa[i] = sa_of<NC>(S, q, i);
       double invd[NC], yv[NC], st[NC];
       bool good = true;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
-        // G = C^T-contracted basis vector of row i: H_ij = G0 h_j + G1 (h_j wb_j) + G2 hS_j - q2 hsa_i omk_ij hsa_j
-        const double hb = h[i] * S.wb[i];
-        const double G0 = fma(hS[i], mc.c20, fma(hb, c10p, h[i] * mc.c00));
-        const double G1 = fma(hS[i], c21p, fma(hb, c11p, h[i] * c01p));
-        const double G2 = fma(hS[i], mc.c22, fma(hb, c12p, h[i] * mc.c02));
-        const double qs = mc.q2 * hsa[i];
+        // row i of M: M_ij = G0 + G1 wb_j + G2 S_j - q2 sa_i omk_ij sa_j with G = C F_i, F_i = (1, wb_i, S_i)
+        const double G0 = fma(Sv[i], mc.c20, fma(S.wb[i], c10p, mc.c00));
+        const double G1 = fma(Sv[i], c21p, fma(S.wb[i], c11p, c01p));
+        const double G2 = fma(Sv[i], mc.c22, fma(S.wb[i], c12p, mc.c02));
+        const double qs = mc.q2 * sa[i];
         double row[NC];
 #pragma unroll
         for (int j = 0; j < NC; ++j) {
-          if (j <= i) {
-            double a = fma(G2, hS[j], fma(G1, h[j] * S.wb[j], G0 * h[j]));
-            a = fma(-(KIJ0 ? qs : qs * S.omk[i * NC + j]), hsa[j], a);
-            row[j] = a;
-          }
+          if (j <= i) row[j] = fma(-(KIJ0 ? qs : qs * S.omk[i * NC + j]), sa[j], fma(G2, Sv[j], fma(G1, S.wb[j], G0)));
         }
-        row[i] += 1.0 + 0.5 * r[i] + es.eta;
-        chol_row<NC>(i, row, L, invd, yv, -h[i] * r[i] * sqW, good);   // rhs = -g_i = -beta_i r_i / 2 (B.2a)
+        const double ri = sr[i * NEWTON_THREADS];
+        const double ih = 2.0 * sqW * rcp_fast(sb[i * NEWTON_THREADS]);          // 1 / h_i (beta_i = 2 h_i sqrt(sum W))
+        const double iw = ((act >> i) & 1u) ? ih * ih : 1.0e300;
+        row[i] = fma(1.0 + 0.5 * ri + es.eta, iw, row[i]);
+        chol_row<NC>(i, row, L, invd, yv, st, -ri * sqW, good);
       }
       chol_back<NC>(L, invd, yv, st);
-      double sn = 0.0;
+      double sn = 0.0, sg = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
+        const double b = sb[i * NEWTON_THREADS];
+        sg = fma(st[i], sr[i * NEWTON_THREADS], sg);                             // s.g = sqrt(sum W) u.r
+        st[i] = ((act >> i) & 1u) ? st[i] * (2.0 * sqW * rcp_fast(b)) : 0.0;     // s_i = u_i / h_i
         sn = fma(st[i], st[i], sn);
-        if (((act >> i) & 1u) && !(sb[i * NEWTON_THREADS] + st[i] > 0.0)) good = false;
+        if (((act >> i) & 1u) && !(b + st[i] > 0.0)) good = false;
       }
       sn = sqrt_fast(sn);
       good = good && (sn <= Delta);
       const double eta_used = es.eta;
       if (es.feed(good, sn, Delta, kept_sn)) {
-        double sg = 0.0;   // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
 #pragma unroll
-        for (int i = 0; i < NC; ++i) { sp[i * NEWTON_THREADS] = st[i]; sg = fma(st[i], h[i] * r[i], sg); }
+        for (int i = 0; i < NC; ++i) sp[i * NEWTON_THREADS] = st[i];
         snorm = sn;
-        pred = 0.5 * sg * sqW - 0.5 * eta_used * sn * sn;
+        pred = 0.5 * sg * sqW - 0.5 * eta_used * sn * sn;   // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
         exact = (eta_used == 0.0);
       }
       if (es.phase == 4) { finish = true; fin_cap = true; searching = false; }
@@ -326,7 +341,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         double smax = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * NEWTON_THREADS]));
-        if (exact && smax < o.tol_newton_step) {
+        if (exact && smax < o.tol_newton_step_stab) {
           // quadratic-convergence finish: apply the full Newton step and stop
           finish = true;
           fin_conv = true;
@@ -366,7 +381,7 @@ template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(NEWTON_THREADS, PTF_SPLITN_MINB)
 k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o, const __grid_constant__ Io io,
                 const __grid_constant__ Work w) {
-  constexpr int NL = NC * (NC - 1) / 2;
+  constexpr int NL = newton_lrows<NC>();
   constexpr int T = NEWTON_THREADS;
   constexpr unsigned FULL = 0xffffffffu;
   extern __shared__ double ptf_smem[];
@@ -550,7 +565,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           }
         }
         row[i] = fma(sD[i * T], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
-        chol_row<NC>(i, row, L, invd, yv, -sg[i * T], pd);
+        chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd);
       }
       chol_back<NC>(L, invd, yv, st);
       bool good = pd;
@@ -579,9 +594,14 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
       else if (es.phase == 3) {
         searching = false;
-        double smax = 0.0;
+        double smax = 0.0;   // largest step relative to the smaller of the two mole numbers n_i, z_i - n_i
 #pragma unroll
-        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * T]));
+        for (int i = 0; i < NC; ++i) {
+          if ((act >> i) & 1u) {
+            const double ni = sn[i * T];
+            smax = fmax(smax, fabs(sp[i * T]) * rcp_fast(fmin(ni, __ldg(&w.zn[(int64_t)i * N + n]) - ni)));
+          }
+        }
         if (exact && smax < o.tol_newton_step) {
           finish = true;
           fin_conv = true;

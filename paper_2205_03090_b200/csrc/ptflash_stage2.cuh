@@ -2,9 +2,9 @@
 //
 //   k2_probe / k2_stab_ss / k2_split_ss   one work item per thread, iterate in registers, warm-started cubic and
 //                                         Rachford-Rice, everything inlined (no per-mixture struct in local memory)
-//   k2_stab_newton / k2_split_newton      persistent warps with LANE REFILL: every lane owns one work item; one loop
-//                                         trip = one trust-region iteration (one lnphi evaluation per phase + one
-//                                         packed in-register Cholesky); a lane whose item finishes stores it and
+//   k3_stab_newton / k3_split_newton      (ptflash_newton.cuh) persistent warps with LANE REFILL: every lane owns one
+//                                         work item; one loop trip = one trust-region iteration (one lnphi evaluation
+//                                         per phase + one row-wise Cholesky); a lane whose item finishes stores it and
 //                                         pulls the next item from a global ticket (warp ballot + popc prefix), so
 //                                         early finishers do not stall their warp (north_star subsystem 4; the
 //                                         paper's per-iteration mask-and-compact, eq. 10).
@@ -221,12 +221,6 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
   }
 }
 
-#ifndef PTF_TRI_SMEM
-#define PTF_TRI_SMEM 1   // packed Newton matrices in shared memory (440 B per thread at nc = 10) instead of registers
-#endif
-#ifndef PTF_NEWTON_MINB
-#define PTF_NEWTON_MINB 3
-#endif
 // ---- lane refill ----------------------------------------------------------------------------------
 // Lanes with want == true take consecutive tickets; returns the ticket (>= total means the queue is exhausted).
 __device__ __forceinline__ int64_t take_ticket(bool want, int* __restrict__ ticket) {
@@ -266,226 +260,6 @@ struct EtaSearch {
     return keep;
   }
 };
-
-// ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
-template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                      const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  constexpr int NT = NC * (NC + 1) / 2;
-  constexpr unsigned FULL = 0xffffffffu;
-  const int64_t N = io.N;
-  const int total = w.qcount[Q_STAB_NEWTON];
-  int* ticket = &w.qcount[Q_TICKET_STAB];
-  // ---- lane state ----
-  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
-  int n = 0, sidx = 0, iters = 0, tr_it = 0;
-  unsigned act = 0u;
-  double spt = 0.0, sT = 0.0, pt = 0.0;   // sqrt(P)/T, sqrt(T), P/T: sqrt(A_i), B_i are rebuilt from constants
-  double beta[NC], s[NC];                 // accepted point (beta = 2 sqrt(W), B.1a) and pending / best-so-far step
-  double tm = 0.0, rmax_acc = 0.0, pred = 0.0, Delta = 1.0, Delta_cap = 8.0, snorm = 0.0, Zw = 0.0, kept_sn = 0.0;
-  EtaSearch es;
-  es.start(1.0e-3);
-#pragma unroll
-  for (int i = 0; i < NC; ++i) { beta[i] = 0.0; s[i] = 0.0; }
-
-#pragma unroll 1
-  while (true) {
-    // ---- refill idle lanes from the ticket ----
-    if (__any_sync(FULL, !busy && !exhausted)) {
-      const int64_t tk = take_ticket(!busy && !exhausted, ticket);
-      if (tk >= 0) {
-        if (tk < total) {
-          const int item = w.q_stab_newton[tk];
-          n = item >> 1;
-          sidx = item & 1;
-          const double P = io.P[n], T = io.T[n];
-          { const double iT = rcp_fast(T); sT = sqrt_fast(T); spt = sqrt_fast(P) * iT; pt = P * iT; }
-          act = (unsigned)w.actmask[n];
-#pragma unroll
-          for (int i = 0; i < NC; ++i) {
-            beta[i] = w.lnW[((int64_t)sidx * NC + i) * N + n];   // k2_stab_ss left beta = 2 sqrt(W) here
-            s[i] = 0.0;
-          }
-          iters = w.tflags[(int64_t)sidx * N + n] >> TF_ITER_SHIFT;
-          tr_it = 0;
-          first = true;
-          reeval = false;
-          searching = false;
-          Zw = w.Zw[(int64_t)sidx * N + n];
-          busy = true;
-        } else {
-          exhausted = true;
-        }
-      }
-    }
-    if (!__any_sync(FULL, busy)) break;
-
-    // The trip below is written WITHOUT early `continue`s and with explicit __syncwarp() joins: the factorisation
-    // block must be entered once per trip by all searching lanes together (a divergent entry makes the warp run
-    // the ~1500-instruction block twice with half the lanes each).
-    double sa[NC], bi[NC], W[NC], lp[NC], Sv[NC], r[NC];
-    double sumW = 0.0;
-    Eos e;
-    e.Z = Zw;
-    bool finish = false, fin_conv = false, fin_exact = false, fin_cap = false;
-    if (busy) {
-    // ---- evaluate tm and its gradient: at the trial point beta + s, or at beta while an eta search is pending ----
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));
-      bi[i] = pt * S.wb[i];
-      const double h = 0.5 * (searching ? beta[i] : beta[i] + s[i]);
-      W[i] = h * h;                                              // B.1d
-      r[i] = ((act >> i) & 1u) ? 2.0 * log_fast(h) : 0.0;        // ln W_i
-      sumW += W[i];
-    }
-    {
-      const double inv = rcp_fast(sumW);
-      double wn[NC];
-#pragma unroll
-      for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
-      lnphi_fast<NC, KIJ0>(S, sa, bi, wn, lp, Sv, e);
-    }
-    Zw = e.Z;
-    double rmax = 0.0, tm_new = 1.0;
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - w.d[(int64_t)i * N + n] : 0.0;
-      rmax = fmax(rmax, fabs(r[i]));
-      tm_new = fma(W[i], r[i] - 1.0, tm_new);
-    }
-    if (!searching) {
-      // ---- accept / reject the pending step (B.3) ----
-      bool accepted = true;
-      if (first) {
-        double bn = 0.0;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) bn = fma(beta[i], beta[i], bn);
-        Delta = fmax(1.0, 0.5 * sqrt_fast(bn));
-        Delta_cap = 8.0 * Delta;
-      } else if (!reeval) {
-        const double act_red = tm_new - tm;
-        accepted = (act_red < 0.0) || (rmax < rmax_acc);
-        if (accepted) {
-          if (fabs(pred) > 1.0e-13) {
-            const double ratio = fabs(act_red * rcp_fast(pred));
-            if (ratio <= 0.25) Delta *= 0.5;
-            else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
-          }
-        } else {
-          Delta = 0.5 * fmin(Delta, snorm);
-          reeval = true;   // next trip re-evaluates at the accepted point (s = 0) and continues from there
-        }
-      }
-      if (!accepted) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) s[i] = 0.0;
-      } else {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) { beta[i] += s[i]; s[i] = 0.0; }
-        tm = tm_new;
-        rmax_acc = rmax;
-        first = false;
-        reeval = false;
-        // ---- convergence / cap, else start the eta search of a new trust-region iteration ----
-        if (rmax < o.tol_newton_g) { finish = true; fin_conv = true; }
-        else if (tr_it >= o.stab_tr_iters) { finish = true; fin_cap = true; }
-        else {
-          tr_it++;
-          iters++;
-          es.start(1.0e-3);
-          kept_sn = 0.0;
-          searching = true;
-        }
-      }
-    }
-    }  // busy
-    __syncwarp();
-    if (busy && searching) {
-      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.1b): build H + eta I, factor, solve ----
-      const MCoef mc = mcoef(e);
-      const double isq = rsqrt_fast(sumW);
-      double g[NC], st[NC];
-#pragma unroll
-      for (int i = 0; i < NC; ++i) g[i] = 0.5 * beta[i] * r[i];   // B.2a
-#if PTF_TRI_SMEM
-      extern __shared__ double ptf_smem[];
-      TriSmem<128> Lm{ptf_smem + threadIdx.x};
-#else
-      double Lm[NT];
-#endif
-#pragma unroll
-      for (int j = 0; j < NC; ++j) {
-        const double ej = bi[j] * mc.invB;
-        double pj, cj, Dqj;
-        mcol(mc, ej - 1.0, Sv[j] - mc.A, pj, cj, Dqj);
-        const double hj = 0.5 * beta[j] * isq;
-#pragma unroll
-        for (int i = j; i < NC; ++i) {
-          const double ei = bi[i] * mc.invB;
-          const double ui = fma(2.0, Sv[i], -mc.A * ei);
-          const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
-          const double Mij = fma(ei, pj, cj) - fma(Dqj, ui, mc.q2 * (Aij - Sv[i]));
-          const double hi_ = 0.5 * beta[i] * isq;
-          double hij = hi_ * hj * Mij;                                   // B.2b
-          if (i == j) hij += 1.0 + 0.5 * r[i] + es.eta;
-          Lm[tri(i, j)] = hij;
-        }
-      }
-      bool good = chol_packed<NC>(Lm, g, st);
-      double sn = 0.0;
-#pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        sn = fma(st[i], st[i], sn);
-        if (((act >> i) & 1u) && !(beta[i] + st[i] > 0.0)) good = false;
-      }
-      sn = sqrt_fast(sn);
-      good = good && (sn <= Delta);
-      const double eta_used = es.eta;
-      if (es.feed(good, sn, Delta, kept_sn)) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) s[i] = st[i];
-        snorm = sn;
-        double sg = 0.0;   // predicted reduction s.g + s.H.s/2 with H s = -g - eta s
-#pragma unroll
-        for (int i = 0; i < NC; ++i) sg = fma(s[i], g[i], sg);
-        pred = 0.5 * sg - 0.5 * eta_used * sn * sn;
-        exact = (eta_used == 0.0);
-      }
-      if (es.phase == 4) { finish = true; fin_cap = true; searching = false; }
-      else if (es.phase == 3) {
-        searching = false;
-        double smax = 0.0;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(s[i]));
-        if (exact && smax < o.tol_newton_step) {
-          // quadratic-convergence finish: apply the full Newton step and stop
-          finish = true;
-          fin_conv = true;
-          fin_exact = true;
-          sumW = 0.0;
-#pragma unroll
-          for (int i = 0; i < NC; ++i) {
-            beta[i] += s[i];
-            const double h = 0.5 * beta[i];
-            sumW = fma(h, h, sumW);
-          }
-        }
-      }
-    }
-    __syncwarp();
-    if (finish) {
-      // beta is stored; k_stab_decide turns it into ln W = 2 ln(beta/2) with all lanes active (TF_BETA)
-#pragma unroll
-      for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = beta[i];
-      w.tm[(int64_t)sidx * N + n] = tm;
-      w.sumW[(int64_t)sidx * N + n] = sumW;
-      w.tflags[(int64_t)sidx * N + n] = (fin_conv ? TF_CONVERGED : 0) | (fin_exact ? TF_EXACT : 0) |
-                                        (fin_cap ? TF_CAPPED : 0) | TF_BETA | (iters << TF_ITER_SHIFT);
-      busy = false;
-    }
-  }
-}
 
 // ---- K5: phase-split SS ---------------------------------------------------------------------------
 template <int NC>
@@ -579,238 +353,9 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
   }
 }
 
-// ---- K6: phase-split trust-region Newton on G (B.4-B.5), persistent warps with lane refill --------
-template <int NC, bool KIJ0>
-__global__ void __launch_bounds__(128, PTF_NEWTON_MINB) k2_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                       const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  constexpr int NT = NC * (NC + 1) / 2;
-  constexpr unsigned FULL = 0xffffffffu;
-  const int64_t N = io.N;
-  const int total = w.qcount[Q_SPLIT_NEWTON];
-  int* ticket = &w.qcount[Q_TICKET_SPLIT];
-  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
-  int n = 0, tr_it = 0, status = 0;
-  unsigned act = 0u;
-  double spt = 0.0, sT = 0.0, pt = 0.0;
-  double nV[NC], s[NC];   // accepted vapour mole numbers (B.4) and pending / best-so-far step
-  double G = 0.0, gmax_acc = 0.0, pred = 0.0, Delta = 0.25, snorm = 0.0, Zx = 0.0, Zy = 0.0, kept_sn = 0.0;
-  EtaSearch es;
-  es.start(1.0);
-#pragma unroll
-  for (int i = 0; i < NC; ++i) { nV[i] = 0.0; s[i] = 0.0; }
-
-#pragma unroll 1
-  while (true) {
-    if (__any_sync(FULL, !busy && !exhausted)) {
-      const int64_t tk = take_ticket(!busy && !exhausted, ticket);
-      if (tk >= 0) {
-        if (tk < total) {
-          n = w.q_split_newton[tk];
-          const double P = io.P[n], T = io.T[n];
-          { const double iT = rcp_fast(T); sT = sqrt_fast(T); spt = sqrt_fast(P) * iT; pt = P * iT; }
-          act = (unsigned)w.actmask[n];
-          // k2_split_ss left n^V = theta y of its last Rachford-Rice here
-#pragma unroll
-          for (int i = 0; i < NC; ++i) { nV[i] = w.lnK[(int64_t)i * N + n]; s[i] = 0.0; }
-          tr_it = 0;
-          status = 0;
-          first = true;
-          reeval = false;
-          searching = false;
-          Delta = 0.25;
-          Zx = w.Zxy[n];
-          Zy = w.Zxy[N + n];
-          busy = true;
-        } else {
-          exhausted = true;
-        }
-      }
-    }
-    if (!__any_sync(FULL, busy)) break;
-
-    double sa[NC], bi[NC], z[NC], x[NC], y[NC], lp[NC], Sx[NC], Sy[NC], gt[NC];
-    double theta = 0.0;
-    Eos ex, ey;
-    bool finish = false, fin_conv = false;
-    if (busy) {
-    // ---- evaluate G (eq. 8) and its gradient (B.5a): at n^V + s, or at n^V while an eta search is pending ----
-    load_zn<NC>(io, w, n, z);
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      sa[i] = spt * fabs(fma(-S.v[i], sT, S.u[i]));
-      bi[i] = pt * S.wb[i];
-      const double v = searching ? nV[i] : nV[i] + s[i];
-      y[i] = v;
-      theta += v;
-    }
-    {
-      const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
-#pragma unroll
-      for (int i = 0; i < NC; ++i) { const double v = y[i]; y[i] = v * it; x[i] = (z[i] - v) * il; }
-    }
-    ex.Z = Zx;
-    lnphi_call<NC, KIJ0>(S, sa, bi, x, lp, Sx, ex);
-    Zx = ex.Z;
-    double G_new = 0.0, gmax = 0.0;
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      double fx = 0.0;
-      if ((act >> i) & 1u) { fx = log_fast(x[i]) + lp[i]; G_new = fma(x[i] * (1.0 - theta), fx, G_new); }
-      gt[i] = -fx;
-    }
-    ey.Z = Zy;
-    lnphi_call<NC, KIJ0>(S, sa, bi, y, lp, Sy, ey);
-    Zy = ey.Z;
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      if ((act >> i) & 1u) { const double fy = log_fast(y[i]) + lp[i]; G_new = fma(y[i] * theta, fy, G_new); gt[i] += fy; }
-      gmax = fmax(gmax, fabs(gt[i]));
-    }
-    if (!searching) {
-      // ---- accept / reject ----
-      bool accepted = true;
-      if (!first && !reeval) {
-        const double act_red = G_new - G;
-        accepted = (act_red < 0.0) || (gmax < gmax_acc);
-        if (accepted) {
-          if (fabs(pred) > 1.0e-13) {
-            const double ratio = fabs(act_red * rcp_fast(pred));
-            if (ratio <= 0.25) Delta *= 0.5;
-            else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
-          }
-        } else {
-          Delta = 0.5 * fmin(Delta, snorm);
-          reeval = true;
-        }
-      }
-      if (!accepted) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) s[i] = 0.0;
-      } else {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) { nV[i] += s[i]; s[i] = 0.0; }
-        G = G_new;
-        gmax_acc = gmax;
-        first = false;
-        reeval = false;
-        if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
-        else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
-        else {
-          tr_it++;
-          es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
-          kept_sn = 0.0;
-          searching = true;
-        }
-      }
-    }
-    }  // busy
-    __syncwarp();
-    if (busy && searching) {
-      // ---- ONE attempt of the restricted-step sub-problem at es.eta (B.4a) ----
-      const MCoef mx = mcoef(ex), my = mcoef(ey);
-      const double tt = theta * (1.0 - theta), itt = rcp_fast(tt);
-      const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
-      double D[NC], st[NC];
-#pragma unroll
-      for (int i = 0; i < NC; ++i) D[i] = ((act >> i) & 1u) ? z[i] * rcp_fast(x[i] * y[i]) : 1.0;
-#if PTF_TRI_SMEM
-      extern __shared__ double ptf_smem[];
-      TriSmem<128> Lm{ptf_smem + threadIdx.x};
-#else
-      double Lm[NT];
-#endif
-#pragma unroll
-      for (int j = 0; j < NC; ++j) {
-        const double exj = bi[j] * mx.invB, eyj = bi[j] * my.invB;
-        double pxj, cxj, Dqxj, pyj, cyj, Dqyj;
-        mcol(mx, exj - 1.0, Sx[j] - mx.A, pxj, cxj, Dqxj);
-        mcol(my, eyj - 1.0, Sy[j] - my.A, pyj, cyj, Dqyj);
-        const bool aj = (act >> j) & 1u;
-#pragma unroll
-        for (int i = j; i < NC; ++i) {
-          const bool ai = (act >> i) & 1u;
-          const double exi = bi[i] * mx.invB, eyi = bi[i] * my.invB;
-          const double uxi = fma(2.0, Sx[i], -mx.A * exi), uyi = fma(2.0, Sy[i], -my.A * eyi);
-          const double Aij = (KIJ0 ? 1.0 : S.omk[i * NC + j]) * sa[i] * sa[j];
-          const double Mx = fma(exi, pxj, cxj) - fma(Dqxj, uxi, mx.q2 * (Aij - Sx[i]));
-          const double My = fma(eyi, pyj, cyj) - fma(Dqyj, uyi, my.q2 * (Aij - Sy[i]));
-          double hij = fma(wx, Mx, wy * My) - itt;                                  // B.5b
-          if (i == j) hij += D[i] * (itt + es.eta);                                // + eta D (B.4a)
-          if (!(ai && aj)) hij = (i == j) ? 1.0 : 0.0;
-          Lm[tri(i, j)] = hij;
-        }
-      }
-      bool good = chol_packed<NC>(Lm, gt, st);
-      double sn = 0.0, sds = 0.0;
-#pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        sn = fma(st[i], st[i], sn);
-        sds = fma(st[i] * st[i], D[i], sds);
-        if ((act >> i) & 1u) {
-          const double nv = nV[i] + st[i];
-          if (!(nv > 0.0) || !(nv < z[i])) good = false;
-        }
-      }
-      sn = sqrt_fast(sn);
-      good = good && (sn <= Delta);
-      const double eta_used = es.eta;
-      if (es.feed(good, sn, Delta, kept_sn)) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) s[i] = st[i];
-        snorm = sn;
-        double sg = 0.0;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) sg = fma(s[i], gt[i], sg);
-        pred = 0.5 * sg - 0.5 * eta_used * sds;
-        exact = (eta_used == 0.0);
-      }
-      if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
-      else if (es.phase == 3) {
-        searching = false;
-        double smax = 0.0;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(s[i]));
-        if (exact && smax < o.tol_newton_step) {
-          finish = true;
-          fin_conv = true;
-          theta = 0.0;
-#pragma unroll
-          for (int i = 0; i < NC; ++i) { nV[i] += s[i]; theta += nV[i]; }
-          const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
-#pragma unroll
-          for (int i = 0; i < NC; ++i) { y[i] = nV[i] * it; x[i] = (z[i] - nV[i]) * il; }
-        }
-      }
-    }
-    __syncwarp();
-    if (finish) {
-      double lnK[NC];
-      // trivial collapse x = y (max |ln K| < 1e-9): |y/x - 1| is the same test to first order and needs no logarithm
-      double mkn = 0.0;
-#pragma unroll
-      for (int i = 0; i < NC; ++i)
-        if ((act >> i) & 1u) mkn = fmax(mkn, fabs(y[i] - x[i]) * rcp_fast(x[i]));
-      const bool trivial = mkn < 1.0e-9;
-      if (io.lnK) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
-      } else {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
-      }
-      store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, Zx, Zy);
-      busy = false;
-    }
-  }
-}
-
 }  // namespace ptf
 #include "ptflash_newton.cuh"
 namespace ptf {
-
-#ifndef PTF_NEWTON_V3
-#define PTF_NEWTON_V3 1   // 1: matrix-free rows + shared-memory Cholesky (ptflash_newton.cuh); 0: register-resident k2_* kernels
-#endif
 
 template <int NC, bool KIJ0>
 int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work& w_in, int sms, cudaStream_t st) {
@@ -821,14 +366,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     return (unsigned)(need < cap ? (need > 0 ? need : 1) : cap);
   };
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
-  const unsigned gP = (unsigned)(sms * PTF_NEWTON_MINB);   // persistent refill kernels: a few CTAs per SM pull tickets
   Work w = w_in;
-  const size_t tri_bytes = PTF_TRI_SMEM ? (size_t)(NC * (NC + 1) / 2) * threads * sizeof(double) : 0;
-  if (tri_bytes > 48 * 1024) {
-    cudaFuncSetAttribute(k2_stab_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tri_bytes);
-    cudaFuncSetAttribute(k2_split_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tri_bytes);
-  }
-#if PTF_NEWTON_V3
   // persistent refill kernels: as many CTAs per SM as registers and shared memory allow (queried once per instantiation)
   const size_t stab_bytes = (size_t)stabn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
   const size_t split_bytes = (size_t)splitn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
@@ -842,7 +380,6 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     stab_cta = a > 0 ? a : 1;
     split_cta = b > 0 ? b : 1;
   }
-#endif
   // optional stage profiling: one event before the first kernel and one after every stage kernel
   cudaEvent_t* ev = (cudaEvent_t*)o.prof_events;
   int nev = 0;
@@ -859,21 +396,13 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     mark();
     k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
     mark();
-#if PTF_NEWTON_V3
-    k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), threads, stab_bytes, st>>>(s, o, io, w);
-#else
-    k2_stab_newton<NC, KIJ0><<<gP, threads, tri_bytes, st>>>(s, o, io, w);
-#endif
+    k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), NEWTON_THREADS, stab_bytes, st>>>(s, o, io, w);
     mark();
     k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
     k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
-#if PTF_NEWTON_V3
-    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), threads, split_bytes, st>>>(s, o, io, w);
-#else
-    k2_split_newton<NC, KIJ0><<<gP, threads, tri_bytes, st>>>(s, o, io, w);
-#endif
+    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w);
     k_finalize_counters<<<1, 32, 0, st>>>(w);
     mark();
     launches += 7;
