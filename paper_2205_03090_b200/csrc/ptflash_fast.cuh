@@ -11,6 +11,7 @@
 #pragma once
 #include "ptflash_device.cuh"
 #include "ptflash_math.cuh"
+#include <cstdio>
 
 namespace ptf {
 
@@ -262,6 +263,9 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
   const double width = fmin(ar - al, 1.0);
 
   const double scale = 1.0e-8 * width;
+#ifdef PTF_DEBUG_COUNT
+  int dbg_it = 0, dbg_bis = 0;
+#endif
 #pragma unroll 1
   for (int it = 0; it < 100; ++it) {
     if (!(hi > lo)) break;
@@ -278,13 +282,29 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     const double h = u * w * f;
     const double dh = (w - u) * f + u * w * df;
     double tn = th - h * rcp_fast(dh);
+#ifdef PTF_DEBUG_COUNT
+    dbg_it = it + 1;
+#endif
+    // Newton step below the tolerance: apply it and stop (quadratic convergence leaves an error ~ step^2).  th is an end
+    // of the sign bracket here, so a converged tn can land ON or an ulp beyond that end; it is clamped, not bisected
+    // (bisecting from a converged iterate cost ~25 extra iterations in 1 % of the calls, i.e. in every fourth warp).
+    if (fabs(tn - th) <= scale) { th = fmin(fmax(tn, lo), hi); break; }
     const bool inside = (tn > lo && tn < hi);
     if (!inside) tn = 0.5 * (lo + hi);
-    const double step = fabs(tn - th);
+#ifdef PTF_DEBUG_COUNT
+    if (!inside) dbg_bis++;
+#endif
+    if (fabs(tn - th) <= 2.3e-16 * fabs(tn)) { th = tn; break; }
     th = tn;
-    if (inside && step <= scale) break;   // quadratic convergence: the applied step leaves an error ~ step^2
-    if (step <= 2.3e-16 * fabs(th)) break;
   }
+#ifdef PTF_DEBUG_COUNT
+  if (dbg_it >= 15 && atomicAdd(&g_dbg[63], 1ull) < 12) {
+    printf("RR slow: warm=%d its=%d bis=%d f0=%.3e f1=%.3e al=%.6e ar=%.6e th=%.17g lo=%.17g hi=%.17g theta_in=%.6e\n", (int)warm, dbg_it, dbg_bis, f0, f1, al, ar, th, lo, hi, theta);
+    for (int i = 0; i < NC; ++i) printf("   i=%d z=%.6e K=%.6e\n", i, z[i], K[i]);
+  }
+  PTF_DBG((warm ? 32 : 16) + (dbg_it < 15 ? dbg_it : 15), 1);
+  PTF_DBG(warm ? 49 : 48, dbg_bis);
+#endif
   theta = th;
   double sx = 0.0, sy = 0.0;
 #pragma unroll

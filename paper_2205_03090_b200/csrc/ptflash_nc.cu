@@ -43,8 +43,8 @@ int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& i
 #if PTF_NC == 10
 extern "C" void ptflash_debug_counters(unsigned long long* out, int reset) {
   cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, ptf::g_dbg, sizeof(unsigned long long) * 16);
-  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(ptf::g_dbg, z, sizeof(z)); }
+  cudaMemcpyFromSymbol(out, ptf::g_dbg, sizeof(unsigned long long) * 64);
+  if (reset) { unsigned long long z[64] = {0}; cudaMemcpyToSymbol(ptf::g_dbg, z, sizeof(z)); }
 }
 #endif
 #endif

@@ -24,12 +24,6 @@ constexpr int NEWTON_THREADS = 128;
 #ifndef PTF_NEWTON_CTA_SYNC
 #define PTF_NEWTON_CTA_SYNC 1
 #endif
-#ifdef PTF_DEBUG_COUNT
-__device__ unsigned long long g_dbg[16];
-#define PTF_DBG(k, v) atomicAdd(&g_dbg[k], (unsigned long long)(v))
-#else
-#define PTF_DBG(k, v)
-#endif
 
 // Coefficients of M_ij = sum_ab F_ia C[a][b] F_jb - q2 A_ij with F_i = (1, B_i, S_i) (B_i, not B_i/B).
 // Derivation: DESIGN.md section 2 (M_ij = e_i p_j + c_j - Dq_j u_i + 2q(S_i - A_ij) with p, c, Dq affine in
