@@ -33,7 +33,11 @@ UNIT = "flashes/s"
 WORKLOAD = "config3: 10-component CO2-rich SRK flash (8 n-alkanes + CO2 + N2, kij per BASELINE.json), z=0.6*Dir(1)+0.4*e_CO2, T~U[220,500]K, P~U[5,300]bar, seed 2205030903"
 # Algorithmic FP64 work per flash on this workload: thread-level predicated-on DADD + DMUL + 2*DFMA of
 # all stage kernels, counted by ncu on the committed build (profiles/), per mixture.
-FLOPS_PER_FLASH = float(os.environ.get("PTFLASH_FLOPS_PER_FLASH", "4.56e4"))
+# Per stage kernel, in flops per mixture of the batch (profiles/r01c_kernels.md):
+STAGES = ("k_init", "k2_probe", "k2_stab_ss", "k3_stab_newton", "k_stab_decide", "k2_split_ss", "k3_split_newton")
+STAGE_FLOPS_PER_FLASH = {"k_init": 1.92e3, "k2_probe": 4.36e3, "k2_stab_ss": 13.55e3, "k3_stab_newton": 11.82e3,
+                         "k_stab_decide": 0.69e3, "k2_split_ss": 5.48e3, "k3_split_newton": 1.89e3}
+FLOPS_PER_FLASH = float(os.environ.get("PTFLASH_FLOPS_PER_FLASH", sum(STAGE_FLOPS_PER_FLASH.values())))
 BYTES_PER_FLASH_NC10 = 272.0   # 8(nc+2) in + 8(2nc+1)+8 out, SURVEY.md section 8(d)
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # SMs x DFMA lanes/clk x 2 flop x max SM clock
 
@@ -183,6 +187,18 @@ def main():
         torch.cuda.synchronize()
         sampler.terminate()
     stats = f.stats()
+    # per-stage times of a few extra (untimed) calls: CUDA events recorded by the library on the call's stream between
+    # the stage kernels (PTFLASH_OPT_STAGE_PROFILE) -- the live launch durations behind the dominant-kernel roofline
+    stage_ms = None
+    if args.engine == 1 and rank == 0:
+        f.set_option("stage_profile", 1)
+        acc = []
+        for _ in range(5):
+            step()
+            acc.append(f.stage_ms()[:len(STAGES)])
+        f.set_option("stage_profile", 0)
+        if acc and len(acc[0]) == len(STAGES):
+            stage_ms = [float(np.mean([a[i] for a in acc])) for i in range(len(STAGES))]
     t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -240,6 +256,15 @@ def main():
         "hbm_peak_gbs": hbm, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback",
         "kernel": "all stage kernels of one ptflash_flash call (k_init .. k_split_newton)",
     }
+    if stage_ms:
+        # the same figure per stage kernel; "dominant" = the kernel with the largest share of the step
+        per = {}
+        for name, ms in zip(STAGES, stage_ms):
+            a = STAGE_FLOPS_PER_FLASH[name] * N / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+            per[name] = {"ms": ms, "share": ms / sum(stage_ms), "achieved": a, "frac": a / peak}
+        dom = max(per, key=lambda k: per[k]["ms"])
+        roofline["stages"] = per
+        roofline["dominant"] = dict(kernel=dom, **per[dom])
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
