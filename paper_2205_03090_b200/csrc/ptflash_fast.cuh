@@ -18,6 +18,18 @@ namespace ptf {
 // packed lower-triangle index, i >= j
 __host__ __device__ constexpr int tri(int i, int j) { return i * (i + 1) / 2 + j; }
 
+// Newton polish of the two deflated roots (A.5), interleaved: a step is taken only if it lowers |f| (near a double root
+// the deflated value is already the best available), twice.
+__device__ __forceinline__ void cub_polish2(double& za, double& zb, double r1, double r0) {
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const double fa = cub_f(za, r1, r0), fb = cub_f(zb, r1, r0);
+    const double na = za - fa * rcp_nr1(cub_df(za, r1)), nb = zb - fb * rcp_nr1(cub_df(zb, r1));
+    za = (fabs(cub_f(na, r1, r0)) < fabs(fa)) ? na : za;   // a NaN step (df == 0) fails the test and is dropped
+    zb = (fabs(cub_f(nb, r1, r0)) < fabs(fb)) ? nb : zb;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // cubic with warm start.  Zg: previous root of this phase (<= 0: none).
 // ------------------------------------------------------------------------------------------------
@@ -63,10 +75,9 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
     const double sq = sqrt_fast(disc);
     const double t = (p >= 0.0) ? -0.5 * (p + sq) : 0.5 * (sq - p);
     double ra = t, rb = (t != 0.0) ? div_fast(q, t) : -p - t;
-    ra = cub_polish(ra, r1, r0);
-    rb = cub_polish(rb, r1, r0);
-    if (ra > B) { zmin = fmin(zmin, ra); zmax = fmax(zmax, ra); }
-    if (rb > B) { zmin = fmin(zmin, rb); zmax = fmax(zmax, rb); }
+    cub_polish2(ra, rb, r1, r0);
+    if (ra > B) { zmin = dmin(zmin, ra); zmax = dmax(zmax, ra); }
+    if (rb > B) { zmin = dmin(zmin, rb); zmax = dmax(zmax, rb); }
   }
   double lz = log_fast(zmin - B), ll = log1p_fast(B * rcp_fast(zmin));
   if (zmax != zmin) {
@@ -244,7 +255,7 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
   for (int i = 0; i < NC; ++i) {
     const bool a = z[i] > 0.0;
     km1[i] = a ? K[i] - 1.0 : 0.0;
-    if (a) { Kmax = fmax(Kmax, K[i]); Kmin = fmin(Kmin, K[i]); }
+    if (a) { Kmax = dmax(Kmax, K[i]); Kmin = dmin(Kmin, K[i]); }
     f0 = fma(z[i], km1[i], f0);
     f1 = fma(z[i] * km1[i], rcp_fast(K[i]), f1);
   }
@@ -254,13 +265,13 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
   if (f0 > 0.0) {
     if (f1 < 0.0) { lo = 0.0; hi = 1.0; th = f0 * rcp_fast(f0 - f1); }
     else if (f1 == 0.0) { lo = hi = 1.0; th = 1.0; }
-    else { lo = 1.0; th = fmin(1.0 + 0.5 * (ar - 1.0), 2.0); }
-  } else if (f0 < 0.0) { hi = 0.0; th = fmax(0.5 * al, -1.0); }
+    else { lo = 1.0; th = dmin(1.0 + 0.5 * (ar - 1.0), 2.0); }
+  } else if (f0 < 0.0) { hi = 0.0; th = dmax(0.5 * al, -1.0); }
   else { lo = hi = 0.0; th = 0.0; }
   const bool warm = (theta > lo && theta < hi);
   if (warm) th = theta;
   if (!(th > lo && th < hi)) th = 0.5 * (lo + hi);
-  const double width = fmin(ar - al, 1.0);
+  const double width = dmin(ar - al, 1.0);
 
   const double scale = 1.0e-8 * width;
 #ifdef PTF_DEBUG_COUNT
@@ -288,7 +299,7 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     // Newton step below the tolerance: apply it and stop (quadratic convergence leaves an error ~ step^2).  th is an end
     // of the sign bracket here, so a converged tn can land ON or an ulp beyond that end; it is clamped, not bisected
     // (bisecting from a converged iterate cost ~25 extra iterations in 1 % of the calls, i.e. in every fourth warp).
-    if (fabs(tn - th) <= scale) { th = fmin(fmax(tn, lo), hi); break; }
+    if (fabs(tn - th) <= scale) { th = dmin(dmax(tn, lo), hi); break; }
     const bool inside = (tn > lo && tn < hi);
     if (!inside) tn = 0.5 * (lo + hi);
 #ifdef PTF_DEBUG_COUNT
@@ -309,7 +320,7 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
   double sx = 0.0, sy = 0.0;
 #pragma unroll
   for (int i = 0; i < NC; ++i) {
-    const double xi = (z[i] > 0.0) ? z[i] * rcp_fast(fma(km1[i], th, 1.0)) : 0.0;
+    const double xi = z[i] * rcp_fast(fma(km1[i], th, 1.0));   // z_i = 0: km1_i = 0, x_i = 0
     x[i] = xi;
     y[i] = K[i] * xi;
     sx += xi;

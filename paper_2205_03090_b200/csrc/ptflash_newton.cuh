@@ -129,7 +129,7 @@ __device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&inv
 template <int NC>
 constexpr int newton_lrows() { return (NC - 1) * (NC - 2) / 2; }            // rows 1 .. NC-2 of the strict lower triangle
 template <int NC>
-constexpr int stabn_smem_doubles() { return newton_lrows<NC>() + 3 * NC; }   // per thread: L, beta, pending step, residual r
+constexpr int stabn_smem_doubles() { return newton_lrows<NC>() + 4 * NC; }   // per thread: L, beta, pending step, residual r, d
 template <int NC>
 constexpr int splitn_smem_doubles() { return newton_lrows<NC>() + 6 * NC; }  // per thread: L, n^V, pending step, g, D, S(x), S(y)
 
@@ -146,6 +146,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
   double* const sb = sm + NL * NEWTON_THREADS;   // accepted point beta = 2 sqrt(W) (B.1a)
   double* const sp = sb + NC * NEWTON_THREADS;   // pending / best-so-far step
   double* const sr = sp + NC * NEWTON_THREADS;   // residual r_i = ln W_i + lnphi_i(w) - d_i at the evaluated point
+  double* const sdd = sr + NC * NEWTON_THREADS;  // d_i = ln z_i + lnphi_i(z) of the lane's mixture
   const int64_t N = io.N;
   const int total = w.qcount[Q_STAB_NEWTON];
   int* ticket = &w.qcount[Q_TICKET_STAB];
@@ -176,6 +177,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
           for (int i = 0; i < NC; ++i) {
             sb[i * NEWTON_THREADS] = w.lnW[((int64_t)sidx * NC + i) * N + n];   // k2_stab_ss left beta = 2 sqrt(W) here
             sp[i * NEWTON_THREADS] = 0.0;
+            sdd[i * NEWTON_THREADS] = __ldg(&w.d[(int64_t)i * N + n]);
           }
           iters = w.tflags[(int64_t)sidx * N + n] >> TF_ITER_SHIFT;
           tr_it = 0;
@@ -210,7 +212,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         const double b = sb[i * NEWTON_THREADS], s = sp[i * NEWTON_THREADS];
         const double h = 0.5 * (searching ? b : b + s);
         W[i] = h * h;                                              // B.1d
-        r[i] = ((act >> i) & 1u) ? 2.0 * log_fast(h) : 0.0;        // ln W_i
+        r[i] = 2.0 * log_fast_m(h, (act >> i) & 1u);                // ln W_i (0 for a z_i = 0 component), branch-free
         sumW += W[i];
       }
       {
@@ -224,8 +226,8 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
       double rmax = 0.0, tm_new = 1.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
-        r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - __ldg(&w.d[(int64_t)i * N + n]) : 0.0;
-        rmax = fmax(rmax, fabs(r[i]));
+        r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - sdd[i * NEWTON_THREADS] : 0.0;
+        rmax = dmax(rmax, fabs(r[i]));
         tm_new = fma(W[i], r[i] - 1.0, tm_new);
         sr[i * NEWTON_THREADS] = r[i];
       }
@@ -236,7 +238,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
           double bn = 0.0;
 #pragma unroll
           for (int i = 0; i < NC; ++i) bn = fma(W[i], 4.0, bn);   // |beta|^2 = 4 sum W
-          Delta = fmax(1.0, 0.5 * sqrt_fast(bn));
+          Delta = dmax(1.0, 0.5 * sqrt_fast(bn));
           Delta_cap = 8.0 * Delta;
         } else if (!reeval) {
           const double act_red = tm_new - tm;
@@ -245,10 +247,10 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
             if (fabs(pred) > 1.0e-13) {
               const double ratio = fabs(act_red * rcp_fast(pred));
               if (ratio <= 0.25) Delta *= 0.5;
-              else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, Delta_cap);
+              else if (ratio >= 0.75) Delta = dmin(2.0 * Delta, Delta_cap);
             }
           } else {
-            Delta = 0.5 * fmin(Delta, snorm);
+            Delta = 0.5 * dmin(Delta, snorm);
             reeval = true;   // next trip re-evaluates at the accepted point (s = 0) and continues from there
           }
         }
@@ -334,7 +336,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         searching = false;
         double smax = 0.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) smax = fmax(smax, fabs(sp[i * NEWTON_THREADS]));
+        for (int i = 0; i < NC; ++i) smax = dmax(smax, fabs(sp[i * NEWTON_THREADS]));
         if (exact && smax < o.tol_newton_step_stab) {
           // quadratic-convergence finish: apply the full Newton step and stop
           finish = true;
@@ -463,7 +465,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           const bool a = (act >> i) & 1u;
-          const double f = a ? log_fast(c[i]) + lp[i] : 0.0;
+          const double f = a ? log_fast_m(c[i], a) + lp[i] : 0.0;
           G_new = fma(c[i] * wph, f, G_new);
           sS[(ph * NC + i) * T] = a ? Sv[i] : 0.0;
           if (ph == 0) {
@@ -472,7 +474,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           } else {
             const double g = sg[i * T] + f;
             sg[i * T] = g;
-            gmax = fmax(gmax, fabs(g));
+            gmax = dmax(gmax, fabs(g));
             sD[i * T] = a ? __ldg(&w.zn[(int64_t)i * N + n]) * rcp_fast(sD[i * T] * c[i]) : 1.0;
           }
         }
@@ -486,10 +488,10 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           if (fabs(pred) > 1.0e-13) {
             const double ratio = fabs(act_red * rcp_fast(pred));
             if (ratio <= 0.25) Delta *= 0.5;
-            else if (ratio >= 0.75) Delta = fmin(2.0 * Delta, 1.0);
+            else if (ratio >= 0.75) Delta = dmin(2.0 * Delta, 1.0);
           }
         } else {
-          Delta = 0.5 * fmin(Delta, snorm);
+          Delta = 0.5 * dmin(Delta, snorm);
           reeval = true;
           PTF_DBG(1, 1);
         }
@@ -593,7 +595,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         for (int i = 0; i < NC; ++i) {
           if ((act >> i) & 1u) {
             const double ni = sn[i * T];
-            smax = fmax(smax, fabs(sp[i * T]) * rcp_fast(fmin(ni, __ldg(&w.zn[(int64_t)i * N + n]) - ni)));
+            smax = dmax(smax, fabs(sp[i * T]) * rcp_fast(dmin(ni, __ldg(&w.zn[(int64_t)i * N + n]) - ni)));
           }
         }
         if (exact && smax < o.tol_newton_step) {
@@ -620,7 +622,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       double mkn = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i)
-        if ((act >> i) & 1u) mkn = fmax(mkn, fabs(y[i] - x[i]) * rcp_fast(x[i]));
+        if ((act >> i) & 1u) mkn = dmax(mkn, fabs(y[i] - x[i]) * rcp_fast(x[i]));
       const bool trivial = mkn < 1.0e-9;
       if (io.lnK) {
 #pragma unroll

@@ -51,7 +51,7 @@ __device__ __forceinline__ bool split_iteration(const Sys<NC>& S, const double (
   rk = 0.0;
 #pragma unroll
   for (int i = 0; i < NC; ++i)
-    if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = fmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
+    if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = dmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
   return true;
 }
 
@@ -106,11 +106,12 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           const double di = __ldg(&w.d[(int64_t)i * io.N + n]);
-          if (x[i] > 0.0) tx = fma(x[i], log_fast(x[i]) + lpx[i] - di, tx);
-          if (y[i] > 0.0) ty = fma(y[i], log_fast(y[i]) + lpy[i] - di, ty);
+          // z_i = 0: x_i = y_i = 0 and the term is 0 * (ln 1 + ..) = 0, without a branch around the logarithms
+          tx = fma(x[i], log_fast_m(x[i], x[i] > 0.0) + lpx[i] - di, tx);
+          ty = fma(y[i], log_fast_m(y[i], y[i] > 0.0) + lpy[i] - di, ty);
         }
         const double dG = (1.0 - theta) * tx + theta * ty;
-        const double mn = fmin(dG, fmin(tx, ty));
+        const double mn = dmin(dG, dmin(tx, ty));
         if (mn < -o.probe_margin) { tpd_min = mn; pcase = 3; }
       }
       w.iters[n] += iters;
@@ -131,14 +132,21 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
 }
 
 // ---- K2: stability SS -----------------------------------------------------------------------------
-// Register-lean: the only per-component state kept across iterations is ln W; d is re-read from the workspace
-// (L1/L2 resident) and sqrt(A_i), B_i are rebuilt from three scalars, so four CTAs of 128 threads fit per SM.
+// Register-lean: the only per-component state kept in registers across iterations is ln W; d sits in shared memory
+// (one conflict-free column per thread) and sqrt(A_i), B_i are rebuilt from three scalars, so four CTAs of 128 threads
+// fit per SM.  Branch-free over the components: a component with z_i = 0 is carried at ln W_i = LNW_ZERO (W_i underflows
+// to ~1e-308 and drops out of every sum) and masked out of the residual with selects, so that the ten exponentials
+// of an iteration are one straight-line block the scheduler can interleave (with `act ? exp(..) : 0` the compiler
+// emitted ten branch-around blocks, i.e. ten serial Horner chains).
 #ifndef PTF_SS_MINB
 #define PTF_SS_MINB 4
 #endif
+constexpr double LNW_ZERO = -1000.0;
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  __shared__ double s_d[NC * 128];
+  double* const sd = s_d + threadIdx.x;
   const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
@@ -161,7 +169,10 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
         start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
         const double side = sidx ? -1.0 : 1.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], w.lnz[(int64_t)i * N + n]) : 0.0;
+        for (int i = 0; i < NC; ++i) {
+          lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], w.lnz[(int64_t)i * N + n]) : LNW_ZERO;
+          sd[i * 128] = __ldg(&w.d[(int64_t)i * N + n]);
+        }
       }
       Eos e;
       e.Z = 0.0;
@@ -174,7 +185,7 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
         // evaluate the residual r = ln W + lnphi(w) - d at the current iterate
         sumW = 0.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) { W[i] = ((act >> i) & 1u) ? exp_fast(lnW[i]) : 0.0; sumW += W[i]; }
+        for (int i = 0; i < NC; ++i) { W[i] = exp_fast(lnW[i]); sumW += W[i]; }
         {
           const double inv = rcp_fast(sumW);
           double wn[NC];
@@ -182,36 +193,30 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
           for (int i = 0; i < NC; ++i) wn[i] = W[i] * inv;
           lnphi_pt<NC, KIJ0>(S, q, wn, lp, Sv, e);
         }
-        double rmax = 0.0;
+        bool conv = true;
         tm = 1.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           // lp <- d - lnphi (the next iterate of eq. 5); r = ln W - (d - lnphi)
-          lp[i] = __ldg(&w.d[(int64_t)i * N + n]) - lp[i];
-          const double r = ((act >> i) & 1u) ? lnW[i] - lp[i] : 0.0;
-          rmax = fmax(rmax, fabs(r));
-          tm = fma(W[i], r - 1.0, tm);
+          lp[i] = sd[i * 128] - lp[i];
+          const double r = lnW[i] - lp[i];
+          conv = conv && (!((act >> i) & 1u) || fabs(r) < o.tol_ss);
+          tm = fma(W[i], r - 1.0, tm);   // a z_i = 0 component adds ~1e-305
         }
-        if (rmax < o.tol_ss) { converged = true; break; }
+        if (conv) { converged = true; break; }
         if (k == ss_max) { capped = !o.use_newton; break; }   // the last pass only evaluates (pure-SS mode reports the cap)
-        if (k == ss_max - 1 && o.use_newton) {
-          // hand-over to the Newton stage after ss_max updates: no further evaluation needed here
 #pragma unroll
-          for (int i = 0; i < NC; ++i)
-            if ((act >> i) & 1u) lnW[i] = lp[i];
-          iters++;
-          break;
-        }
-#pragma unroll
-        for (int i = 0; i < NC; ++i)
-          if ((act >> i) & 1u) lnW[i] = lp[i];  // eq. 5
+        for (int i = 0; i < NC; ++i) lnW[i] = ((act >> i) & 1u) ? lp[i] : LNW_ZERO;  // eq. 5
         iters++;
+        if (k == ss_max - 1 && o.use_newton) break;   // hand-over to the Newton stage after ss_max updates: no further evaluation needed here
       }
       need_newton = !converged && o.use_newton;
 #pragma unroll
-      for (int i = 0; i < NC; ++i)
-        w.lnW[((int64_t)sidx * NC + i) * N + n] =
-            need_newton ? (((act >> i) & 1u) ? 2.0 * exp_fast(0.5 * lnW[i]) : 0.0) : lnW[i];   // Newton works in beta = 2 sqrt(W) (B.1a)
+      for (int i = 0; i < NC; ++i) {
+        const bool a = (act >> i) & 1u;
+        const double hb = 2.0 * exp_fast(0.5 * lnW[i]);   // Newton works in beta = 2 sqrt(W) (B.1a)
+        w.lnW[((int64_t)sidx * NC + i) * N + n] = a ? (need_newton ? hb : lnW[i]) : 0.0;
+      }
       w.tm[(int64_t)sidx * N + n] = tm;
       w.sumW[(int64_t)sidx * N + n] = sumW;
       w.tflags[(int64_t)sidx * N + n] = (converged ? TF_CONVERGED : 0) | (capped ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
@@ -300,7 +305,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         double mk = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i)
-          if (z[i] > 0.0) mk = fmax(mk, fabs(lnK[i]));
+          if (z[i] > 0.0) mk = dmax(mk, fabs(lnK[i]));
         if (mk < 1.0e-9) { failed = true; break; }   // trivial collapse
         {
           double K[NC];
@@ -324,7 +329,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         double rk = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i)
-          if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = fmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
+          if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = dmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
         ++k;
         if (rk < 1.0e-14) final_rr = true;
         else if (r_prev > 0.0 && rk < o.tol_ss) {
@@ -340,7 +345,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         // and its stationary point are the same, and the final store restores the phase identity by Z (C23).
         const bool mirror = theta > 0.5;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = fmin(mirror ? (1.0 - theta) * x[i] : theta * y[i], z[i]);
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = dmin(mirror ? (1.0 - theta) * x[i] : theta * y[i], z[i]);
         w.iters[n] += k;
         w.status[n] |= status;
         w.Zxy[n] = mirror ? Zy : Zx;

@@ -311,11 +311,11 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
       // trials finished by the Newton stage come back as beta = 2 sqrt(W) (B.1a): ln W = 2 ln(beta / 2)
       if (fv & TF_BETA) {
 #pragma unroll
-        for (int i = 0; i < NC; ++i) sv.lnW[i] = (m.z[i] > 0.0) ? 2.0 * log_fast(0.5 * sv.lnW[i]) : 0.0;
+        for (int i = 0; i < NC; ++i) sv.lnW[i] = 2.0 * log_fast_m(0.5 * sv.lnW[i], m.z[i] > 0.0);
       }
       if (fl_ & TF_BETA) {
 #pragma unroll
-        for (int i = 0; i < NC; ++i) sl.lnW[i] = (m.z[i] > 0.0) ? 2.0 * log_fast(0.5 * sl.lnW[i]) : 0.0;
+        for (int i = 0; i < NC; ++i) sl.lnW[i] = 2.0 * log_fast_m(0.5 * sl.lnW[i], m.z[i] > 0.0);
       }
       sv.tm = w.tm[n]; sv.sumW = w.sumW[n]; sv.iters = fv >> TF_ITER_SHIFT;
       sv.converged = fv & TF_CONVERGED; sv.stationary_exact = fv & TF_EXACT; sv.capped = fv & TF_CAPPED;
