@@ -44,6 +44,10 @@ struct ptflash_handle_s {
   cudaEvent_t events[PTF_MAX_STAGE_EVENTS];
   bool events_made;
   int n_events;
+  // second stream + fork/join events of the staged engine (created on first use)
+  cudaStream_t aux_stream;
+  cudaEvent_t ev_fork, ev_join;
+  bool aux_made;
 };
 
 namespace {
@@ -66,6 +70,7 @@ ptf::Opt make_opt(const double* o) {
   r.ss_cap = (int)o[PTFLASH_OPT_SS_CAP];
   r.prof_events = nullptr;
   r.prof_count = nullptr;
+  r.aux_stream = r.ev_fork = r.ev_join = nullptr;
   return r;
 }
 
@@ -160,6 +165,7 @@ int ptflash_destroy(ptflash_handle_t h) {
   if (h->counters_host) cudaFreeHost(h->counters_host);
   if (h->events_made)
     for (int i = 0; i < PTF_MAX_STAGE_EVENTS; ++i) cudaEventDestroy(h->events[i]);
+  if (h->aux_made) { cudaStreamDestroy(h->aux_stream); cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join); }
   delete h;
   return rc;
 }
@@ -210,6 +216,14 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
     }
     o.prof_events = h->events;
     o.prof_count = &h->n_events;
+  } else if (engine) {
+    if (!h->aux_made) {
+      if (!cuda_ok(cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking), "cudaStreamCreate")) return PTFLASH_ECUDA;
+      if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+      if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+      h->aux_made = true;
+    }
+    o.aux_stream = h->aux_stream; o.ev_fork = h->ev_fork; o.ev_join = h->ev_join;
   }
   const int launches = fn(h->sys, o, d, h->ws, st);
   if (launches < 0) { cuda_ok(cudaGetLastError(), "kernel launch"); if (g_err.empty()) set_err("kernel launch failed"); return PTFLASH_ECUDA; }

@@ -29,6 +29,9 @@ struct Opt {
   // host only: cudaEvent_t[PTF_MAX_STAGE_EVENTS] recorded between the stage kernels when stage profiling is on (else null)
   void* prof_events;
   int* prof_count;   // host only: number of events recorded by the last launch
+  // host only: second stream of the handle and two events (fork / join) so that the phase split of the mixtures the probe
+  // already found unstable runs concurrently with the stability analysis of the others (null: everything on one stream)
+  void *aux_stream, *ev_fork, *ev_join;
 };
 #define PTF_MAX_STAGE_EVENTS 24
 

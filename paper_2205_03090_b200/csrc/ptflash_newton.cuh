@@ -19,7 +19,10 @@
 
 namespace ptf {
 
-constexpr int NEWTON_THREADS = 128;
+#ifndef PTF_NEWTON_THREADS
+#define PTF_NEWTON_THREADS 128
+#endif
+constexpr int NEWTON_THREADS = PTF_NEWTON_THREADS;
 
 #ifndef PTF_NEWTON_CTA_SYNC
 #define PTF_NEWTON_CTA_SYNC 1
@@ -376,7 +379,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(NEWTON_THREADS, PTF_SPLITN_MINB)
 k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o, const __grid_constant__ Io io,
-                const __grid_constant__ Work w) {
+                const __grid_constant__ Work w, const int part) {
   constexpr int NL = newton_lrows<NC>();
   constexpr int T = NEWTON_THREADS;
   constexpr unsigned FULL = 0xffffffffu;
@@ -389,8 +392,9 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   double* const sD = sg + NC * T;    // D_i = z_i / (x_i y_i)
   double* const sS = sD + NC * T;    // S(x) [NC], S(y) [NC]
   const int64_t N = io.N;
-  const int total = w.qcount[Q_SPLIT_NEWTON];
-  int* ticket = &w.qcount[Q_TICKET_SPLIT];
+  const int total = w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON];
+  const int* const q_in = part ? w.q_split_newton_b : w.q_split_newton;
+  int* ticket = &w.qcount[part ? Q_TICKET_SPLIT_B : Q_TICKET_SPLIT];
   bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
   int n = 0, tr_it = 0, status = 0;
   unsigned act = 0u;
@@ -409,7 +413,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       const int64_t tk = take_ticket(!busy && !exhausted, ticket);
       if (tk >= 0) {
         if (tk < total) {
-          n = w.q_split_newton[tk];
+          n = q_in[tk];
           const double P = io.P[n], Tk = io.T[n];
           { const double iT = rcp_fast(Tk); q.sT = sqrt_fast(Tk); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
           act = (unsigned)w.actmask[n];

@@ -277,8 +277,10 @@ __device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, 
 
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                                   const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  const int64_t cnt = w.qcount[Q_SPLIT];
+                                                                   const __grid_constant__ Io io, const __grid_constant__ Work w,
+                                                                   const int part) {
+  const int* const q_in = part ? w.q_split_b : w.q_split;
+  const int64_t cnt = w.qcount[part ? Q_SPLIT_B : Q_SPLIT];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
   PTF_GRID_STRIDE(idx, pad) {
@@ -286,7 +288,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
     bool go_newton = false;
     int n = 0;
     if (in) {
-      n = w.q_split[idx];
+      n = q_in[idx];
       double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
       const double P = io.P[n], T = io.T[n];
       PT3<NC> q;
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         store_split<NC>(io, w, n, z, converged, failed, theta, k, status, x, y, lnK, Zx, Zy);
       }
     }
-    queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
+    queue_push(go_newton, &w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON], part ? w.q_split_newton_b : w.q_split_newton, n);
   }
 }
 
@@ -393,24 +395,41 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
   mark();
   int launches = 1;
+  // Fork: the split of the mixtures the probe (or the caller's flag) already declared unstable (part 0) does not depend on
+  // the stability kernels, so it runs on the handle's second stream; its long tail (a few hard mixtures with many
+  // trust-region iterations) then overlaps with the stability stages instead of idling the GPU.  With stage profiling
+  // on, everything stays on the caller's stream so that the event-to-event times are per stage.
+  cudaStream_t aux = (cudaStream_t)o.aux_stream;
+  const bool fork = aux != nullptr && ev == nullptr;
+  w.decide_part = 1;
   const int passes = (io.flags && io.lnK0) ? 2 : 1;   // pass 1: cold re-flash of mixtures whose skip-stability hint failed
   for (int pass = 0; pass < passes; ++pass) {
     w.pass = pass;
     if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
     k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
+    if (fork) {
+      cudaEventRecord((cudaEvent_t)o.ev_fork, st);
+      cudaStreamWaitEvent(aux, (cudaEvent_t)o.ev_fork, 0);
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, aux>>>(s, o, io, w, 0);
+      k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, aux>>>(s, o, io, w, 0);
+      cudaEventRecord((cudaEvent_t)o.ev_join, aux);
+    }
     k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
     mark();
     k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), NEWTON_THREADS, stab_bytes, st>>>(s, o, io, w);
     mark();
     k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
-    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+    if (!fork) k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0);
+    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1);
     mark();
-    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w);
+    if (!fork) k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
+    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 1);
+    if (fork) cudaStreamWaitEvent(st, (cudaEvent_t)o.ev_join, 0);   // join
     k_finalize_counters<<<1, 32, 0, st>>>(w);
     mark();
-    launches += 7;
+    launches += 9;
   }
   if (o.prof_count) *o.prof_count = nev;
   return cudaGetLastError() == cudaSuccess ? launches : -1;

@@ -25,13 +25,18 @@
 
 namespace ptf {
 
-enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_RETRY = 7, Q_COUNT = 8 };
+// The phase split has two queue sets: part 0 = mixtures the probe (or the caller) sent straight to the split, part 1 =
+// mixtures the stability analysis found unstable (Q_*_B).  Engine 1 runs part 0 on a second stream, concurrently with
+// the stability kernels; the plain stage kernels (launch_staged) use part 0 for both.
+enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_RETRY = 7,
+              Q_SPLIT_B = 8, Q_SPLIT_NEWTON_B = 9, Q_TICKET_SPLIT_B = 10, Q_COUNT = 11 };
 enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_BETA = 8, TF_ITER_SHIFT = 8 + 0 };
 
 struct Work {
   StageCounters* ctr;
   int* qcount;  // [Q_COUNT]
-  int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton, *q_retry;
+  int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton, *q_retry, *q_split_b, *q_split_newton_b;
+  int decide_part;  // queue set k_stab_decide feeds (0 / 1)
   int pass;  // 0: first pass; 1: re-flash of mixtures whose skip-stability hint failed (ST_WARM_RESTART)
   double *lnz, *d, *lnK;   // [NC][N]
   double* zn;              // [NC][N] normalised feed z / sum z (written once by k_init)
@@ -60,7 +65,9 @@ inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   p = take(n * 4); if (w) w->q_split = (int*)p;
   p = take(n * 4); if (w) w->q_split_newton = (int*)p;
   p = take(n * 4); if (w) w->q_retry = (int*)p;
-  if (w) w->pass = 0;
+  p = take(n * 4); if (w) w->q_split_b = (int*)p;
+  p = take(n * 4); if (w) w->q_split_newton_b = (int*)p;
+  if (w) { w->pass = 0; w->decide_part = 0; }
   p = take(c * n * 8); if (w) w->lnz = (double*)p;
   p = take(c * n * 8); if (w) w->d = (double*)p;
   p = take(c * n * 8); if (w) w->lnK = (double*)p;
@@ -337,7 +344,7 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
         store_result<NC>(io, n, false, 0.0, m.z, m.z, m.z, lnK, w.Zfeed[n], w.iters[n], status & ~ST_INTERNAL_SKIPPED, tpd_min, stab_iters, false);
       }
     }
-    queue_push(unstable, &w.qcount[Q_SPLIT], w.q_split, n);
+    queue_push(unstable, &w.qcount[w.decide_part ? Q_SPLIT_B : Q_SPLIT], w.decide_part ? w.q_split_b : w.q_split, n);
   }
 }
 
@@ -429,8 +436,8 @@ static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     w.ctr->n_stab += w.qcount[Q_STAB];
     w.ctr->n_stab_newton += w.qcount[Q_STAB_NEWTON];
-    w.ctr->n_split += w.qcount[Q_SPLIT];
-    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON];
+    w.ctr->n_split += w.qcount[Q_SPLIT] + w.qcount[Q_SPLIT_B];
+    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_B];
   }
 }
 
@@ -443,6 +450,7 @@ static __global__ void k_begin_pass2(const __grid_constant__ Work w) {
     w.qcount[Q_PROBE] = cnt;
     w.qcount[Q_STAB] = 0; w.qcount[Q_STAB_NEWTON] = 0; w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0;
     w.qcount[Q_TICKET_STAB] = 0; w.qcount[Q_TICKET_SPLIT] = 0; w.qcount[Q_RETRY] = 0;
+    w.qcount[Q_SPLIT_B] = 0; w.qcount[Q_SPLIT_NEWTON_B] = 0; w.qcount[Q_TICKET_SPLIT_B] = 0;
     w.ctr->reserved[0] = cnt;   // number of warm restarts
   }
 }
