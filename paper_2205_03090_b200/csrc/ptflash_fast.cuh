@@ -38,21 +38,22 @@ __device__ __forceinline__ double pick_root_fast(double A, double B, double Zg, 
   double Z = Zg;
   bool ok = false;
   if (Zg > B) {
-    // plain Newton from the previous root; accept only a clean quadratic finish
+    // Halley's iteration (A.4, third order) from the previous root: a step below 1e-5 Z leaves an error ~ step^3, i.e.
+    // rounding level, so the typical warm start costs two evaluations (Newton needed three plus a confirming one).
 #pragma unroll 1
     for (int k = 0; k < 4; ++k) {
-      const double df = cub_df(Z, r1);
-      const double dz = cub_f(Z, r1, r0) * rcp_nr1(df);
+      const double f = cub_f(Z, r1, r0), df = cub_df(Z, r1);
+      const double d2 = fma(3.0, Z, -1.0);                     // f'' / 2
+      const double dz = f * df * rcp_nr1(fma(df, df, -f * d2));
       const double Zn = Z - dz;
-      if (!(Zn > B) || !(Zn < 2.0 + B)) break;   // also catches NaN / df == 0
+      if (!(Zn > B) || !(Zn < 2.0 + B)) break;   // also catches NaN / a vanishing denominator
       Z = Zn;
-      if (fabs(dz) <= 1.0e-8 * Zn) { ok = true; break; }
+      if (fabs(dz) <= 1.0e-5 * Zn) { ok = true; break; }
     }
     if (ok) {
-      // one more guarded step brings the root to rounding (and detects a linear-rate, i.e. nearly double, root)
-      const double df = cub_df(Z, r1);
-      const double dz = cub_f(Z, r1, r0) * rcp_nr1(df);
-      if (fabs(dz) <= 1.0e-13 * Z) Z -= dz; else ok = false;
+      // one Newton step brings the root to rounding and detects a linear-rate (nearly double) root
+      const double dz = cub_f(Z, r1, r0) * rcp_nr1(cub_df(Z, r1));
+      if (fabs(dz) <= 1.0e-11 * Z) Z -= dz; else ok = false;
     }
   }
   if (!ok) {
@@ -152,13 +153,18 @@ template <int NC, bool KIJ0>
 __device__ __forceinline__ void lnphi_pt(const Sys<NC>& S, const PT3<NC>& q, const double (&c)[NC], double (&lp)[NC],
                                          double (&Sv)[NC], Eos& e) {
   double t[NC];
-  double B = 0.0;
+  double B0 = 0.0, B1 = 0.0;   // two accumulation chains each (depth NC/2 instead of NC)
 #pragma unroll
-  for (int j = 0; j < NC; ++j) { t[j] = sa_of<NC>(S, q, j) * c[j]; B = fma(c[j], bi_of<NC>(S, q, j), B); }
+  for (int j = 0; j < NC; ++j) {
+    t[j] = sa_of<NC>(S, q, j) * c[j];
+    if (j & 1) B1 = fma(c[j], S.wb[j], B1); else B0 = fma(c[j], S.wb[j], B0);
+  }
+  const double B = q.pt * (B0 + B1);   // B_i = (P/T) wb_i
   if (KIJ0) {
-    double sum = 0.0;
+    double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-    for (int j = 0; j < NC; ++j) sum += t[j];
+    for (int j = 0; j < NC; ++j) { if (j & 1) s1 += t[j]; else s0 += t[j]; }
+    const double sum = s0 + s1;
 #pragma unroll
     for (int i = 0; i < NC; ++i) Sv[i] = sa_of<NC>(S, q, i) * sum;
   } else {

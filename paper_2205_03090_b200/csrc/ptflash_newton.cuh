@@ -210,14 +210,16 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
     if (busy) {
       // ---- evaluate tm and its gradient: at the trial point beta + s, or at beta while an eta search is pending ----
       double W[NC], lp[NC], r[NC];
+      double sumW1 = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
         const double b = sb[i * NEWTON_THREADS], s = sp[i * NEWTON_THREADS];
         const double h = 0.5 * (searching ? b : b + s);
         W[i] = h * h;                                              // B.1d
         r[i] = 2.0 * log_fast_m(h, (act >> i) & 1u);                // ln W_i (0 for a z_i = 0 component), branch-free
-        sumW += W[i];
+        if (i & 1) sumW1 += W[i]; else sumW += W[i];                // two accumulation chains
       }
+      sumW += sumW1;
       {
         const double inv = rcp_fast(sumW);
         double wn[NC];
@@ -226,14 +228,16 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         lnphi_pt<NC, KIJ0>(S, q, wn, lp, Sv, e);
       }
       Zw = e.Z;
-      double rmax = 0.0, tm_new = 1.0;
+      double rmax = 0.0, rmax1 = 0.0, tm_new = 1.0, tm_new1 = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
         r[i] = ((act >> i) & 1u) ? r[i] + lp[i] - sdd[i * NEWTON_THREADS] : 0.0;
-        rmax = dmax(rmax, fabs(r[i]));
-        tm_new = fma(W[i], r[i] - 1.0, tm_new);
+        if (i & 1) { rmax1 = dmax(rmax1, fabs(r[i])); tm_new1 = fma(W[i], r[i] - 1.0, tm_new1); }
+        else { rmax = dmax(rmax, fabs(r[i])); tm_new = fma(W[i], r[i] - 1.0, tm_new); }
         sr[i * NEWTON_THREADS] = r[i];
       }
+      rmax = dmax(rmax, rmax1);
+      tm_new += tm_new1;
       if (!searching) {
         // ---- accept / reject the pending step (B.3) ----
         bool accepted = true;

@@ -183,9 +183,10 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
 #pragma unroll 1
       for (int k = 0; k <= ss_max; ++k) {
         // evaluate the residual r = ln W + lnphi(w) - d at the current iterate
-        sumW = 0.0;
+        double sw0 = 0.0, sw1 = 0.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) { W[i] = exp_fast(lnW[i]); sumW += W[i]; }
+        for (int i = 0; i < NC; ++i) { W[i] = exp_fast(lnW[i]); if (i & 1) sw1 += W[i]; else sw0 += W[i]; }
+        sumW = sw0 + sw1;
         {
           const double inv = rcp_fast(sumW);
           double wn[NC];
@@ -194,15 +195,16 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
           lnphi_pt<NC, KIJ0>(S, q, wn, lp, Sv, e);
         }
         bool conv = true;
-        tm = 1.0;
+        double tm0 = 1.0, tm1 = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           // lp <- d - lnphi (the next iterate of eq. 5); r = ln W - (d - lnphi)
           lp[i] = sd[i * 128] - lp[i];
           const double r = lnW[i] - lp[i];
           conv = conv && (!((act >> i) & 1u) || fabs(r) < o.tol_ss);
-          tm = fma(W[i], r - 1.0, tm);   // a z_i = 0 component adds ~1e-305
+          if (i & 1) tm1 = fma(W[i], r - 1.0, tm1); else tm0 = fma(W[i], r - 1.0, tm0);   // a z_i = 0 component adds ~1e-305
         }
+        tm = tm0 + tm1;
         if (conv) { converged = true; break; }
         if (k == ss_max) { capped = !o.use_newton; break; }   // the last pass only evaluates (pure-SS mode reports the cap)
 #pragma unroll

@@ -22,6 +22,7 @@
 #include "ptflash_flash.cuh"
 #include "ptflash_launch.h"
 #include "ptflash_math.cuh"
+#include "ptflash_fast.cuh"
 
 namespace ptf {
 
@@ -142,7 +143,19 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
     count_add(in && !valid, &w.ctr->n_invalid);
     int dest = -1;  // 0 probe, 1 stab, 2 split
     if (valid) {
-      feed_reference<NC>(S, P, T, m, Zf);
+      {
+        // ln z, per-(P,T) setup and d = ln z + lnphi(z) with the lean math (cold cubic: no previous root)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) m.lnz[i] = log_fast_m(m.z[i], m.z[i] > 0.0);
+        eos_setup<NC>(S, P, T, m.sa, m.bi);
+        double lp[NC], Sv[NC];
+        Eos e;
+        e.Z = 0.0;
+        lnphi_fast<NC, false>(S, m.sa, m.bi, m.z, lp, Sv, e);
+        Zf = e.Z;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) m.d[i] = m.lnz[i] + lp[i];
+      }
       int status = 0, fl = 0;
       double lnKs[NC];
       const bool have0 = start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
@@ -177,13 +190,12 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
         double f0 = 0.0, f1 = 0.0, Kmax = 0.0, Kmin = 1.0e300;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
-          if (m.z[i] > 0.0) {
-            const double K = exp(lnKs[i]);
-            Kmax = fmax(Kmax, K);
-            Kmin = fmin(Kmin, K);
-            f0 = fma(m.z[i], K - 1.0, f0);
-            f1 += m.z[i] * (K - 1.0) / K;
-          }
+          const bool a = m.z[i] > 0.0;
+          const double K = exp_fast(a ? lnKs[i] : 0.0);   // z_i = 0: K = 1 drops out of every term below
+          Kmax = dmax(Kmax, K);
+          Kmin = dmin(Kmin, K);
+          f0 = fma(m.z[i], K - 1.0, f0);
+          f1 = fma(m.z[i] * (K - 1.0), rcp_fast(K), f1);
         }
         dest = (Kmax > 1.0 && Kmin < 1.0 && f0 > 0.0 && f1 < 0.0) ? 0 : 1;
       }
