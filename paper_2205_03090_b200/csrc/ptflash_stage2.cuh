@@ -397,10 +397,13 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
   mark();
   int launches = 1;
-  // Fork: the split of the mixtures the probe (or the caller's flag) already declared unstable (part 0) does not depend on
-  // the stability kernels, so it runs on the handle's second stream; its long tail (a few hard mixtures with many
-  // trust-region iterations) then overlaps with the stability stages instead of idling the GPU.  With stage profiling
-  // on, everything stays on the caller's stream so that the event-to-event times are per stage.
+  // Fork after the stability stages.  The phase split has two parts: (0) the mixtures the probe (or the caller's flag)
+  // declared unstable -- most of them, well conditioned -- and (1) the few the stability analysis found unstable: close
+  // to the phase boundary, where single mixtures take ~100 trust-region trips, so that part 1 alone ends in a long tail
+  // with a handful of busy lanes (0.7 ms of a 4.2 ms call on config 3).  Part 1 runs on the caller's stream, part 0 on the
+  // handle's second stream at the same time, so the tail of one is covered by the bulk of the other.  (Running part 0
+  // earlier, concurrently with the stability kernels, gains little: those fill the register file on their own.)
+  // With stage profiling on, everything stays on the caller's stream so that the event-to-event times are per stage.
   cudaStream_t aux = (cudaStream_t)o.aux_stream;
   const bool fork = aux != nullptr && ev == nullptr;
   w.decide_part = 1;
@@ -410,25 +413,30 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
     k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
-    if (fork) {
-      cudaEventRecord((cudaEvent_t)o.ev_fork, st);
-      cudaStreamWaitEvent(aux, (cudaEvent_t)o.ev_fork, 0);
-      k2_split_ss<NC, KIJ0><<<gN, threads, 0, aux>>>(s, o, io, w, 0);
-      k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, aux>>>(s, o, io, w, 0);
-      cudaEventRecord((cudaEvent_t)o.ev_join, aux);
-    }
     k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
     mark();
     k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), NEWTON_THREADS, stab_bytes, st>>>(s, o, io, w);
     mark();
     k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
-    if (!fork) k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0);
-    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1);
-    mark();
-    if (!fork) k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
-    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 1);
-    if (fork) cudaStreamWaitEvent(st, (cudaEvent_t)o.ev_join, 0);   // join
+    if (fork) {
+      cudaEventRecord((cudaEvent_t)o.ev_fork, st);
+      cudaStreamWaitEvent(aux, (cudaEvent_t)o.ev_fork, 0);
+      // part 1 first: its hard items should start as early as possible, every one on a lane of its own if they fit
+      // (one CTA per SM: 19 k lanes on B200, and room for part 0 next to it)
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1);
+      k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 1);
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, aux>>>(s, o, io, w, 0);
+      k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, aux>>>(s, o, io, w, 0);
+      cudaEventRecord((cudaEvent_t)o.ev_join, aux);
+      cudaStreamWaitEvent(st, (cudaEvent_t)o.ev_join, 0);   // join
+    } else {
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0);
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1);
+      mark();
+      k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
+      k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 1);
+    }
     k_finalize_counters<<<1, 32, 0, st>>>(w);
     mark();
     launches += 9;
