@@ -289,8 +289,8 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     double f = 0.0, df = 0.0;
 #pragma unroll
     for (int i = 0; i < NC; ++i) {
-      const double r = rcp_fast(fma(km1[i], th, 1.0));
-      const double a = z[i] * km1[i] * r;
+      const double r = rcp_nr1(fma(km1[i], th, 1.0));   // 2^-40 is enough inside the iteration: the error of the final theta
+      const double a = z[i] * km1[i] * r;                // is (relative error of the last step) x (last step <= 1e-8 window)
       f += a;
       df = fma(-a, km1[i] * r, df);
     }

@@ -62,6 +62,8 @@ __device__ __forceinline__ bool split_iteration(const Sys<NC>& S, const double (
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                 const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  __shared__ double s_exp[PTF_EXP_TAB];
+  exp_tab_init(s_exp);
   const int64_t cnt = w.qcount[Q_PROBE];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   PTF_GRID_STRIDE(idx, pad) {
@@ -84,7 +86,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
         {
           double K[NC];
 #pragma unroll
-          for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
+          for (int i = 0; i < NC; ++i) K[i] = exp_tab(lnK[i], s_exp);
           if (!rr_fast<NC>(K, z, theta, x, y) || !(theta > 0.0) || !(theta < 1.0)) { pcase = 1; break; }
         }
         Eos e;
@@ -146,6 +148,8 @@ template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
   __shared__ double s_d[NC * 128];
+  __shared__ double s_exp[PTF_EXP_TAB];
+  exp_tab_init(s_exp);
   double* const sd = s_d + threadIdx.x;
   const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
@@ -185,7 +189,7 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
         // evaluate the residual r = ln W + lnphi(w) - d at the current iterate
         double sw0 = 0.0, sw1 = 0.0;
 #pragma unroll
-        for (int i = 0; i < NC; ++i) { W[i] = exp_fast(lnW[i]); if (i & 1) sw1 += W[i]; else sw0 += W[i]; }
+        for (int i = 0; i < NC; ++i) { W[i] = exp_tab(lnW[i], s_exp); if (i & 1) sw1 += W[i]; else sw0 += W[i]; }
         sumW = sw0 + sw1;
         {
           const double inv = rcp_fast(sumW);
@@ -281,6 +285,8 @@ template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                    const __grid_constant__ Io io, const __grid_constant__ Work w,
                                                                    const int part) {
+  __shared__ double s_exp[PTF_EXP_TAB];
+  exp_tab_init(s_exp);
   const int* const q_in = part ? w.q_split_b : w.q_split;
   const int64_t cnt = w.qcount[part ? Q_SPLIT_B : Q_SPLIT];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
@@ -314,7 +320,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         {
           double K[NC];
 #pragma unroll
-          for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
+          for (int i = 0; i < NC; ++i) K[i] = exp_tab(lnK[i], s_exp);
           if (!rr_fast<NC>(K, z, theta, x, y)) { failed = true; break; }
         }
         if (final_rr) { converged = true; break; }
