@@ -75,9 +75,13 @@ struct LRows {
 // yv[i] = forward substitution of rhs.  Rows 1 .. NC-2 are stored to shared memory; the LAST row is never read by a later
 // row, so it stays in registers and the first step of the back substitution is taken right here (s[NC-1], yv updated).
 // `i` is a compile-time constant after unrolling, so every j < i / k < j test disappears.
-template <int NC>
+// MOD (modified Cholesky): a pivot that is not safely positive is replaced by max(-pivot, 1e-10 |H_ii|) and pd is cleared --
+// the factor then belongs to H + E with a diagonal E >= 0, so the solve still gives a descent direction (a negative
+// curvature direction is followed with its Newton length, sign flipped).
+template <int NC, bool MOD = false>
 __device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const LRows<NC>& L, double (&invd)[NC],
                                          double (&yv)[NC], double (&s)[NC], const double rhs, bool& pd) {
+  const double hii = row[i];
 #pragma unroll
   for (int j = 0; j < NC; ++j) {
     if (j < i) {
@@ -92,7 +96,12 @@ __device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const L
 #pragma unroll
   for (int k = 0; k < NC; ++k)
     if (k < i) { acc = fma(-row[k], row[k], acc); a = fma(-row[k], yv[k], a); }
-  pd = pd && (acc > 0.0);
+  if (MOD) {
+    const double fl = 1.0e-10 * fabs(hii);
+    if (!(acc > fl)) { acc = dmax(-acc, fl); pd = false; }
+  } else {
+    pd = pd && (acc > 0.0);
+  }
   const double inv = rsqrt_fast(acc);
   invd[i] = inv;
   yv[i] = a * inv;
@@ -122,6 +131,9 @@ __device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&inv
   }
 }
 
+#ifndef PTF_SPLIT_MODCHOL
+#define PTF_SPLIT_MODCHOL 1   // split Newton: one modified-Cholesky factorisation per iteration + step truncation (0: eta search)
+#endif
 #ifndef PTF_STABN_MINB
 #define PTF_STABN_MINB 2
 #endif
@@ -569,9 +581,39 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           }
         }
         row[i] = fma(sD[i * T], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
-        chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd);
+        chol_row<NC, PTF_SPLIT_MODCHOL != 0>(i, row, L, invd, yv, st, -sg[i * T], pd);
       }
       chol_back<NC>(L, invd, yv, st);
+#if PTF_SPLIT_MODCHOL
+      // Restricted step without a search: the direction of the (modified) factorisation is cut back to the trust region and
+      // to 90 % of the way to the nearest face of the box 0 < n_i < z_i.  One factorisation, i.e. one trip, per iteration;
+      // the eta search of the paper's B.4a (grow x8, then bisect: up to ten factorisations) is kept for the stability
+      // kernel, whose path decides labels.  Acceptance and the radius update (B.3) are unchanged.
+      {
+        double s2 = 0.0, sgd = 0.0, over = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          const bool a = (act >> i) & 1u;
+          st[i] = a ? st[i] : 0.0;
+          s2 = fma(st[i], st[i], s2);
+          sgd = fma(st[i], sg[i * T], sgd);
+          const double ni = sn[i * T];
+          const double room = a ? dmax(st[i] < 0.0 ? ni : __ldg(&w.zn[(int64_t)i * N + n]) - ni, 1.0e-300) : 1.0;
+          over = dmax(over, fabs(st[i]) * rcp_fast(room));
+        }
+        const double sl = sqrt_fast(s2);
+        double t = 1.0;
+        if (over > 0.9) t = 0.9 * rcp_fast(over);
+        if (sl * t > Delta) t = Delta * rcp_fast(sl);
+        const bool ok = (t == t) && (sl == sl) && sgd < 0.0;   // NaN-free descent direction
+#pragma unroll
+        for (int i = 0; i < NC; ++i) sp[i * T] = ok ? t * st[i] : 0.0;
+        snorm = sl * t;
+        pred = (t - 0.5 * t * t) * sgd;
+        exact = pd && t == 1.0;
+        es.phase = ok ? 3 : 4;
+      }
+#else
       bool good = pd;
       double s2 = 0.0, sds = 0.0, sgd = 0.0;
 #pragma unroll
@@ -595,6 +637,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         exact = (eta_used == 0.0);
       }
       if (!good) PTF_DBG(5, 1);
+#endif
       if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
       else if (es.phase == 3) {
         searching = false;
