@@ -33,15 +33,15 @@ UNIT = "flashes/s"
 WORKLOAD = "config3: 10-component CO2-rich SRK flash (8 n-alkanes + CO2 + N2, kij per BASELINE.json), z=0.6*Dir(1)+0.4*e_CO2, T~U[220,500]K, P~U[5,300]bar, seed 2205030903"
 # Algorithmic FP64 work per flash on this workload: thread-level predicated-on DADD + DMUL + 2*DFMA of
 # all stage kernels, counted by ncu on the committed build (profiles/), per mixture.
-# Per stage kernel, in flops per mixture of the batch (profiles/r01e_kernels.md; the two launches of the split kernels --
+# Per stage kernel, in flops per mixture of the batch (profiles/r01f_kernels.md; the two launches of the split kernels --
 # probe-found and stability-found part -- are summed):
 STAGES = ("k_init", "k2_probe", "k2_stab_ss", "k3_stab_newton", "k_stab_decide", "k2_split_ss", "k3_split_newton")
 STAGE_FLOPS_PER_FLASH = {"k_init": 1.74e3, "k2_probe": 3.93e3, "k2_stab_ss": 10.85e3, "k3_stab_newton": 11.85e3,
-                         "k_stab_decide": 0.69e3, "k2_split_ss": 4.93e3, "k3_split_newton": 1.89e3}
+                         "k_stab_decide": 0.69e3, "k2_split_ss": 4.93e3, "k3_split_newton": 1.86e3}
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch at N = 1e6 from the same ncu passes: whole call,
 # and the dominant kernel k3_stab_newton from its `ncu --set full` capture (profiles/r01e_stab_newton_full.md)
-TRAFFIC_CALL_1M = 4.494e9
-TRAFFIC_STAB_NEWTON_1M = 7.55e8
+TRAFFIC_CALL_1M = 4.507e9
+TRAFFIC_STAB_NEWTON_1M = 7.65e8
 FLOPS_PER_FLASH = float(os.environ.get("PTFLASH_FLOPS_PER_FLASH", sum(STAGE_FLOPS_PER_FLASH.values())))
 BYTES_PER_FLASH_NC10 = 272.0   # 8(nc+2) in + 8(2nc+1)+8 out, SURVEY.md section 8(d)
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # SMs x DFMA lanes/clk x 2 flop x max SM clock
