@@ -220,6 +220,40 @@ def test_host_buffers_stream_and_stats(oracle_mod):
     f.close()
 
 
+def test_two_streams_equal_one_stream(oracle_mod):
+    """Engine 1 forks the two parts of the phase split onto two streams after the stability stages; with stage profiling on
+    everything runs on the caller's stream.  Both orders must give the same bits, repeatedly (no race between the parts),
+    also for the warm-start pass structure, and the stage timers must cover the seven stages."""
+    import torch
+    import config5
+    from paper_2205_03090_b200 import binding as B
+    dev = torch.device("cuda:0")
+    w = W.config3(200_000)
+    z, P, T = (torch.from_numpy(a).to(dev) for a in (w.z, w.P, w.T))
+    f = B.PTFlash.from_system(w.system)
+    ref = {k: v.clone() for k, v in f.flash(z, P, T).items()}
+    for rep in range(3):
+        out = f.flash(z, P, T)
+        for k in ("phase", "beta", "x", "y", "iters", "status"):
+            assert torch.equal(out[k], ref[k]), k
+    f.set_option("stage_profile", 1)
+    out = f.flash(z, P, T)
+    ms = f.stage_ms()
+    assert len(ms) == 7 and all(m > 0 for m in ms)
+    for k in ("phase", "beta", "x", "y", "iters", "status"):
+        assert torch.equal(out[k], ref[k]), k
+    st = f.stats()
+    assert st["n_split"] >= st["n_probe_case3"] and st["n_two_phase"] == int((ref["phase"] == 2).sum())
+    f.close()
+    # warm start with skip-stability flags (two passes), forked vs single stream
+    orc = oracle_mod.Oracle.from_system(W.system_co2_10())
+    w5, lnK0, flags, info = config5.build(orc, 3000)
+    g_fork = _gpu_flash(w5, 1, lnK0=lnK0, flags=flags)
+    g_one = _gpu_flash(w5, 1, lnK0=lnK0, flags=flags, stage_profile=1)
+    for k in ("phase", "beta", "x", "y", "iters", "status"):
+        assert np.array_equal(g_fork[k], g_one[k]), k
+
+
 def test_full_size_sampled_parity_and_invariants(oracle_mod):
     """BASELINE size (config 3, N = 1,000,000, the launch configuration bench.py times): invariants on every mixture,
     oracle parity on a seeded sample computed one by one (mixtures are independent)."""
