@@ -30,6 +30,10 @@ sys.path.insert(0, str(ROOT))
 
 METRIC = "two-phase flashes/sec (fp64, 1 B200) and % of FP64/HBM roofline"
 UNIT = "flashes/s"
+WORKLOADS = {
+    2: "config2: 8-component n-alkane SRK flash (kij = 0), z~Dir(1), T~U[200,600]K, P~U[1,200]bar, seed 2205030902",
+    4: "config4: the 10-component CO2-rich system with z~Dir(0.5), T~U[220,500]K, P~U[5,300]bar, seed 2205030904 (scaling sweep: --n 65536 .. 16777216)",
+}
 WORKLOAD = "config3: 10-component CO2-rich SRK flash (8 n-alkanes + CO2 + N2, kij per BASELINE.json), z=0.6*Dir(1)+0.4*e_CO2, T~U[220,500]K, P~U[5,300]bar, seed 2205030903"
 # Algorithmic FP64 work per flash on this workload: thread-level predicated-on DADD + DMUL + 2*DFMA of
 # all stage kernels, counted by ncu on the committed build (profiles/), per mixture.
@@ -127,6 +131,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=1_000_000, help="mixtures per GPU per step")
     ap.add_argument("--engine", type=int, default=1)
+    ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4],
+                    help="BASELINE config to time (3 = the headline workload; 2 and 4 report throughput only: the flop count "
+                         "behind the roofline fraction is config 3's)")
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--cpu-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -151,7 +158,8 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     N = args.n
-    w = W.config3(N, offset=rank * N)      # each rank: its own shard of the same seeded stream
+    w = W.CONFIGS[args.config](N, offset=rank * N)      # each rank: its own shard of the same seeded stream
+    workload = WORKLOAD if args.config == 3 else WORKLOADS[args.config]
     nc = w.system.nc
     f = B.PTFlash.from_system(w.system, engine=args.engine)
     z, P, T = (torch.from_numpy(a).to(dev) for a in (w.z, w.P, w.T))
@@ -262,7 +270,11 @@ def main():
         "hbm_peak_gbs": hbm, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback",
         "kernel": "all stage kernels of one ptflash_flash call (k_init .. k_split_newton)",
     }
-    if stage_ms:
+    if args.config != 3:
+        for k in ("achieved", "frac", "flops_per_flash", "traffic"):
+            roofline[k] = None
+        roofline["note"] = "flops per flash are counted for config 3 only"
+    if stage_ms and args.config == 3:
         # the same figure per stage kernel; "dominant" = the kernel with the largest share of the step
         per = {}
         for name, ms in zip(STAGES, stage_ms):
@@ -284,9 +296,11 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": WORKLOAD, "mixtures_per_gpu_per_step": N, "nc": nc, "engine": args.engine,
+        "config": {"workload": workload, "mixtures_per_gpu_per_step": N, "nc": nc, "engine": args.engine,
                    "two_phase_fraction": two_phase,
-                   "l2": "inputs+outputs per step are 272 MB > 126 MB L2 (plus the stage workspace), so every step streams from HBM",
+                   "l2": ("inputs+outputs+workspace per step are %.0f MB > 126 MB L2, so every step streams from HBM" % (N * (16.0 * nc + 32 + 60.0 * nc) / 1e6)
+                          if N * (16.0 * nc + 32 + 60.0 * nc) > 126e6 else
+                          "working set %.0f MB fits the 126 MB L2 (small-N sweep point; no flush between steps)" % (N * (16.0 * nc + 32 + 60.0 * nc) / 1e6)),
                    "stats_last_step": stats},
         "clocks": _parse_clocks(clk_path),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

@@ -144,6 +144,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
 #define PTF_SS_MINB 4
 #endif
 constexpr double LNW_ZERO = -1000.0;
+constexpr int HINT_SS_CAP = 30;
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
@@ -305,6 +306,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
 #pragma unroll
       for (int i = 0; i < NC; ++i) lnK[i] = w.lnK[(int64_t)i * N + n];
       double theta = -1.0e300, r_prev = -1.0;
+      const bool hinted = (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED);
       double Zx = w.Zxy[n], Zy = w.Zxy[N + n];   // roots of the stage that produced lnK (0: none)
       bool converged = false, failed = false, final_rr = false;
       int k = 0, status = 0;
@@ -326,6 +328,10 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         if (final_rr) { converged = true; break; }
         if (o.use_newton && k >= o.split_ss_iters && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
         if (k >= o.ss_cap) { status |= ST_SPLIT_CAP; break; }
+        // A skip-stability hint (C21) whose successive substitution has not brought theta into (0,1) after HINT_SS_CAP
+        // iterations is dropped here (-> cold re-flash in pass 1) instead of crawling towards the SS cap: next to the
+        // phase boundary such a mixture can take 1e5 iterations (40 ms for the whole call) to fail.
+        if (hinted && k >= HINT_SS_CAP) { failed = true; break; }
         {
           Eos e;
           double Sv[NC];

@@ -104,9 +104,13 @@ def test_parity_config5_warm_start(oracle_mod):
         # a failed skip-stability hint is dropped and reported (ST_WARM_RESTART), on both sides for the same mixtures
         # up to a handful of borderline cases; after the restart the answer is the cold one
         assert 0 < restarted.sum() < 0.03 * w.N
-        # (which near-boundary hints fail depends on the Newton path: the oracle searches eta as in B.4a, the CUDA split
-        # uses one modified-Cholesky factorisation per iteration; the answers after a restart are the cold ones either way)
-        assert np.sum(restarted != ((o_warm["status"] & 64) != 0)) <= 0.005 * w.N
+        # Which near-boundary hints fail depends on the path: the oracle searches eta as in B.4a and lets a hinted split
+        # crawl outside (0,1) up to the SS cap; the CUDA split uses one modified-Cholesky factorisation per iteration
+        # (C25) and drops a hint whose SS is still outside (0,1) after 30 iterations (C21).  So the CUDA path restarts a
+        # few more mixtures; the answers after a restart are the cold ones either way (checked above and below).
+        o_restarted = (o_warm["status"] & 64) != 0
+        assert np.sum(o_restarted & ~restarted) <= 0.005 * w.N
+        assert np.sum(restarted & ~o_restarted) <= 0.015 * w.N
         assert np.array_equal(g_warm["phase"][restarted], g_cold["phase"][restarted])
         print("config5 engine", engine, "mean iters (two-phase): warm %.2f cold %.2f; cold stability iters %.2f" %
               (g_warm["iters"][two].mean(), g_cold["iters"][two].mean(), g_cold["stab_iters"][two].mean()), rep_w, rep_c)
