@@ -72,7 +72,11 @@ ptflash_handle_t ptflash_create(int nc, const double* Tc, const double* Pc, cons
  *   stream                            cudaStream_t (NULL = legacy default stream)
  * Asynchronous: enqueues work on `stream` and returns; outputs are valid once the stream reaches that point.
  * The caller owns every buffer; inputs and outputs must not alias.  The handle owns a workspace that
- * grows on first use (a growth synchronises the stream).  N == 0 is a no-op.  Returns PTFLASH_OK / EINVAL / ECUDA. */
+ * grows on first use (a growth synchronises the stream) and a second, internal stream: after the stability stages the two
+ * parts of the phase split run concurrently, forked from and joined back into `stream` by events, so the ordering
+ * guarantees above hold for `stream` alone.  One call in flight per handle (use one handle per stream for concurrency).
+ * The call makes the handle's device current while it runs and restores the caller's.  N == 0 is a no-op.
+ * Returns PTFLASH_OK / EINVAL / ECUDA. */
 int ptflash_flash(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T,
                   double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
                   void* stream);

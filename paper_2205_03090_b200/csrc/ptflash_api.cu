@@ -52,6 +52,17 @@ struct ptflash_handle_s {
 
 namespace {
 
+// Makes the handle's device current for the duration of a call and restores the caller's device afterwards
+// (a handle is bound to the device that was current in ptflash_create).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 ptf::Opt make_opt(const double* o) {
   ptf::Opt r;
   r.tol_ss = o[PTFLASH_OPT_TOL_SS];
@@ -190,6 +201,7 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
     set_err("ptflash_flash: null required pointer");
     return PTFLASH_EINVAL;
   }
+  DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
   const int engine = (int)h->opts[PTFLASH_OPT_ENGINE];
   ptf::launch_fn fn = pick_launcher(h->sys.nc, engine);
@@ -255,6 +267,7 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
   if (N < 0) { set_err("ptflash_flash_host: N < 0"); return PTFLASH_EINVAL; }
   if (N == 0) return PTFLASH_OK;
   if (!z || !P || !T || !out_beta || !out_x || !out_y || !out_phase) { set_err("ptflash_flash_host: null required pointer"); return PTFLASH_EINVAL; }
+  DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
   const int nc = h->sys.nc;
   const size_t nd = (size_t)N;

@@ -391,7 +391,12 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   // persistent refill kernels: as many CTAs per SM as registers and shared memory allow (queried once per instantiation)
   const size_t stab_bytes = (size_t)stabn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
   const size_t split_bytes = (size_t)splitn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
-  static int stab_cta = 0, split_cta = 0;
+  // (per device: the shared-memory attribute of a kernel is device state, and a process may hold handles on several GPUs)
+  static int stab_cta_dev[64] = {0}, split_cta_dev[64] = {0};
+  int dev_id = 0;
+  cudaGetDevice(&dev_id);
+  int& stab_cta = stab_cta_dev[dev_id & 63];
+  int& split_cta = split_cta_dev[dev_id & 63];
   if (stab_cta == 0) {
     cudaFuncSetAttribute(k3_stab_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stab_bytes);
     cudaFuncSetAttribute(k3_split_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)split_bytes);
