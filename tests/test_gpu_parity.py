@@ -258,6 +258,45 @@ def test_two_streams_equal_one_stream(oracle_mod):
         assert np.array_equal(g_fork[k], g_one[k]), k
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("N", [1, 31, 33, 1025, 4133])
+def test_outputs_stay_inside_their_buffers(N):
+    """Guard words around every output array must survive a call (compute-sanitizer is not available on the GPU pool, so
+    this is the bounds check for the stores of the user-visible arrays; cold call and warm-start call with flags)."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    dev = torch.device("cuda:0")
+    w = W.config3(N)
+    nc = w.system.nc
+    z, P, T = (torch.from_numpy(a).to(dev) for a in (w.z, w.P, w.T))
+    PAD, S64, S32 = 64, -7.25e300, -123456789
+
+    def guarded(n_elem, dtype, sentinel):
+        buf = torch.full((n_elem + 2 * PAD,), sentinel, dtype=dtype, device=dev)
+        return buf, buf[PAD:PAD + n_elem]
+
+    f = B.PTFlash.from_system(w.system)
+    lnK_prev = None
+    for warm in (False, True):
+        bufs = {k: guarded(nc * N, torch.float64, S64) for k in ("x", "y", "lnK")}
+        bufs.update({k: guarded(N, torch.float64, S64) for k in ("beta", "tpd")})
+        bufs.update({k: guarded(N, torch.int32, S32) for k in ("phase", "iters", "status", "stab")})
+        kw = {}
+        if warm:
+            kw = dict(lnK0=lnK_prev, flags=torch.ones(N, dtype=torch.uint8, device=dev))
+        B.ptflash_flash_ex(f.h, N, z, P, T, bufs["beta"][1], bufs["x"][1], bufs["y"][1], bufs["phase"][1], bufs["iters"][1],
+                           out_tpd_min=bufs["tpd"][1], out_lnK=bufs["lnK"][1], out_status=bufs["status"][1],
+                           out_stab_iters=bufs["stab"][1], **kw)
+        torch.cuda.synchronize()
+        for k, (buf, view) in bufs.items():
+            sent = S64 if buf.dtype == torch.float64 else S32
+            assert bool((buf[:PAD] == sent).all()) and bool((buf[-PAD:] == sent).all()), (k, warm)
+        assert bool(((bufs["phase"][1] == 1) | (bufs["phase"][1] == 2)).all())     # every element was written
+        assert bool((bufs["beta"][1] != S64).all()) and bool((bufs["x"][1] != S64).all()) and bool((bufs["y"][1] != S64).all())
+        lnK_prev = bufs["lnK"][1].clone()
+    f.close()
+
+
 def test_full_size_sampled_parity_and_invariants(oracle_mod):
     """BASELINE size (config 3, N = 1,000,000, the launch configuration bench.py times): invariants on every mixture,
     oracle parity on a seeded sample computed one by one (mixtures are independent)."""
