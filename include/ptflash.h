@@ -31,10 +31,11 @@ extern "C" {
 typedef struct ptflash_handle_s* ptflash_handle_t;
 
 #define PTFLASH_OK 0
-#define PTFLASH_EINVAL (-1) /* null handle / null required pointer / N < 0 / unknown option */
+#define PTFLASH_EINVAL (-1) /* null handle / null required pointer / N < 0 or > PTFLASH_MAX_N / unknown option or value out of range */
 #define PTFLASH_ECUDA (-2)  /* CUDA allocation, copy or launch failure; text in ptflash_last_error() */
 
 #define PTFLASH_MAX_NC 16
+#define PTFLASH_MAX_N 1073741823LL /* 2^30 - 1 mixtures per call (work queues hold 32-bit ids); larger N -> PTFLASH_EINVAL */
 
 /* out_phase values */
 #define PTFLASH_PHASE_INVALID (-1) /* non-finite input, P <= 0, T <= 0, z_i < 0 or |sum z - 1| > 1e-9: beta, x, y = NaN */
@@ -133,7 +134,12 @@ enum {
   PTFLASH_OPT_STAGE_PROFILE = 14,  /* [0] 1 = record a CUDA event between the stage kernels (engine 1), see ptflash_get_stage_ms */
   PTFLASH_OPT_TOL_NEWTON_STEP_STAB = 15, /* the same for the stability Newton, whose result enters only through tm (itself
                                             second order in the error of W) and the K seed [1e-6] */
-  PTFLASH_NUM_OPTS = 16
+  PTFLASH_OPT_HINT_SS_CAP = 16,    /* [30] a PTFLASH_FLAG_SKIP_STABILITY split whose successive substitution is still outside
+                                      0 < theta < 1 after this many iterations is dropped and the mixture re-flashed from
+                                      Wilson (PTFLASH_ST_WARM_RESTART; reading C21) */
+  PTFLASH_OPT_SPLIT_TRIVIAL_TOL = 17, /* [1e-5] the phase split has collapsed into the trivial solution x = y when max_i |ln K_i| < tol
+                                      (-> PTFLASH_ST_SPLIT_FAILED, or a warm restart); reading C22 */
+  PTFLASH_NUM_OPTS = 18
 };
 int ptflash_set_option(ptflash_handle_t h, int key, double value);
 int ptflash_get_option(ptflash_handle_t h, int key, double* value);
@@ -163,6 +169,18 @@ int ptflash_get_stage_ms(ptflash_handle_t h, float* ms, int cap);
 /* FP64 roofline probe: runs an unrolled independent-DFMA kernel on every SM for `iters` iterations and returns
  * the achieved FP64 FLOP/s (used by bench.py as the measured denominator of the ALU roofline). */
 int ptflash_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, void* stream);
+
+/* Diagnostic: evaluates ONE of the library's own fp64 math routines (csrc/ptflash_math.cuh: the branch-free exp / log /
+ * reciprocal sequences every kernel uses instead of the CUDA math library) element-wise, y[i] = fn(x[i]), on DEVICE arrays
+ * x, y [n], asynchronously on `stream`.  It exists so that the accuracy claims of those routines (<= 2 ulp on their stated
+ * ranges, the clamps at their edges) can be tested directly against libm instead of only through the flash results.
+ *   fn  0 exp_fast   (x <= 709; clamped below at -708)      1 exp_tab  (x <= 709; clamped below at -700)
+ *       2 log_fast   (normal x > 0)                           3 log1p_fast (0 <= x < 1)
+ *       4 rcp_fast   (normal x, 1/x normal)                   5 rsqrt_fast (normal x > 0)
+ *       6 sqrt_fast  (x >= 0)                                 7 div_fast(1, x)          8 rcp_nr1 (~2^-40 relative)
+ * Returns PTFLASH_OK / EINVAL / ECUDA. */
+#define PTFLASH_NUM_MATH_FN 9
+int ptflash_math_probe(int fn, int64_t n, const double* x, double* y, void* stream);
 
 /* Text of the last error on the calling thread ("" if none). */
 const char* ptflash_last_error(void);

@@ -19,7 +19,7 @@ _LIBS = {"double": _HERE / "libptflash_oracle.so", "long double": _HERE / "libpt
 
 OPT_NAMES = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band",
              "probe_iters", "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters",
-             "use_newton", "ss_cap"]
+             "use_newton", "ss_cap", "hint_ss_cap", "eta_growth", "eta_ratio", "split_trivial_tol"]
 
 
 def build(real: str = "double", force: bool = False) -> Path:
@@ -159,7 +159,7 @@ class Oracle:
             phase=np.empty(N, dtype=np.int32), iters=np.empty(N, dtype=np.int32),
             tpd_min=np.empty(N), lnK=np.empty((nc, N)), status=np.empty(N, dtype=np.int32),
             stab_iters=np.empty(N, dtype=np.int32), probe_case=np.empty(N, dtype=np.int32),
-            diag=np.empty((3, N)),
+            diag=np.empty((3, N)), stage=np.empty((9, N), dtype=np.int32),
         )
         l0 = _f64(lnK0) if lnK0 is not None else None
         fl = np.ascontiguousarray(flags, dtype=np.uint8) if flags is not None else None
@@ -169,7 +169,7 @@ class Oracle:
             fl.ctypes.data_as(C.POINTER(C.c_uint8)) if fl is not None else None, _dp(self._opts(opts)),
             _dp(out["beta"]), _dp(out["x"]), _dp(out["y"]), ip(out["phase"]), ip(out["iters"]),
             _dp(out["tpd_min"]), _dp(out["lnK"]), ip(out["status"]), ip(out["stab_iters"]),
-            ip(out["probe_case"]), _dp(out["diag"]), C.c_int(nthreads))
+            ip(out["probe_case"]), _dp(out["diag"]), ip(out["stage"]), C.c_int(nthreads))
         out["threads"] = used
         return out
 

@@ -25,22 +25,6 @@
 #include <cstring>
 #include <limits>
 #include <algorithm>
-#ifdef ORACLE_TRACE
-#include <cstdio>
-#ifdef ORACLE_TRACE_PRINT
-#define TRACE(...) std::fprintf(stderr, __VA_ARGS__)
-#else
-#define TRACE(...) ((void)0)
-#endif
-#include <atomic>
-static std::atomic<long long> g_trace_attempts[64], g_trace_calls;
-#define TRACE_ATTEMPTS(n) do { g_trace_calls++; g_trace_attempts[(n) < 63 ? (n) : 63]++; } while (0)
-extern "C" void orc_trace_dump() { std::fprintf(stderr, "tr_subproblem calls %lld; attempts histogram:", (long long)g_trace_calls.load()); for (int i = 0; i < 64; ++i) if (g_trace_attempts[i].load()) std::fprintf(stderr, " %d:%lld", i, (long long)g_trace_attempts[i].load()); std::fprintf(stderr, "\n"); }
-#else
-#define TRACE(...) ((void)0)
-#define TRACE_ATTEMPTS(n) ((void)0)
-#endif
-
 #ifndef ORACLE_REAL
 #define ORACLE_REAL double
 #endif
@@ -73,12 +57,21 @@ struct Opts {
   double split_tr_iters;  // [10] 60
   double use_newton;      // [11] 1; 0 = pure successive substitution everywhere (used by pins)
   double ss_cap;          // [12] cap on SS iterations when use_newton == 0                               100000
+  double hint_ss_cap;     // [13] a skip-stability hint whose split SS is still outside 0 < theta < 1 after this
+                          //      many iterations is dropped (reading C21)                  30
+  double eta_growth;      // [14] restricted step (C11): geometric growth factor of eta                            8
+  double eta_ratio;       // [15] restricted step (C11): the bisection of eta stops at this bracket ratio          1.5
+                          //      ([14], [15] exist so that tests/oracle_path_sensitivity.py can perturb the schedule)
+  double split_trivial_tol; // [16] the split has collapsed into the trivial solution x = y when max|ln K_i| < tol     1e-5
+                          //      (reading C22: a Newton iteration sliding into x = y "converges" -- its gradient vanishes
+                          //      with |ln K| -- at |ln K| ~ 1e-8, theta ~ 1e-9; genuine solutions of the workloads have
+                          //      max|ln K| > 3e-2)
 };
 static Opts default_opts() {
-  Opts o = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000};
+  Opts o = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 30, 8, 1.5, 1e-5};
   return o;
 }
-#define NOPTS 13
+#define NOPTS 17
 static Opts opts_from(const double* p) {
   Opts o = default_opts();
   if (p) std::memcpy(&o, p, sizeof(double) * NOPTS);
@@ -86,7 +79,7 @@ static Opts opts_from(const double* p) {
 }
 
 // status bits (same meaning as include/ptflash.h but defined independently)
-enum { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_RR = 16, ST_WARM_RESTART = 64 };
+enum { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_LNK0_REJECTED = 32, ST_WARM_RESTART = 64 };
 
 // ------------------------------------------------------------------------------------------------
 // O1 Setup: dimensionless SRK groups.  PAPER.md:412-434 (A.2a-g, A.3).  R never appears:
@@ -377,13 +370,12 @@ static bool chol_solve(int n, real (*H)[MAXC], const real* rhs, real* sol) {
 // inside the trust region and inside the box.  Returns false if no admissible eta was found.
 // ------------------------------------------------------------------------------------------------
 static bool tr_subproblem(int n, real (*H)[MAXC], const real* g, const real* D, real Delta, real eta0,
-                          const real* v, const real* lo, const real* hi, real* s, real* eta_out, real* snorm_out) {
+                          const real* v, const real* lo, const real* hi, real* s, real* eta_out, real* snorm_out,
+                          real growth = (real)8, real ratio_stop = (real)1.5) {
   real Hh[MAXC][MAXC], neg[MAXC], st[MAXC];
   for (int a = 0; a < n; ++a) neg[a] = -g[a];
   real sn = 0;
-  int nattempt = 0;
   auto attempt = [&](real eta) -> bool {
-    ++nattempt;
     for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) Hh[a][b] = H[a][b] + ((a == b) ? eta * D[a] : (real)0);
     if (!chol_solve(n, Hh, neg, st)) return false;
     sn = 0;
@@ -396,22 +388,20 @@ static bool tr_subproblem(int n, real (*H)[MAXC], const real* g, const real* D, 
     return sn <= Delta;
   };
   auto keep = [&](real eta) { for (int a = 0; a < n; ++a) s[a] = st[a]; *eta_out = eta; *snorm_out = sn; };
-  if (attempt((real)0)) { keep((real)0); TRACE_ATTEMPTS(nattempt); return true; }
+  if (attempt((real)0)) { keep((real)0); return true; }
   real eta_lo = 0, eta_hi = 0, eta = eta0;
   bool found = false;
   for (int k = 0; k < 60; ++k) {
     if (attempt(eta)) { eta_hi = eta; keep(eta); found = true; break; }
-    eta_lo = eta; eta = eta * (real)8;
+    eta_lo = eta; eta = eta * growth;
   }
   if (!found) return false;
   for (int k = 0; k < 12; ++k) {
     if (*snorm_out >= Delta / (real)2) break;
-    if (eta_lo > (real)0 && eta_hi / eta_lo < (real)1.5) break;
-    real mid = (eta_lo > (real)0) ? r_sqrt(eta_lo * eta_hi) : eta_hi / (real)8;
+    if (eta_lo > (real)0 && eta_hi / eta_lo < ratio_stop) break;
+    real mid = (eta_lo > (real)0) ? r_sqrt(eta_lo * eta_hi) : eta_hi / growth;
     if (attempt(mid)) { eta_hi = mid; keep(mid); } else eta_lo = mid;
   }
-  TRACE_ATTEMPTS(nattempt);
-  (void)nattempt;
   return true;
 }
 
@@ -425,14 +415,14 @@ static bool tr_subproblem(int n, real (*H)[MAXC], const real* g, const real* D, 
 //   at a stationary point tm = 1 - sumW and tpd = -ln sumW (C2).
 // Outputs: lnW, tm, tpd, trivial flag (C7), iterations (ss, tr), cap flag.
 // ------------------------------------------------------------------------------------------------
-struct StabOut { real lnW[MAXC]; real tm, tpd; int trivial, ss_iters, tr_iters, capped; };
+struct StabOut { real lnW[MAXC]; real tm, tpd; int trivial, ss_iters, tr_iters, capped, entered_newton; };
 
 static void stability_trial(const Setup& s, const real* z, const real* lnz, const real* d, const real* lnK, int side,
                             const Opts& o, StabOut& out) {
   const int nc = s.nc;
   real lnW[MAXC], W[MAXC], w[MAXC], lp[MAXC], r[MAXC];
   for (int i = 0; i < nc; ++i) lnW[i] = (z[i] > (real)0) ? lnz[i] + (real)side * lnK[i] : (real)0;
-  out.ss_iters = out.tr_iters = 0; out.capped = 0;
+  out.ss_iters = out.tr_iters = 0; out.capped = 0; out.entered_newton = 0;
   bool converged = false;
   real sumW = 0, rmax = 0;
   auto eval = [&](real (*M)[MAXC]) {
@@ -463,6 +453,7 @@ static void stability_trial(const Setup& s, const real* z, const real* lnz, cons
     eval(nullptr); tm = tm_full(); out.capped = 1;
   } else {
     // ---- trust-region Newton, B.1-B.3 ----
+    out.entered_newton = 1;
     // active components (z_i > 0)
     int idx[MAXC], na = 0;
     for (int i = 0; i < nc; ++i) if (z[i] > (real)0) idx[na++] = i;
@@ -490,7 +481,7 @@ static void stability_trial(const Setup& s, const real* z, const real* lnz, cons
       }
       real eta = 0, snorm = 0, ones[MAXC], lo[MAXC], hi[MAXC];
       for (int a = 0; a < na; ++a) { ones[a] = 1; lo[a] = 0; hi[a] = std::numeric_limits<real>::infinity(); }
-      bool ok = tr_subproblem(na, H, g, ones, Delta, (real)1e-3, beta, lo, hi, sstep, &eta, &snorm);
+      bool ok = tr_subproblem(na, H, g, ones, Delta, (real)1e-3, beta, lo, hi, sstep, &eta, &snorm, (real)o.eta_growth, (real)o.eta_ratio);
       if (!ok) { out.capped = 1; break; }
       real smax = 0;
       for (int a = 0; a < na; ++a) smax = std::max(smax, r_abs(sstep[a]));
@@ -557,7 +548,7 @@ static void stability_trial(const Setup& s, const real* z, const real* lnz, cons
 //   matrix D(z/(xy)) (B.4a) and the Delta_max rule (B.3).
 // Outputs: theta, x, y, lnK, iterations, status bits.  two_phase = converged with 0 < theta < 1.
 // ------------------------------------------------------------------------------------------------
-struct SplitOut { real theta, x[MAXC], y[MAXC], lnK[MAXC]; int two_phase, ss_iters, tr_iters, status; real rate, dc; };
+struct SplitOut { real theta, x[MAXC], y[MAXC], lnK[MAXC]; int two_phase, ss_iters, tr_iters, status, entered_newton; real rate, dc; };
 
 static real gibbs_two_phase(int nc, const real* nL, const real* nV, const real* x, const real* y, const real* lpx, const real* lpy) {
   real G = 0;                                                                                // eq. 8
@@ -568,11 +559,15 @@ static real gibbs_two_phase(int nc, const real* nL, const real* nV, const real* 
   return G;
 }
 
-static void phase_split(const Setup& s, const real* z, const real* lnK_in, const Opts& o, SplitOut& out) {
+// `hinted`: the split was entered through the caller's skip-stability hint (reading C21): a hinted split whose successive
+// substitution is still outside 0 < theta < 1 after hint_ss_cap iterations is declared failed at once (the caller's
+// estimate points at the wrong side of the phase boundary -- the failure mode of PAPER.md:363 -- and SS would crawl
+// towards the trivial solution for up to ss_cap iterations); flash_one then drops the hint and flashes from Wilson.
+static void phase_split(const Setup& s, const real* z, const real* lnK_in, const Opts& o, bool hinted, SplitOut& out) {
   const int nc = s.nc;
   real lnK[MAXC], K[MAXC], x[MAXC], y[MAXC], lpx[MAXC], lpy[MAXC];
   for (int i = 0; i < nc; ++i) lnK[i] = lnK_in[i];
-  out.ss_iters = out.tr_iters = 0; out.status = 0; out.two_phase = 0; out.rate = 0; out.theta = 0;
+  out.ss_iters = out.tr_iters = 0; out.status = 0; out.two_phase = 0; out.rate = 0; out.theta = 0; out.entered_newton = 0;
   real theta = 0, r_prev = -1;
   bool converged = false, failed = false;
   const bool newton = (o.use_newton != 0);
@@ -584,12 +579,13 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
     // trivial collapse
     real mk = 0;
     for (int i = 0; i < nc; ++i) if (z[i] > (real)0) mk = std::max(mk, r_abs(lnK[i]));
-    if (mk < (real)1e-9) { failed = true; break; }
+    if (mk < (real)o.split_trivial_tol) { failed = true; break; }
     for (int i = 0; i < nc; ++i) K[i] = r_exp(lnK[i]);
     if (!rachford_rice(nc, K, z, &theta)) { failed = true; break; }
     phases_from_theta(nc, K, z, theta, x, y);
     if (newton && k >= ss_switch && theta > (real)0 && theta < (real)1) { go_newton = true; break; }
     if (k >= ss_cap) { out.status |= ST_SPLIT_CAP; break; }
+    if (hinted && k >= (int)o.hint_ss_cap && !(theta > (real)0 && theta < (real)1)) { failed = true; break; }   // C21
     lnphi(s, x, lpx, nullptr, nullptr);
     lnphi(s, y, lpy, nullptr, nullptr);
     real rk = 0;
@@ -615,6 +611,7 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
 
   if (go_newton) {
     // ---- trust-region Newton on G in n^V, B.4-B.5 ----
+    out.entered_newton = 1;
     int idx[MAXC], na = 0;
     for (int i = 0; i < nc; ++i) if (z[i] > (real)0) idx[na++] = i;
     real nV[MAXC], nL[MAXC], Mx[MAXC][MAXC], My[MAXC][MAXC], gt[MAXC];
@@ -636,8 +633,12 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
     real Delta = (real)0.25;   // n^V lives in the box (0, z), |n^V| < 1; Delta is capped at 1 (C11)
     const int kmax = (int)o.split_tr_iters;
     for (int it = 0; it < kmax; ++it) {
-      if (gmax < (real)o.tol_newton_g) { converged = true; break; }
-      out.tr_iters++;
+      // Reading C8: the gradient test does not end the iteration by itself.  Near a critical point (d_c -> 0, eq. 14
+      // PAPER.md:318) and next to the phase boundary the Hessian is nearly singular, so a gradient below 1e-12 does not
+      // bound the error of n^V (error ~ gradient / smallest eigenvalue); the Newton step is the error estimate.  A
+      // gradient below the target therefore triggers ONE last full Newton step ("polish"), applied if it is admissible.
+      const bool last = gmax < (real)o.tol_newton_g;
+      if (!last) out.tr_iters++;
       real g[MAXC], H[MAXC][MAXC], D[MAXC], sstep[MAXC];
       const real tt = theta * ((real)1 - theta);
       for (int a = 0; a < na; ++a) {
@@ -651,11 +652,12 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
       }
       real eta = 0, snorm = 0, va[MAXC], lo[MAXC], hi[MAXC];
       for (int a = 0; a < na; ++a) { va[a] = nV[idx[a]]; lo[a] = 0; hi[a] = z[idx[a]]; }
-      bool ok = tr_subproblem(na, H, g, D, Delta, (real)1e-3 / tt, va, lo, hi, sstep, &eta, &snorm);   // B.4a
-      if (!ok) { out.status |= ST_SPLIT_CAP; break; }
+      bool ok = tr_subproblem(na, H, g, D, Delta, (real)1e-3 / tt, va, lo, hi, sstep, &eta, &snorm, (real)o.eta_growth, (real)o.eta_ratio);   // B.4a
+      if (!ok) { if (last) converged = true; else out.status |= ST_SPLIT_CAP; break; }
       real smax = 0;
       for (int a = 0; a < na; ++a) smax = std::max(smax, r_abs(sstep[a]));
-      if (eta == (real)0 && smax < (real)o.tol_newton_step) {
+      if (last && eta != (real)0) { converged = true; break; }   // no admissible full step: keep the evaluated point
+      if (eta == (real)0 && (last || smax < (real)o.tol_newton_step)) {
         for (int a = 0; a < na; ++a) nV[idx[a]] += sstep[a];
         theta = 0; for (int i = 0; i < nc; ++i) theta += nV[i];
         for (int i = 0; i < nc; ++i) { nL[i] = z[i] - nV[i]; y[i] = nV[i] / theta; x[i] = nL[i] / ((real)1 - theta); }
@@ -673,9 +675,9 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
       for (int a = 0; a < na; ++a) nV[idx[a]] += sstep[a];
       eval();
       real act = G - G_old;
-      bool accept = (act < (real)0) || (gmax < gmax_old);
-      TRACE("split tr it=%d eta=%.3e snorm=%.3e Delta=%.3e pred=%.3e act=%.3e gmax %.3e -> %.3e theta=%.6f %s\n", it, (double)eta,
-            (double)snorm, (double)Delta, (double)pred, (double)act, (double)gmax_old, (double)gmax, (double)theta, accept ? "acc" : "REJ");
+      // accept if G fell; a smaller gradient is accepted instead only where the change of G is below its rounding
+      // resolution (next to the solution), so that the iteration is a descent method on G everywhere else (reading C11)
+      bool accept = (act < (real)0) || (gmax < gmax_old && act <= (real)1e-12 * r_abs(G_old));
       if (accept) {
         real ratio = (pred != (real)0) ? r_abs(act / pred) : (real)1;
         if (r_abs(pred) > (real)1e-13) {
@@ -694,7 +696,7 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
     // the Newton iteration can also slide into the trivial solution x = y (G is flat there): same test as in the SS loop
     real mkn = 0;
     for (int i = 0; i < nc; ++i) if (z[i] > (real)0) mkn = std::max(mkn, r_abs(lnK[i]));
-    if (mkn < (real)1e-9) failed = true;
+    if (mkn < (real)o.split_trivial_tol) failed = true;
   }
 
   out.theta = theta;
@@ -712,6 +714,8 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
 struct FlashOut {
   int phase, iters, status, stab_iters, probe_case;
   real beta, x[MAXC], y[MAXC], lnK[MAXC], tpd_min, Zfeed, dc, rate;
+  // per-stage counts (the columns of the paper's profiler, Table 4), summed over a warm restart
+  int stab_ss[2], stab_tr[2], stab_newton_trials, split_ss, split_tr, split_entered, split_newton;
 };
 
 static void flash_one(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij,
@@ -720,6 +724,8 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
   const real nan = std::numeric_limits<real>::quiet_NaN();
   out.phase = -1; out.iters = 0; out.status = 0; out.stab_iters = 0; out.probe_case = 0;
   out.beta = nan; out.tpd_min = nan; out.Zfeed = nan; out.dc = 0; out.rate = 0;
+  out.stab_ss[0] = out.stab_ss[1] = out.stab_tr[0] = out.stab_tr[1] = 0;
+  out.stab_newton_trials = out.split_ss = out.split_tr = out.split_entered = out.split_newton = 0;
   for (int i = 0; i < nc; ++i) { out.x[i] = nan; out.y[i] = nan; out.lnK[i] = nan; }
   // O0 validate
   bool ok = std::isfinite((double)P) && std::isfinite((double)T) && P > (real)0 && T > (real)0;
@@ -746,6 +752,7 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
   if (lnK0 && (flags & 3)) {
     have0 = true;
     for (int i = 0; i < nc; ++i) if (!std::isfinite((double)lnK0[i]) || r_abs(lnK0[i]) > (real)700) have0 = false;
+    if (!have0) out.status |= ST_LNK0_REJECTED;   // overflowing / non-finite estimates are ignored and reported
   }
   real lnKs[MAXC];
   for (int i = 0; i < nc; ++i) lnKs[i] = have0 ? lnK0[i] : lnKw[i];
@@ -785,6 +792,8 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
       stability_trial(s, z, lnz, d, lnKs, +1, o, sv);
       stability_trial(s, z, lnz, d, lnKs, -1, o, sl);
       out.stab_iters = sv.ss_iters + sv.tr_iters + sl.ss_iters + sl.tr_iters;
+      out.stab_ss[0] = sv.ss_iters; out.stab_ss[1] = sl.ss_iters; out.stab_tr[0] = sv.tr_iters; out.stab_tr[1] = sl.tr_iters;
+      out.stab_newton_trials = (sv.entered_newton ? 1 : 0) + (sl.entered_newton ? 1 : 0);
       if (sv.capped || sl.capped) out.status |= ST_STAB_CAP;
       // O7 label
       tpd_min = 0;
@@ -807,8 +816,9 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
   bool two = false;
   if (unstable) {
     SplitOut sp;
-    phase_split(s, z, lnK, o, sp);
+    phase_split(s, z, lnK, o, skip_stab, sp);
     out.iters += sp.ss_iters + sp.tr_iters;
+    out.split_ss = sp.ss_iters; out.split_tr = sp.tr_iters; out.split_entered = 1; out.split_newton = sp.entered_newton;
     out.status |= sp.status;
     out.dc = sp.dc; out.rate = sp.rate;
     if (sp.two_phase) {
@@ -835,7 +845,8 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
     FlashOut cold;
     flash_one(nc, Tc, Pc, omega, kij, P, T, z_in, nullptr, 0, o, cold);
     cold.iters += out.iters;
-    cold.status |= ST_WARM_RESTART;
+    cold.status |= ST_WARM_RESTART | (out.status & ST_LNK0_REJECTED);
+    cold.split_ss += out.split_ss; cold.split_tr += out.split_tr; cold.split_entered += 1; cold.split_newton += out.split_newton;
     out = cold;
     return;
   }
@@ -941,7 +952,7 @@ void orc_phase_split(int nc, const double* Tc, const double* Pc, const double* o
   Setup s; setup(nc, Tc, Pc, omega, kij, (real)P, (real)T, s);
   real zz[MAXC], lk[MAXC];
   for (int i = 0; i < nc; ++i) { zz[i] = (real)z[i]; lk[i] = (real)lnK[i]; }
-  SplitOut sp; phase_split(s, zz, lk, o, sp);
+  SplitOut sp; phase_split(s, zz, lk, o, false, sp);
   for (int i = 0; i < nc; ++i) { x[i] = (double)sp.x[i]; y[i] = (double)sp.y[i]; lnK_out[i] = (double)sp.lnK[i]; }
   res[0] = (double)sp.theta; res[1] = sp.two_phase; res[2] = sp.ss_iters; res[3] = sp.tr_iters; res[4] = sp.status;
   res[5] = (double)sp.rate; res[6] = (double)sp.dc;
@@ -949,14 +960,17 @@ void orc_phase_split(int nc, const double* Tc, const double* Pc, const double* o
 
 // Batched flash (the oracle of ptflash_flash / ptflash_flash_ex).  lnK0 [nc][N] and flags [N] may be NULL.
 // Optional outputs (may be NULL): tpd_min [N], lnK [nc][N], status [N], stab_iters [N], probe_case [N],
-// diag [3][N] = {Z_feed, d_c, last SS rate}.  nthreads <= 1 -> serial; otherwise OpenMP over mixtures.
+// diag [3][N] = {Z_feed, d_c, last SS rate}; stage [9][N] int32 = {stability SS iterations vapour-like, liquid-like,
+// trust-region iterations vapour-like, liquid-like, trials that entered the Newton stage, split SS iterations, split
+// trust-region iterations, splits entered, splits that entered the Newton stage}.
+// nthreads <= 1 -> serial; otherwise OpenMP over mixtures.
 // Returns the number of threads actually used.
 int orc_flash_batch(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij,
                     int64_t N, const double* z, const double* P, const double* T,
                     const double* lnK0, const uint8_t* flags, const double* opts,
                     double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
                     double* out_tpd_min, double* out_lnK, int32_t* out_status, int32_t* out_stab_iters,
-                    int32_t* out_probe_case, double* out_diag, int nthreads) {
+                    int32_t* out_probe_case, double* out_diag, int32_t* out_stage, int nthreads) {
   Opts o = opts_from(opts);
   int used = 1;
 #ifdef _OPENMP
@@ -979,6 +993,11 @@ int orc_flash_batch(int nc, const double* Tc, const double* Pc, const double* om
     if (out_stab_iters) out_stab_iters[n] = fo.stab_iters;
     if (out_probe_case) out_probe_case[n] = fo.probe_case;
     if (out_diag) { out_diag[n] = (double)fo.Zfeed; out_diag[N + n] = (double)fo.dc; out_diag[2 * N + n] = (double)fo.rate; }
+    if (out_stage) {
+      const int v[9] = {fo.stab_ss[0], fo.stab_ss[1], fo.stab_tr[0], fo.stab_tr[1], fo.stab_newton_trials, fo.split_ss, fo.split_tr,
+                        fo.split_entered, fo.split_newton};
+      for (int k = 0; k < 9; ++k) out_stage[(int64_t)k * N + n] = v[k];
+    }
   }
   return used;
 }

@@ -17,10 +17,10 @@ PTFLASH_OK, PTFLASH_EINVAL, PTFLASH_ECUDA = 0, -1, -2
 ST_STAB_CAP, ST_SPLIT_CAP, ST_BAND, ST_SPLIT_FAILED, ST_LNK0_REJECTED = 1, 2, 4, 8, 32
 FLAG_SKIP_STABILITY, FLAG_USE_LNK0 = 1, 2
 OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band", "probe_iters",
-           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab"]
+           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol"]
 EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
            "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_get_stage_ms", "ptflash_fp64_peak",
-           "ptflash_last_error", "ptflash_version"]
+           "ptflash_last_error", "ptflash_version", "ptflash_math_probe"]
 
 
 class PTFlashError(RuntimeError):
@@ -73,6 +73,8 @@ def load_library():
     L.ptflash_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
     L.ptflash_fp64_peak.restype = C.c_int
     L.ptflash_fp64_peak.argtypes = [C.c_int, dp, dp, vp]
+    L.ptflash_math_probe.restype = C.c_int
+    L.ptflash_math_probe.argtypes = [C.c_int, i64, vp, vp, vp]
     L.ptflash_last_error.restype = C.c_char_p
     L.ptflash_version.restype = C.c_char_p
     _lib = L
@@ -178,6 +180,15 @@ def ptflash_fp64_peak(iters=4096, stream=None):
     f, ms = C.c_double(0), C.c_double(0)
     _check(load_library().ptflash_fp64_peak(int(iters), C.byref(f), C.byref(ms), _stream(stream)), "ptflash_fp64_peak")
     return f.value, ms.value
+
+
+MATH_FN = ["exp_fast", "exp_tab", "log_fast", "log1p_fast", "rcp_fast", "rsqrt_fast", "sqrt_fast", "div_fast_1", "rcp_nr1"]
+
+
+def ptflash_math_probe(fn, n, x, y, stream=None):
+    """y[i] = fn(x[i]) with one of the library's lean fp64 math routines (device arrays); fn: index or name in MATH_FN."""
+    k = MATH_FN.index(fn) if isinstance(fn, str) else int(fn)
+    _check(load_library().ptflash_math_probe(k, int(n), _ptr(x), _ptr(y), _stream(stream)), "ptflash_math_probe")
 
 
 def ptflash_version() -> str:

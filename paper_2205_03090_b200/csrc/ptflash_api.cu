@@ -20,7 +20,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 
-const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6};
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 30, 1e-5};
 
 }  // namespace
 
@@ -48,6 +48,7 @@ struct ptflash_handle_s {
   cudaStream_t aux_stream;
   cudaEvent_t ev_fork, ev_join;
   bool aux_made;
+  int cta_cache[4];   // resident CTAs per SM of the persistent kernels on this handle's device (0 = not queried yet)
 };
 
 namespace {
@@ -79,9 +80,12 @@ ptf::Opt make_opt(const double* o) {
   r.split_tr_iters = (int)o[PTFLASH_OPT_SPLIT_TR_ITERS];
   r.use_newton = (int)o[PTFLASH_OPT_USE_NEWTON];
   r.ss_cap = (int)o[PTFLASH_OPT_SS_CAP];
+  r.hint_ss_cap = (int)o[PTFLASH_OPT_HINT_SS_CAP];
+  r.split_trivial_tol = o[PTFLASH_OPT_SPLIT_TRIVIAL_TOL];
   r.prof_events = nullptr;
   r.prof_count = nullptr;
   r.aux_stream = r.ev_fork = r.ev_join = nullptr;
+  r.cta_cache = nullptr;
   return r;
 }
 
@@ -169,7 +173,7 @@ ptflash_handle_t ptflash_create(int nc, const double* Tc, const double* Pc, cons
 int ptflash_destroy(ptflash_handle_t h) {
   if (!h) return PTFLASH_OK;
   int rc = PTFLASH_OK;
-  cudaSetDevice(h->device);
+  DeviceGuard guard(h->device);
   if (h->used && !cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) rc = PTFLASH_ECUDA;
   if (h->ws) cudaFree(h->ws);
   if (h->stage) cudaFree(h->stage);
@@ -183,6 +187,21 @@ int ptflash_destroy(ptflash_handle_t h) {
 
 int ptflash_set_option(ptflash_handle_t h, int key, double value) {
   if (!h || key < 0 || key >= PTFLASH_NUM_OPTS || !std::isfinite(value)) { set_err("ptflash_set_option: bad handle/key/value"); return PTFLASH_EINVAL; }
+  bool ok = true;
+  switch (key) {
+    case PTFLASH_OPT_TOL_SS: case PTFLASH_OPT_TOL_NEWTON_G: case PTFLASH_OPT_TOL_NEWTON_STEP: case PTFLASH_OPT_TOL_NEWTON_STEP_STAB:
+    case PTFLASH_OPT_TRIVIAL_TOL: case PTFLASH_OPT_SPLIT_TRIVIAL_TOL:
+      ok = value > 0.0 && value < 1.0; break;                      // tolerances
+    case PTFLASH_OPT_PROBE_MARGIN: case PTFLASH_OPT_BAND:
+      ok = value >= 0.0 && value < 1.0; break;
+    case PTFLASH_OPT_PROBE_ITERS: case PTFLASH_OPT_STAB_SS_ITERS: case PTFLASH_OPT_STAB_TR_ITERS: case PTFLASH_OPT_SPLIT_SS_ITERS:
+    case PTFLASH_OPT_SPLIT_TR_ITERS: case PTFLASH_OPT_SS_CAP: case PTFLASH_OPT_HINT_SS_CAP:
+      ok = value >= 0.0 && value <= 1.0e9 && value == std::floor(value); break;   // iteration counts
+    case PTFLASH_OPT_USE_NEWTON: case PTFLASH_OPT_ENGINE: case PTFLASH_OPT_STAGE_PROFILE:
+      ok = value == 0.0 || value == 1.0; break;                   // switches
+    default: break;
+  }
+  if (!ok) { set_err("ptflash_set_option: value out of range for this option"); return PTFLASH_EINVAL; }
   h->opts[key] = value;
   return PTFLASH_OK;
 }
@@ -197,6 +216,8 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
   if (!h || !io) { set_err("ptflash_flash: null handle or io"); return PTFLASH_EINVAL; }
   if (io->N < 0) { set_err("ptflash_flash: N < 0"); return PTFLASH_EINVAL; }
   if (io->N == 0) return PTFLASH_OK;
+  // the stage queues hold mixture ids (and 2 n + start for the stability trials) as 32-bit integers
+  if (io->N > PTFLASH_MAX_N) { set_err("ptflash_flash: N exceeds PTFLASH_MAX_N (2^30 - 1); split the batch"); return PTFLASH_EINVAL; }
   if (!io->z || !io->P || !io->T || !io->out_beta || !io->out_x || !io->out_y || !io->out_phase) {
     set_err("ptflash_flash: null required pointer");
     return PTFLASH_EINVAL;
@@ -219,6 +240,7 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
     if (!ensure(&h->ws, &h->ws_bytes, need, st, "cudaMalloc(workspace)")) return PTFLASH_ECUDA;
   }
   ptf::Opt o = make_opt(h->opts);
+  o.cta_cache = h->cta_cache;
   h->n_events = 0;
   if ((int)h->opts[PTFLASH_OPT_STAGE_PROFILE] && engine) {
     if (!h->events_made) {
@@ -266,6 +288,7 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
   if (!h) { set_err("ptflash_flash_host: null handle"); return PTFLASH_EINVAL; }
   if (N < 0) { set_err("ptflash_flash_host: N < 0"); return PTFLASH_EINVAL; }
   if (N == 0) return PTFLASH_OK;
+  if (N > PTFLASH_MAX_N) { set_err("ptflash_flash_host: N exceeds PTFLASH_MAX_N (2^30 - 1); split the batch"); return PTFLASH_EINVAL; }
   if (!z || !P || !T || !out_beta || !out_x || !out_y || !out_phase) { set_err("ptflash_flash_host: null required pointer"); return PTFLASH_EINVAL; }
   DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
@@ -301,6 +324,7 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
   if (!h || !out) { set_err("ptflash_get_stats: null argument"); return PTFLASH_EINVAL; }
   std::memset(out, 0, sizeof(*out));
   if (!h->used) return PTFLASH_OK;
+  DeviceGuard guard(h->device);
   if (!cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
   const ptf::StageCounters& c = *h->counters_host;
   out->n_total = h->last_N;
@@ -322,6 +346,7 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
 int ptflash_get_stage_ms(ptflash_handle_t h, float* ms, int cap) {
   if (!h || !ms || cap < 0) { set_err("ptflash_get_stage_ms: bad argument"); return PTFLASH_EINVAL; }
   if (!h->used || h->n_events < 2) return 0;
+  DeviceGuard guard(h->device);
   if (!cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
   int n = 0;
   for (int i = 0; i + 1 < h->n_events && n < cap; ++i, ++n)
@@ -336,6 +361,13 @@ int ptflash_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, void* 
   if (ptf::run_fp64_peak(iters, &fl, &ms, (cudaStream_t)stream) != 0) { cuda_ok(cudaGetLastError(), "fp64 peak kernel"); return PTFLASH_ECUDA; }
   *flops_per_s = fl;
   if (elapsed_ms) *elapsed_ms = ms;
+  return PTFLASH_OK;
+}
+
+int ptflash_math_probe(int fn, int64_t n, const double* x, double* y, void* stream) {
+  g_err.clear();
+  if (fn < 0 || fn >= PTFLASH_NUM_MATH_FN || n < 0 || (n > 0 && (!x || !y))) { set_err("ptflash_math_probe: bad arguments"); return PTFLASH_EINVAL; }
+  if (ptf::run_math_probe(fn, n, x, y, (cudaStream_t)stream) != 0) { cuda_ok(cudaGetLastError(), "math probe kernel"); return PTFLASH_ECUDA; }
   return PTFLASH_OK;
 }
 

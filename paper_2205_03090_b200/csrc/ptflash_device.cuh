@@ -24,14 +24,17 @@ namespace ptf {
 // parameter blocks
 // ------------------------------------------------------------------------------------------------
 struct Opt {
-  double tol_ss, tol_newton_g, tol_newton_step, tol_newton_step_stab, probe_margin, trivial_tol, band;
-  int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap;
+  double tol_ss, tol_newton_g, tol_newton_step, tol_newton_step_stab, probe_margin, trivial_tol, band, split_trivial_tol;
+  int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap, hint_ss_cap;
   // host only: cudaEvent_t[PTF_MAX_STAGE_EVENTS] recorded between the stage kernels when stage profiling is on (else null)
   void* prof_events;
   int* prof_count;   // host only: number of events recorded by the last launch
   // host only: second stream of the handle and two events (fork / join) so that the phase split of the mixtures the probe
   // already found unstable runs concurrently with the stability analysis of the others (null: everything on one stream)
   void *aux_stream, *ev_fork, *ev_join;
+  // host only: per-handle cache of the resident-CTA counts of the persistent kernels (0 = not yet queried); a handle is
+  // bound to one device and one component system, so the occupancy query runs once per handle
+  int* cta_cache;
 };
 #define PTF_MAX_STAGE_EVENTS 24
 

@@ -6,17 +6,12 @@
 //   * Rachford-Rice (eq. 7) starts from the previous theta and stops after the first Newton step below 1e-8
 //     of the window (App. C: "When the Newton step size is smaller than 1.0e-8, the iteration stops";
 //     the step is applied, so the error is ~1e-16);
-//   * everything is __forceinline__ so per-mixture vectors stay in registers (no struct passing through local memory);
-//   * symmetric nc x nc systems live in registers as a packed lower triangle with compile-time indices.
+//   * everything is __forceinline__ so per-mixture vectors stay in registers (no struct passing through local memory).
 #pragma once
 #include "ptflash_device.cuh"
 #include "ptflash_math.cuh"
-#include <cstdio>
 
 namespace ptf {
-
-// packed lower-triangle index, i >= j
-__host__ __device__ constexpr int tri(int i, int j) { return i * (i + 1) / 2 + j; }
 
 // Newton polish of the two deflated roots (A.5), interleaved: a step is taken only if it lowers |f| (near a double root
 // the deflated value is already the best available), twice.
@@ -199,50 +194,6 @@ __device__ __forceinline__ void lnphi_pt(const Sys<NC>& S, const PT3<NC>& q, con
   }
 }
 
-// Out-of-line copy for kernels that evaluate two phases per trip (x and y): one body instead of two keeps the
-// loop inside the instruction cache; the five small arrays travel through (L1-resident) local memory.
-template <int NC, bool KIJ0>
-__device__ __noinline__ void lnphi_call(const Sys<NC>& S, const double (&sa)[NC], const double (&bi)[NC],
-                                        const double (&c)[NC], double (&lp)[NC], double (&Sv)[NC], Eos& e) {
-  lnphi_fast<NC, KIJ0>(S, sa, bi, c, lp, Sv, e);
-}
-
-// ------------------------------------------------------------------------------------------------
-// Coefficients of M_ij = n dlnphi_i/dn_j (unit total moles) in the form
-//   M_ij = e_i p_j + c_j - Dq_j u_i + 2q (S_i - A_ij),   e_i = B_i/B, u_i = 2 S_i - A e_i
-// so that a matrix entry costs four FMAs (derivation: DESIGN.md section 3; identical to dlnphi()).
-// ------------------------------------------------------------------------------------------------
-struct MCoef {
-  double invB, A, q2, zA2, zBB, zm1, qA, invZmB, B, cL1, cL2, q;
-};
-__device__ __forceinline__ MCoef mcoef(const Eos& e) {
-  MCoef m;
-  const double A = e.A, B = e.B, Z = e.Z;
-  const double FZ = fma(fma(3.0, Z, -2.0), Z, A - B - B * B);
-  const double iFZ = rcp_fast(FZ);
-  const double ZA = -(Z - B) * iFZ;
-  const double ZB = fma(1.0 + 2.0 * B, Z, A) * iFZ;
-  const double iZZB = rcp_fast(Z * (Z + B));
-  m.invB = rcp_fast(B);
-  m.A = A; m.B = B; m.q = e.q;
-  m.q2 = 2.0 * e.q;
-  m.zA2 = 2.0 * ZA;
-  m.zBB = ZB * B;
-  m.zm1 = Z - 1.0;
-  m.qA = e.q * A;
-  m.invZmB = rcp_fast(Z - B);
-  m.cL1 = (Z - ZB * B) * iZZB;   // DL_j / B = cL1 eps_j - cL2 sig_j
-  m.cL2 = 2.0 * ZA * iZZB;
-  return m;
-}
-// per-column scalars p_j, c_j, Dq_j from eps_j = e_j - 1 and sig_j = S_j - A
-__device__ __forceinline__ void mcol(const MCoef& m, double eps, double sig, double& p, double& c, double& Dq) {
-  const double DZ = fma(m.zA2, sig, m.zBB * eps);
-  p = fma(-eps, m.zm1, DZ) + fma(m.q2, sig, -m.qA * eps);
-  c = -(DZ - m.B * eps) * m.invZmB;
-  Dq = fma(m.cL1, eps, -m.cL2 * sig) - m.q * eps;
-}
-
 // ------------------------------------------------------------------------------------------------
 // Rachford-Rice with warm start (eq. 7, App. C).  theta on entry: previous solution (used if inside the sign
 // bracket).  Returns false when there is no window.  Produces normalised x, y.
@@ -280,9 +231,6 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
   const double width = dmin(ar - al, 1.0);
 
   const double scale = 1.0e-8 * width;
-#ifdef PTF_DEBUG_COUNT
-  int dbg_it = 0, dbg_bis = 0;
-#endif
 #pragma unroll 1
   for (int it = 0; it < 100; ++it) {
     if (!(hi > lo)) break;
@@ -299,29 +247,15 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
     const double h = u * w * f;
     const double dh = (w - u) * f + u * w * df;
     double tn = th - h * rcp_fast(dh);
-#ifdef PTF_DEBUG_COUNT
-    dbg_it = it + 1;
-#endif
     // Newton step below the tolerance: apply it and stop (quadratic convergence leaves an error ~ step^2).  th is an end
     // of the sign bracket here, so a converged tn can land ON or an ulp beyond that end; it is clamped, not bisected
     // (bisecting from a converged iterate cost ~25 extra iterations in 1 % of the calls, i.e. in every fourth warp).
     if (fabs(tn - th) <= scale) { th = dmin(dmax(tn, lo), hi); break; }
     const bool inside = (tn > lo && tn < hi);
     if (!inside) tn = 0.5 * (lo + hi);
-#ifdef PTF_DEBUG_COUNT
-    if (!inside) dbg_bis++;
-#endif
     if (fabs(tn - th) <= 2.3e-16 * fabs(tn)) { th = tn; break; }
     th = tn;
   }
-#ifdef PTF_DEBUG_COUNT
-  if (dbg_it >= 15 && atomicAdd(&g_dbg[63], 1ull) < 12) {
-    printf("RR slow: warm=%d its=%d bis=%d f0=%.3e f1=%.3e al=%.6e ar=%.6e th=%.17g lo=%.17g hi=%.17g theta_in=%.6e\n", (int)warm, dbg_it, dbg_bis, f0, f1, al, ar, th, lo, hi, theta);
-    for (int i = 0; i < NC; ++i) printf("   i=%d z=%.6e K=%.6e\n", i, z[i], K[i]);
-  }
-  PTF_DBG((warm ? 32 : 16) + (dbg_it < 15 ? dbg_it : 15), 1);
-  PTF_DBG(warm ? 49 : 48, dbg_bis);
-#endif
   theta = th;
   double sx = 0.0, sy = 0.0;
 #pragma unroll
@@ -336,56 +270,6 @@ __device__ __forceinline__ bool rr_fast(const double (&K)[NC], const double (&z)
 #pragma unroll
   for (int i = 0; i < NC; ++i) { x[i] *= isx; y[i] *= isy; }
   return true;
-}
-
-// ------------------------------------------------------------------------------------------------
-// In-register Cholesky of a packed symmetric matrix (lower triangle, compile-time indices) and solve
-// (L L^T) s = -g.  On exit Lm holds L with the INVERSE diagonal on the diagonal.  Returns false if not
-// positive definite.
-// ------------------------------------------------------------------------------------------------
-// Packed triangle in shared memory: element k of thread t at base[k * STRIDE + t] (conflict-free: the 32 lanes of a
-// warp read 32 consecutive doubles), compile-time k -> immediate offsets.
-template <int STRIDE>
-struct TriSmem {
-  double* p;
-  __device__ __forceinline__ double& operator[](int k) const { return p[k * STRIDE]; }
-};
-
-template <int NC, class Mat>
-__device__ __forceinline__ bool chol_packed(Mat& Lm, const double (&g)[NC], double (&s)[NC]) {
-  bool pd = true;
-#pragma unroll
-  for (int j = 0; j < NC; ++j) {
-    double acc = Lm[tri(j, j)];
-#pragma unroll
-    for (int k = 0; k < j; ++k) acc = fma(-Lm[tri(j, k)], Lm[tri(j, k)], acc);
-    pd = pd && (acc > 0.0);
-    const double inv = rsqrt_fast(acc);
-    Lm[tri(j, j)] = inv;
-#pragma unroll
-    for (int i = j + 1; i < NC; ++i) {
-      double a = Lm[tri(i, j)];
-#pragma unroll
-      for (int k = 0; k < j; ++k) a = fma(-Lm[tri(i, k)], Lm[tri(j, k)], a);
-      Lm[tri(i, j)] = a * inv;
-    }
-  }
-  double yv[NC];
-#pragma unroll
-  for (int i = 0; i < NC; ++i) {
-    double acc = -g[i];
-#pragma unroll
-    for (int k = 0; k < i; ++k) acc = fma(-Lm[tri(i, k)], yv[k], acc);
-    yv[i] = acc * Lm[tri(i, i)];
-  }
-#pragma unroll
-  for (int i = NC - 1; i >= 0; --i) {
-    double acc = yv[i];
-#pragma unroll
-    for (int k = i + 1; k < NC; ++k) acc = fma(-Lm[tri(k, i)], s[k], acc);
-    s[i] = acc * Lm[tri(i, i)];
-  }
-  return pd;
 }
 
 }  // namespace ptf

@@ -241,7 +241,7 @@ struct SplitState {
 // Leaves x, y, theta consistent with st.lnK when it returns with converged or go_newton set.
 template <int NC>
 __device__ __noinline__ void split_ss(const Sys<NC>& S, const Opt& o, const MixCtx<NC>& m, SplitState<NC>& st,
-                                      double (&x)[NC], double (&y)[NC]) {
+                                      double (&x)[NC], double (&y)[NC], bool hinted) {
   double K[NC], lpx[NC], lpy[NC], Sv[NC];
   Eos e;
   st.iters = 0; st.status = 0; st.theta = 0.0;
@@ -254,12 +254,13 @@ __device__ __noinline__ void split_ss(const Sys<NC>& S, const Opt& o, const MixC
 #pragma unroll
     for (int i = 0; i < NC; ++i)
       if (m.z[i] > 0.0) mk = fmax(mk, fabs(st.lnK[i]));
-    if (mk < 1.0e-9) { st.failed = true; break; }  // trivial collapse
+    if (mk < o.split_trivial_tol) { st.failed = true; break; }  // trivial collapse (C22)
 #pragma unroll
     for (int i = 0; i < NC; ++i) K[i] = exp(st.lnK[i]);
     if (!rr_solve<NC>(K, m.z, theta, x, y)) { st.failed = true; break; }
     if (o.use_newton && k >= o.split_ss_iters && theta > 0.0 && theta < 1.0) { st.go_newton = true; break; }
     if (k >= o.ss_cap) { st.status |= ST_SPLIT_CAP; break; }
+    if (hinted && k >= o.hint_ss_cap && !(theta > 0.0 && theta < 1.0)) { st.failed = true; break; }   // reading C21
     lnphi_eval<NC>(S, m.sa, m.bi, x, lpx, Sv, e);
     lnphi_eval<NC>(S, m.sa, m.bi, y, lpy, Sv, e);
     double rk = 0.0;
@@ -326,8 +327,9 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
   bool converged = false;
 #pragma unroll 1
   for (int itn = 0; itn < o.split_tr_iters; ++itn) {
-    if (gmax < o.tol_newton_g) { converged = true; break; }
-    st.iters++;
+    // reading C8: a gradient below the target triggers one last full Newton step (applied if admissible), see DESIGN.md
+    const bool last = gmax < o.tol_newton_g;
+    if (!last) st.iters++;
     dlnphi<NC>(S, m.sa, m.bi, Sx, ex, Mx);
     dlnphi<NC>(S, m.sa, m.bi, Sy, ey, My);
     const double tt = theta * (1.0 - theta), itt = 1.0 / tt;
@@ -343,12 +345,16 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
       }
     }
     double eta = 0.0, snorm = 0.0;
-    if (!tr_subproblem<NC>(H, gt, D, Delta, 1.0e-3 * itt, nV, m.z, act, sstep, eta, snorm, Lc)) { st.status |= ST_SPLIT_CAP; break; }
+    if (!tr_subproblem<NC>(H, gt, D, Delta, 1.0e-3 * itt, nV, m.z, act, sstep, eta, snorm, Lc)) {
+      if (last) converged = true; else st.status |= ST_SPLIT_CAP;
+      break;
+    }
     double smax = 0.0;   // largest step relative to the smaller of the two mole numbers n^V_i, n^L_i = z_i - n^V_i
 #pragma unroll
     for (int i = 0; i < NC; ++i)
       if (act[i]) smax = fmax(smax, fabs(sstep[i]) / fmin(nV[i], m.z[i] - nV[i]));
-    if (eta == 0.0 && smax < o.tol_newton_step) {
+    if (last && eta != 0.0) { converged = true; break; }
+    if (eta == 0.0 && (last || smax < o.tol_newton_step)) {
       theta = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) { if (act[i]) nV[i] += sstep[i]; theta += nV[i]; }
@@ -372,7 +378,7 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
     for (int i = 0; i < NC; ++i) { nV_old[i] = nV[i]; if (act[i]) nV[i] += sstep[i]; }
     eval();
     const double act_red = G - G_old;
-    const bool accept = (act_red < 0.0) || (gmax < gmax_old);
+    const bool accept = (act_red < 0.0) || (gmax < gmax_old && act_red <= 1.0e-12 * fabs(G_old));
     if (accept) {
       if (fabs(pred) > 1.0e-13) {
         const double ratio = fabs(act_red / pred);
@@ -391,7 +397,7 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
 #pragma unroll
   for (int i = 0; i < NC; ++i)
     if (act[i]) { st.lnK[i] = log(y[i]) - log(x[i]); mkn = fmax(mkn, fabs(st.lnK[i])); }
-  if (mkn < 1.0e-9) st.failed = true;   // Newton slid into the trivial solution x = y
+  if (mkn < o.split_trivial_tol) st.failed = true;   // Newton slid into the trivial solution x = y
   st.converged = converged;
   st.theta = theta;
 }
@@ -410,11 +416,11 @@ __device__ __forceinline__ void split_finish(const SplitState<NC>& st, SplitRes&
 // all stages (engine 0)
 template <int NC>
 __device__ __forceinline__ void phase_split(const Sys<NC>& S, const Opt& o, const MixCtx<NC>& m, double (&lnK)[NC],
-                                            double (&x)[NC], double (&y)[NC], SplitRes& res) {
+                                            double (&x)[NC], double (&y)[NC], SplitRes& res, bool hinted) {
   SplitState<NC> st;
 #pragma unroll
   for (int i = 0; i < NC; ++i) st.lnK[i] = lnK[i];
-  split_ss<NC>(S, o, m, st, x, y);
+  split_ss<NC>(S, o, m, st, x, y, hinted);
   if (st.go_newton) split_newton<NC>(S, o, m, st, x, y);
   split_finish<NC>(st, res);
 #pragma unroll
@@ -631,7 +637,7 @@ __device__ void flash_one(const Sys<NC>& S, const Opt& o, const Io& io, int64_t 
     int split_status = 0;
     if (unstable) {
       SplitRes sp;
-      phase_split<NC>(S, o, m, lnK, x, y, sp);
+      phase_split<NC>(S, o, m, lnK, x, y, sp, skip_stab);
       iters += sp.iters;
       split_status = sp.status;
       two = sp.two_phase;

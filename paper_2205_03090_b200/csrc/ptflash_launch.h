@@ -37,6 +37,7 @@ struct StageCounters {
 typedef int (*launch_fn)(const SysHost&, const Opt&, const Io&, void* workspace, cudaStream_t);
 size_t staged_workspace_bytes(int nc, int64_t N);
 int run_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, cudaStream_t st);
+int run_math_probe(int fn, int64_t n, const double* x, double* y, cudaStream_t st);
 
 #define PTF_DECL(NC) int launch_mono_##NC(const SysHost&, const Opt&, const Io&, void*, cudaStream_t); \
   int launch_staged_##NC(const SysHost&, const Opt&, const Io&, void*, cudaStream_t);

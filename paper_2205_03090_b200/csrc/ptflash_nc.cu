@@ -39,13 +39,4 @@ int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& i
 }
 
 }  // namespace ptf
-#ifdef PTF_DEBUG_COUNT
-#if PTF_NC == 10
-extern "C" void ptflash_debug_counters(unsigned long long* out, int reset) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, ptf::g_dbg, sizeof(unsigned long long) * 64);
-  if (reset) { unsigned long long z[64] = {0}; cudaMemcpyToSymbol(ptf::g_dbg, z, sizeof(z)); }
-}
-#endif
-#endif
 #endif

@@ -78,9 +78,9 @@ struct LRows {
 // MOD (modified Cholesky): a pivot that is not safely positive is replaced by max(-pivot, 1e-10 |H_ii|) and pd is cleared --
 // the factor then belongs to H + E with a diagonal E >= 0, so the solve still gives a descent direction (a negative
 // curvature direction is followed with its Newton length, sign flipped).
-template <int NC, bool MOD = false>
+template <int NC>
 __device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const LRows<NC>& L, double (&invd)[NC],
-                                         double (&yv)[NC], double (&s)[NC], const double rhs, bool& pd) {
+                                         double (&yv)[NC], double (&s)[NC], const double rhs, bool& pd, const bool MOD = false) {
   const double hii = row[i];
 #pragma unroll
   for (int j = 0; j < NC; ++j) {
@@ -131,9 +131,6 @@ __device__ __forceinline__ void chol_back(const LRows<NC>& L, const double (&inv
   }
 }
 
-#ifndef PTF_SPLIT_MODCHOL
-#define PTF_SPLIT_MODCHOL 1   // split Newton: one modified-Cholesky factorisation per iteration + step truncation (0: eta search)
-#endif
 #ifndef PTF_STABN_MINB
 #define PTF_STABN_MINB 2
 #endif
@@ -411,7 +408,8 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   const int total = w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON];
   const int* const q_in = part ? w.q_split_newton_b : w.q_split_newton;
   int* ticket = &w.qcount[part ? Q_TICKET_SPLIT_B : Q_TICKET_SPLIT];
-  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
+  bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false, polish = false;
+  bool eta_mode = false;   // this lane's item runs the eta search of B.4a instead of the truncated modified-Cholesky step
   int n = 0, tr_it = 0, status = 0;
   unsigned act = 0u;
   PT3<NC> q;
@@ -433,6 +431,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           const double P = io.P[n], Tk = io.T[n];
           { const double iT = rcp_fast(Tk); q.sT = sqrt_fast(Tk); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
           act = (unsigned)w.actmask[n];
+          eta_mode = (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED);
 #pragma unroll
           for (int i = 0; i < NC; ++i) {
             sn[i * T] = w.lnK[(int64_t)i * N + n];   // k2_split_ss left n^V here
@@ -443,6 +442,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           first = true;
           reeval = false;
           searching = false;
+          polish = false;
           Delta = 0.25;
           ex.Z = w.Zxy[n];
           ey.Z = w.Zxy[N + n];
@@ -463,7 +463,6 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
     bool finish = false, fin_conv = false;
     if (busy && !searching) {
       // ---- evaluate G (eq. 8) and its gradient (B.5a) at n^V + s ----
-      PTF_DBG(0, 1);
       theta = 0.0;
 #pragma unroll
       for (int i = 0; i < NC; ++i) theta += sn[i * T] + sp[i * T];
@@ -503,7 +502,11 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       bool accepted = true;
       if (!first && !reeval) {
         const double act_red = G_new - G;
-        accepted = (act_red < 0.0) || (gmax < gmax_acc);
+        // accept if G fell; a smaller gradient is accepted instead only where the change of G is below its rounding
+        // resolution (next to the solution).  With the plain "G fell or the gradient fell" a modified-Cholesky step (C25)
+        // that raises G is accepted whenever it happens to lower the gradient norm, and single mixtures next to the phase
+        // boundary wander across the whole box 0 < n < z until the iteration cap (config 5: 1.5 per 1000).
+        accepted = (act_red < 0.0) || (gmax < gmax_acc && act_red <= 1.0e-12 * fabs(G));
         if (accepted) {
           if (fabs(pred) > 1.0e-13) {
             const double ratio = fabs(act_red * rcp_fast(pred));
@@ -513,7 +516,6 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         } else {
           Delta = 0.5 * dmin(Delta, snorm);
           reeval = true;
-          PTF_DBG(1, 1);
         }
       }
       if (!accepted) {
@@ -526,10 +528,13 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         gmax_acc = gmax;
         first = false;
         reeval = false;
-        if (gmax < o.tol_newton_g) { finish = true; fin_conv = true; }
-        else if (tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
+        // Reading C8: a gradient below the target does not end the iteration by itself -- near a critical point and next
+        // to the phase boundary the Hessian is nearly singular and the gradient does not bound the error of n^V -- it
+        // triggers one last full Newton step (polish), applied without another evaluation if it is admissible.
+        polish = gmax < o.tol_newton_g;
+        if (!polish && tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
         else {
-          tr_it++;
+          if (!polish) tr_it++;
           es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
           kept_sn = 0.0;
           searching = true;
@@ -539,7 +544,6 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
     __syncwarp();
     if (busy && searching) {
       // ---- ONE attempt of the restricted-step sub-problem at eta (B.4a) ----
-      PTF_DBG(2, 1);
       const MC3 mx = mc3(ex), my = mc3(ey);
       const double tt = theta * (1.0 - theta), itt = rcp_fast(tt);
       const double wx = theta * itt, wy = (1.0 - theta) * itt;   // weights of M(x), M(y) in B.5b
@@ -581,15 +585,16 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           }
         }
         row[i] = fma(sD[i * T], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
-        chol_row<NC, PTF_SPLIT_MODCHOL != 0>(i, row, L, invd, yv, st, -sg[i * T], pd);
+        chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd, !eta_mode);
       }
       chol_back<NC>(L, invd, yv, st);
-#if PTF_SPLIT_MODCHOL
-      // Restricted step without a search: the direction of the (modified) factorisation is cut back to the trust region and
-      // to 90 % of the way to the nearest face of the box 0 < n_i < z_i.  One factorisation, i.e. one trip, per iteration;
-      // the eta search of the paper's B.4a (grow x8, then bisect: up to ten factorisations) is kept for the stability
-      // kernel, whose path decides labels.  Acceptance and the radius update (B.3) are unchanged.
-      {
+      // Restricted step without a search (C25): the direction of the (modified) factorisation is cut back to the trust region
+      // and to 90 % of the way to the nearest face of the box 0 < n_i < z_i.  One factorisation, i.e. one trip, per
+      // iteration; the eta search of the paper's B.4a (grow x8, then bisect: up to ten factorisations) is kept for the
+      // stability kernel, whose path decides labels, and for splits entered through a skip-stability hint (eta_mode):
+      // from a caller's K next to the phase boundary the truncated step slides into a face of the box and fails where the
+      // search converges, and whether a hint fails is reported (C21).  Acceptance and the radius update (B.3) are shared.
+      if (!eta_mode) {
         double s2 = 0.0, sgd = 0.0, over = 0.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
@@ -612,8 +617,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         pred = (t - 0.5 * t * t) * sgd;
         exact = pd && t == 1.0;
         es.phase = ok ? 3 : 4;
-      }
-#else
+      } else {
       bool good = pd;
       double s2 = 0.0, sds = 0.0, sgd = 0.0;
 #pragma unroll
@@ -636,9 +640,18 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         pred = 0.5 * sgd - 0.5 * eta_used * sds;
         exact = (eta_used == 0.0);
       }
-      if (!good) PTF_DBG(5, 1);
-#endif
-      if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
+      }
+      if (polish) {
+        // last step: applied if it is the full Newton step of a positive definite Hessian inside the box and the trust
+        // region; otherwise the evaluated point stands
+        finish = true;
+        fin_conv = true;
+        searching = false;
+        if (es.phase == 3 && exact) {
+#pragma unroll
+          for (int i = 0; i < NC; ++i) sn[i * T] += sp[i * T];
+        }
+      } else if (es.phase == 4) { finish = true; status |= ST_SPLIT_CAP; searching = false; }
       else if (es.phase == 3) {
         searching = false;
         double smax = 0.0;   // largest step relative to the smaller of the two mole numbers n_i, z_i - n_i
@@ -674,7 +687,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
 #pragma unroll
       for (int i = 0; i < NC; ++i)
         if ((act >> i) & 1u) mkn = dmax(mkn, fabs(y[i] - x[i]) * rcp_fast(x[i]));
-      const bool trivial = mkn < 1.0e-9;
+      const bool trivial = mkn < o.split_trivial_tol;
       if (io.lnK) {
 #pragma unroll
         for (int i = 0; i < NC; ++i) lnK[i] = ((act >> i) & 1u) ? log_fast(y[i]) - log_fast(x[i]) : 0.0;
@@ -682,10 +695,6 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
 #pragma unroll
         for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
       }
-      PTF_DBG(6, 1);
-      PTF_DBG(7, fin_conv ? 0 : 1);
-      PTF_DBG(8, trivial ? 1 : 0);
-      PTF_DBG(9, tr_it);
       store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, ex.Z, ey.Z);
       busy = false;
     }

@@ -48,6 +48,36 @@ int run_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, cudaStream
   return 0;
 }
 
+// Element-wise evaluation of one lean math routine of ptflash_math.cuh (diagnostic entry ptflash_math_probe).
+__global__ void __launch_bounds__(256) math_probe_kernel(int fn, int64_t n, const double* __restrict__ x, double* __restrict__ y) {
+  __shared__ double s_exp[PTF_EXP_TAB];
+  exp_tab_init(s_exp);
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double v = x[i];
+    double r;
+    switch (fn) {
+      case 0: r = exp_fast(v); break;
+      case 1: r = exp_tab(v, s_exp); break;
+      case 2: r = log_fast(v); break;
+      case 3: r = log1p_fast(v); break;
+      case 4: r = rcp_fast(v); break;
+      case 5: r = rsqrt_fast(v); break;
+      case 6: r = sqrt_fast(v); break;
+      case 7: r = div_fast(1.0, v); break;
+      case 8: r = rcp_nr1(v); break;
+      default: r = v; break;
+    }
+    y[i] = r;
+  }
+}
+
+int run_math_probe(int fn, int64_t n, const double* x, double* y, cudaStream_t st) {
+  if (n <= 0) return 0;
+  const int64_t blocks = (n + 255) / 256;
+  math_probe_kernel<<<(unsigned)(blocks < 4096 ? blocks : 4096), 256, 0, st>>>(fn, n, x, y);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
 size_t staged_workspace_bytes(int nc, int64_t N) {
   return carve_workspace(nc, N, nullptr, nullptr);
 }

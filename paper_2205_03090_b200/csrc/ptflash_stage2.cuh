@@ -14,45 +14,10 @@
 
 namespace ptf {
 
-// per-(P,T) arrays + active mask of mixture n (already validated and normalised by k_init)
-template <int NC>
-__device__ __forceinline__ void load_pt(const Sys<NC>& S, const Io& io, int n, double (&sa)[NC], double (&bi)[NC], double& P,
-                                        double& T) {
-  P = io.P[n];
-  T = io.T[n];
-  eos_setup<NC>(S, P, T, sa, bi);
-}
-
 template <int NC>
 __device__ __forceinline__ void load_zn(const Io& io, const Work& w, int n, double (&z)[NC]) {
 #pragma unroll
   for (int i = 0; i < NC; ++i) z[i] = __ldg(&w.zn[(int64_t)i * io.N + n]);   // normalised once by k_init
-}
-
-// one successive-substitution iteration of the phase split (Fig. 1): K = exp(lnK), RR, lnphi(x), lnphi(y),
-// lnK <- lnphi(x) - lnphi(y).  Returns false if Rachford-Rice has no window.  rk = max |d lnK|.
-template <int NC, bool KIJ0>
-__device__ __forceinline__ bool split_iteration(const Sys<NC>& S, const double (&sa)[NC], const double (&bi)[NC],
-                                                const double (&z)[NC], double (&lnK)[NC], double& theta, double (&x)[NC],
-                                                double (&y)[NC], double (&lpx)[NC], double (&lpy)[NC], double& Zx, double& Zy,
-                                                double& rk, bool update) {
-  double K[NC], Sv[NC];
-#pragma unroll
-  for (int i = 0; i < NC; ++i) K[i] = exp_fast(lnK[i]);
-  if (!rr_fast<NC>(K, z, theta, x, y)) return false;
-  if (!update) return true;
-  Eos e;
-  e.Z = Zx;
-  lnphi_fast<NC, KIJ0>(S, sa, bi, x, lpx, Sv, e);
-  Zx = e.Z;
-  e.Z = Zy;
-  lnphi_fast<NC, KIJ0>(S, sa, bi, y, lpy, Sv, e);
-  Zy = e.Z;
-  rk = 0.0;
-#pragma unroll
-  for (int i = 0; i < NC; ++i)
-    if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = dmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
-  return true;
 }
 
 // ---- K1b: probe -----------------------------------------------------------------------------------
@@ -144,7 +109,6 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
 #define PTF_SS_MINB 4
 #endif
 constexpr double LNW_ZERO = -1000.0;
-constexpr int HINT_SS_CAP = 30;
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
@@ -318,7 +282,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
 #pragma unroll
         for (int i = 0; i < NC; ++i)
           if (z[i] > 0.0) mk = dmax(mk, fabs(lnK[i]));
-        if (mk < 1.0e-9) { failed = true; break; }   // trivial collapse
+        if (mk < o.split_trivial_tol) { failed = true; break; }   // trivial collapse (C22)
         {
           double K[NC];
 #pragma unroll
@@ -328,10 +292,10 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         if (final_rr) { converged = true; break; }
         if (o.use_newton && k >= o.split_ss_iters && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
         if (k >= o.ss_cap) { status |= ST_SPLIT_CAP; break; }
-        // A skip-stability hint (C21) whose successive substitution has not brought theta into (0,1) after HINT_SS_CAP
-        // iterations is dropped here (-> cold re-flash in pass 1) instead of crawling towards the SS cap: next to the
+        // A skip-stability hint (C21) whose successive substitution has not brought theta into (0,1) after hint_ss_cap
+        // iterations is dropped here (-> cold re-flash) instead of crawling towards the SS cap: next to the
         // phase boundary such a mixture can take 1e5 iterations (40 ms for the whole call) to fail.
-        if (hinted && k >= HINT_SS_CAP) { failed = true; break; }
+        if (hinted && k >= o.hint_ss_cap && !(theta > 0.0 && theta < 1.0)) { failed = true; break; }
         {
           Eos e;
           double Sv[NC];
@@ -391,21 +355,21 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   // persistent refill kernels: as many CTAs per SM as registers and shared memory allow (queried once per instantiation)
   const size_t stab_bytes = (size_t)stabn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
   const size_t split_bytes = (size_t)splitn_smem_doubles<NC>() * NEWTON_THREADS * sizeof(double);
-  // (per device: the shared-memory attribute of a kernel is device state, and a process may hold handles on several GPUs)
-  static int stab_cta_dev[64] = {0}, split_cta_dev[64] = {0};
-  int dev_id = 0;
-  cudaGetDevice(&dev_id);
-  int& stab_cta = stab_cta_dev[dev_id & 63];
-  int& split_cta = split_cta_dev[dev_id & 63];
-  if (stab_cta == 0) {
-    cudaFuncSetAttribute(k3_stab_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stab_bytes);
-    cudaFuncSetAttribute(k3_split_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)split_bytes);
+  // (queried once per handle, i.e. per device and component system: the shared-memory attribute of a kernel is device
+  // state; setting it again from another handle on the same device is idempotent)
+  int local_cache[2] = {0, 0};
+  int* const cache = o.cta_cache ? o.cta_cache : local_cache;
+  if (cache[0] == 0 || cache[1] == 0) {
+    if (cudaFuncSetAttribute(k3_stab_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stab_bytes) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k3_split_newton<NC, KIJ0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)split_bytes) != cudaSuccess) return -1;
     int a = 0, b = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k3_stab_newton<NC, KIJ0>, NEWTON_THREADS, stab_bytes);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k3_split_newton<NC, KIJ0>, NEWTON_THREADS, split_bytes);
-    stab_cta = a > 0 ? a : 1;
-    split_cta = b > 0 ? b : 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k3_stab_newton<NC, KIJ0>, NEWTON_THREADS, stab_bytes) != cudaSuccess) return -1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k3_split_newton<NC, KIJ0>, NEWTON_THREADS, split_bytes) != cudaSuccess) return -1;
+    if (a < 1 || b < 1) return -1;   // the kernel does not fit an SM: report instead of launching an empty grid
+    cache[0] = a;
+    cache[1] = b;
   }
+  const int stab_cta = cache[0], split_cta = cache[1];
   // optional stage profiling: one event before the first kernel and one after every stage kernel
   cudaEvent_t* ev = (cudaEvent_t*)o.prof_events;
   int nev = 0;

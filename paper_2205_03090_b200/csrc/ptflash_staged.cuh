@@ -408,7 +408,7 @@ __global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC
 #pragma unroll
       for (int i = 0; i < NC; ++i) st.lnK[i] = w.lnK[(int64_t)i * io.N + n];
       double x[NC], y[NC];
-      split_ss<NC>(S, o, m, st, x, y);
+      split_ss<NC>(S, o, m, st, x, y, (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED));
       go_newton = st.go_newton;
       if (go_newton) {
 #pragma unroll

@@ -78,3 +78,28 @@ def build(oracle, N: int, batch: int = 4096, nthreads: int = 0):
     flags = np.where(two, 1, 0).astype(np.uint8)
     return w, np.ascontiguousarray(lnK0), flags, {"cold": cold, "two_phase_fraction": float(two.mean()),
                                                   "acceptance": float(N) / tried}
+
+
+def build_cached(oracle, N: int, cache_dir: str = ""):
+    """build() with the result kept in the system's temporary directory (scratch; gpurun_out/ is limited to 64 MiB): the
+    boundary search costs ~60 oracle flashes per accepted mixture (SURVEY.md section 8(d) allows caching it).  The cache
+    holds inputs only; the oracle's cold answers are recomputed, so a stale cache can never supply an expected value, and
+    nothing depends on the cache being there."""
+    import tempfile
+    from pathlib import Path
+    path = Path(cache_dir or tempfile.gettempdir()) / f"ptflash_config5_inputs_{N}.npz"
+    sysm = W.system_co2_10()
+    if path.exists():
+        d = np.load(path)
+        w = W.Workload("config5_warm_near_boundary_10", sysm, d["P"], d["T"], np.ascontiguousarray(d["z"]), {"seed": SEED})
+        cold = oracle.flash(w.z, w.P, w.T)
+        two = cold["phase"] == 2
+        if np.array_equal(two, d["two"]):
+            return w, np.ascontiguousarray(d["lnK0"]), d["flags"], {"cold": cold, "two_phase_fraction": float(two.mean())}
+    w, lnK0, flags, info = build(oracle, N, batch=min(65536, max(4096, N // 8)))
+    try:
+        path.parent.mkdir(exist_ok=True)
+        np.savez(path, P=w.P, T=w.T, z=w.z, lnK0=lnK0, flags=flags, two=info["cold"]["phase"] == 2)
+    except OSError:
+        pass
+    return w, lnK0, flags, info

@@ -7,7 +7,8 @@ import pytest
 from paper_2205_03090_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
-import sys, os
+import os
+import sys
 sys.path.insert(0, os.path.dirname(__file__))
 
 TOL = 1e-8
@@ -29,20 +30,24 @@ def _gpu_flash(w, engine, lnK0=None, flags=None, **opts):
     return res
 
 
-def compare(w, g, o, tol=TOL):
-    """Returns a report dict; raises AssertionError on a parity failure outside the reported band."""
+def compare(w, g, o, tol=TOL, excuse=None):
+    """Element-by-element comparison; returns a report dict.  The near-zero-TPD band (reading C9) is decided from the
+    ORACLE's minimum TPD alone: a label mismatch is excused only where the oracle itself reports 0 < |tpd_min| < 1e-9.
+    `excuse`: boolean mask of mixtures left out of the comparison (the caller bounds and reports them)."""
     N = w.N
-    mism = np.where(g["phase"] != o["phase"])[0]
-    band = np.array([n for n in mism if (o["status"][n] & 4) or (g["status"][n] & 4)
-                     or (np.isfinite(o["tpd_min"][n]) and abs(o["tpd_min"][n]) < 1e-9)], dtype=int)
+    keep = np.ones(N, dtype=bool) if excuse is None else ~excuse
+    mism = np.where((g["phase"] != o["phase"]) & keep)[0]
+    in_band = np.isfinite(o["tpd_min"]) & (o["tpd_min"] != 0.0) & (np.abs(o["tpd_min"]) < 1e-9)
+    band = mism[in_band[mism]]
     hard = np.setdiff1d(mism, band)
-    same2 = (g["phase"] == 2) & (o["phase"] == 2)
-    same1 = (g["phase"] == 1) & (o["phase"] == 1)
+    same2 = (g["phase"] == 2) & (o["phase"] == 2) & keep
+    same1 = (g["phase"] == 1) & (o["phase"] == 1) & keep
     db = np.abs(g["beta"] - o["beta"])
     dx = np.abs(g["x"] - o["x"]).max(0)
     dy = np.abs(g["y"] - o["y"]).max(0)
     err2 = np.maximum(db, np.maximum(dx, dy))
     rep = dict(N=N, two_phase=int(same2.sum()), label_mismatch=len(mism), in_band=len(band),
+               oracle_band_size=int(in_band.sum()),
                max_err_two_phase=float(err2[same2].max()) if same2.any() else 0.0,
                max_err_single=float(np.maximum(dx, dy)[same1].max()) if same1.any() else 0.0,
                beta_convention_mismatch=int((db[same1] != 0).sum()))
@@ -57,16 +62,58 @@ def compare(w, g, o, tol=TOL):
     rep["messages"] = msg
     rep["n_hard"] = len(hard)
     rep["n_bad"] = len(bad)
+    rep["bad"] = bad
+    rep["band"] = band
     return rep
 
 
-def check(w, g, o):
-    rep = compare(w, g, o)
-    print({k: v for k, v in rep.items() if k != "messages"})
+MAX_BAND_PER_MILLION = 5     # label mismatches excused by the oracle's |tpd_min| < 1e-9 band: listed, and bounded by this
+
+
+def check(w, g, o, excuse=None):
+    rep = compare(w, g, o, excuse=excuse)
+    print({k: v for k, v in rep.items() if k not in ("messages", "bad", "band")})
+    for n in rep["band"]:
+        print(f"  in-band label mismatch n={n}: tpd_min oracle {o['tpd_min'][n]:.3e} gpu {g['tpd_min'][n]:.3e}")
     assert rep["n_hard"] == 0 and rep["n_bad"] == 0, "\n".join(rep["messages"])
+    assert rep["in_band"] <= max(1, int(np.ceil(MAX_BAND_PER_MILLION * w.N / 1e6)))
     assert rep["max_err_single"] == 0.0            # single phase: x = y = z bit-exact
     assert rep["beta_convention_mismatch"] == 0
     return rep
+
+
+def _vec(r, n):
+    return np.concatenate([[r["beta"][n]], r["x"][:, n], r["y"][:, n]])
+
+
+def adjudicate(oracle_mod, w, g, o, idx, lnK0=None, flags=None):
+    """Conditioning note of SURVEY.md section 8(c): every two-phase mixture whose beta, x or y differs from the (double)
+    oracle by more than 1e-8 is re-flashed by the oracle in long double with tight tolerances -- the best available
+    value of the exact fixed point -- and reported with d_c = ||ln K||_2 (eq. 14), the last SS rate and the
+    iteration counts.  With e_gpu, e_oracle the distances of the CUDA result and of the double oracle from that value, the
+    miss is attributed
+      * to the ORACLE's rounding        if e_gpu <= 1e-8 (the CUDA result is within the bar of the exact answer);
+      * to CONDITIONING                 if e_gpu <= 4 e_oracle: next to a critical point or the phase boundary the Hessian
+        of G is nearly singular and plain fp64 evaluation of ln phi does not fix n^V to 1e-8 -- the double oracle itself
+        misses the exact answer by e_oracle > 2.5e-9, and the CUDA path is within a small factor of that;
+      * to a BUG                        otherwise (the test fails)."""
+    ld = oracle_mod.Oracle.from_system(w.system, real="long double")
+    tight = dict(tol_ss=1e-13, tol_newton_g=1e-15, tol_newton_step=1e-13)
+    rows = []
+    for n in idx:
+        z, P, T = np.ascontiguousarray(w.z[:, n:n + 1]), w.P[n:n + 1].copy(), w.T[n:n + 1].copy()
+        kw = {} if lnK0 is None else dict(lnK0=np.ascontiguousarray(lnK0[:, n:n + 1]), flags=flags[n:n + 1].copy())
+        b = ld.flash(z, P, T, nthreads=1, opts=tight, **kw)
+        vg, vo = _vec(g, n), _vec(o, n)
+        two = b["phase"][0] == 2
+        e_g = float(np.abs(vg - _vec(b, 0)).max()) if two else float("inf")
+        e_o = float(np.abs(vo - _vec(b, 0)).max()) if two else float("inf")
+        why = "oracle rounding" if e_g <= TOL else ("conditioning" if e_g <= 4.0 * e_o else "BUG")
+        rows.append(dict(n=int(n), gap_gpu_oracle=float(np.abs(vg - vo).max()), e_gpu=e_g, e_oracle=e_o, attributed=why,
+                         d_c=float(o["diag"][1, n]), ss_rate=float(o["diag"][2, n]), iters_oracle=int(o["iters"][n]),
+                         iters_gpu=int(g["iters"][n]), beta_gpu=float(g["beta"][n]), beta_oracle=float(o["beta"][n]),
+                         beta_long_double_tight=float(b["beta"][0])))
+    return rows
 
 
 @pytest.mark.parametrize("engine", [0, 1])
@@ -104,13 +151,10 @@ def test_parity_config5_warm_start(oracle_mod):
         # a failed skip-stability hint is dropped and reported (ST_WARM_RESTART), on both sides for the same mixtures
         # up to a handful of borderline cases; after the restart the answer is the cold one
         assert 0 < restarted.sum() < 0.03 * w.N
-        # Which near-boundary hints fail depends on the path: the oracle searches eta as in B.4a and lets a hinted split
-        # crawl outside (0,1) up to the SS cap; the CUDA split uses one modified-Cholesky factorisation per iteration
-        # (C25) and drops a hint whose SS is still outside (0,1) after 30 iterations (C21).  So the CUDA path restarts a
-        # few more mixtures; the answers after a restart are the cold ones either way (checked above and below).
+        # both sides drop a hinted split that is still outside 0 < theta < 1 after 30 SS iterations (C21), so they restart
+        # the same mixtures up to a handful of borderline cases (the Newton stage of the split follows C25 on the CUDA side)
         o_restarted = (o_warm["status"] & 64) != 0
-        assert np.sum(o_restarted & ~restarted) <= 0.005 * w.N
-        assert np.sum(restarted & ~o_restarted) <= 0.015 * w.N
+        assert np.sum(o_restarted != restarted) <= 3
         assert np.array_equal(g_warm["phase"][restarted], g_cold["phase"][restarted])
         print("config5 engine", engine, "mean iters (two-phase): warm %.2f cold %.2f; cold stability iters %.2f" %
               (g_warm["iters"][two].mean(), g_cold["iters"][two].mean(), g_cold["stab_iters"][two].mean()), rep_w, rep_c)
@@ -297,22 +341,253 @@ def test_outputs_stay_inside_their_buffers(N):
     f.close()
 
 
-def test_full_size_sampled_parity_and_invariants(oracle_mod):
-    """BASELINE size (config 3, N = 1,000,000, the launch configuration bench.py times): invariants on every mixture,
-    oracle parity on a seeded sample computed one by one (mixtures are independent)."""
-    N = 1_000_000
+def test_lnK0_flags_and_rejection(oracle_mod):
+    """Warm-start sub-paths of ptflash_flash_ex (a14): flags 0..3 mixed in one call -- bit 1 (PTFLASH_FLAG_USE_LNK0: the
+    caller's K seeds the probe and both stability starts, reading C19), bit 0 (skip stability), both -- plus rejected
+    estimates (NaN, +-inf, |lnK0| > 700 -> Wilson, PTFLASH_ST_LNK0_REJECTED; the overflow failure of PAPER.md:363), plus
+    skip-stability hints on mixtures that are in fact single phase (-> PTFLASH_ST_WARM_RESTART), all against the oracle."""
+    N = 20000
     w = W.config3(N)
-    g = _gpu_flash(w, 1)
+    orc = oracle_mod.Oracle.from_system(w.system)
+    cold = orc.flash(w.z, w.P, w.T)
+    two = cold["phase"] == 2
+    n = np.arange(N)
+    nc = w.system.nc
+    wil = np.stack([orc.wilson(w.P[k], w.T[k]) for k in range(N)], axis=1)
+    noise = np.stack([W.normal(909, n, 2 * i) for i in range(nc)])
+    lnK0 = np.where(two[None, :], cold["lnK"] + 0.05 * noise, wil + 0.3 * noise)
+    flags = np.minimum((W.uniform(909, n, 50) * 4).astype(np.uint8), 3)
+    u = W.uniform(909, n, 51)
+    comp = np.minimum((W.uniform(909, n, 52) * nc).astype(int), nc - 1)
+    poison = {0: np.nan, 1: np.inf, 2: -np.inf, 3: 800.0, 4: -700.5}
+    bad = np.zeros(N, dtype=bool)
+    for k, v in poison.items():
+        sel = (u >= 0.006 * k) & (u < 0.006 * (k + 1))
+        lnK0[comp[sel], n[sel]] = v
+        bad |= sel
+    lnK0 = np.ascontiguousarray(lnK0)
+    o = orc.flash(w.z, w.P, w.T, lnK0=lnK0, flags=flags)
+    for engine in (1, 0):
+        g = _gpu_flash(w, engine, lnK0=lnK0, flags=flags)
+        g_cold = _gpu_flash(w, engine)
+        # a skip-stability hint on a mixture the stability analysis calls stable is a contradiction the caller created:
+        # whether the split from a noisy K still finds a (metastable) two-phase solution or fails and restarts depends on
+        # the iteration path.  Such mixtures are compared unless the two sides ended with different restart flags.
+        excuse = ((o["status"] ^ g["status"]) & 64) != 0
+        assert excuse.sum() <= 5 and not np.any(excuse & two)
+        check(w, g, o, excuse=excuse)
+        rej_o, rej_g = (o["status"] & 32) != 0, (g["status"] & 32) != 0
+        assert np.array_equal(rej_o, rej_g) and np.array_equal(rej_g, bad & (flags != 0))
+        assert rej_g.sum() > 100
+        # a rejected estimate means the plain Wilson path: bit-identical to the cold call
+        for k in ("phase", "beta", "x", "y", "iters", "stab_iters"):
+            assert np.array_equal(g[k][..., rej_g], g_cold[k][..., rej_g], equal_nan=True), k
+        rs_g = (g["status"] & 64) != 0
+        assert rs_g.sum() > 0.05 * N                                   # wrong hints on single-phase mixtures are dropped
+        assert not np.any(rs_g & ((flags & 1) == 0))
+        # bit 1 alone changes the stability starts (different iteration counts than the Wilson starts) but not the answer
+        use = (flags == 2) & ~bad
+        assert (g["stab_iters"][use] != g_cold["stab_iters"][use]).mean() > 0.02
+        assert (np.abs(g["stab_iters"][use] - o["stab_iters"][use]) <= 2).mean() > 0.97    # the same starts as the oracle's
+        assert np.array_equal(g["phase"][use], g_cold["phase"][use])
+        # flags are ignored without lnK0, and lnK0 is ignored where flags == 0
+        assert np.array_equal(g["beta"][flags == 0], g_cold["beta"][flags == 0])
+        assert np.array_equal(_gpu_flash(w, engine, flags=flags)["beta"], g_cold["beta"])
+
+
+def test_stats_match_oracle_counts(oracle_mod):
+    """ptflash_get_stats (the paper's profiler columns, Table 4) against the same counts derived from the
+    oracle's per-mixture outputs (probe case, per-stage iteration counts, status)."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    for cfg in (3, 2):
+        N = 200_000
+        w = W.CONFIGS[cfg](N)
+        o = oracle_mod.Oracle.from_system(w.system).flash(w.z, w.P, w.T)
+        g = _gpu_flash(w, 1)
+        st = g["stats"]
+        pc, stg = o["probe_case"], o["stage"]
+        exp = dict(n_total=N, n_invalid=0, n_probe_case1=int((pc == 1).sum()), n_probe_case2=int((pc == 2).sum()),
+                   n_probe_case3=int((pc == 3).sum()), n_stability=int(((pc == 1) | (pc == 2)).sum()),
+                   n_stab_newton=int(stg[4].sum()), n_split=int(stg[7].sum()), n_split_newton=int(stg[8].sum()),
+                   n_two_phase=int((o["phase"] == 2).sum()))
+        print(cfg, {k: (st[k], v) for k, v in exp.items()})
+        for k in ("n_total", "n_invalid", "n_stability", "n_two_phase", "n_split"):
+            assert st[k] == exp[k], k
+        # the three probe outcomes and the "needed the Newton stage" counts hinge on floating-point thresholds (theta in
+        # (0,1), min < -1e-8, residual < 1e-10 after 9 iterations): equal up to a few borderline mixtures per million
+        for k in ("n_probe_case1", "n_probe_case2", "n_probe_case3", "n_stab_newton", "n_split_newton"):
+            assert abs(st[k] - exp[k]) <= max(2, 2e-5 * N), k
+        assert np.array_equal(g["stab_iters"] > 0, stg[0] + stg[1] + stg[2] + stg[3] > 0)
+        # iteration counts are path quantities (the CUDA stability Newton ends on a looser step criterion, C8), but close
+        went = o["stab_iters"] > 0
+        d = np.abs(g["stab_iters"] - o["stab_iters"])[went]
+        print("stability iterations (both starts): |gpu - oracle| mean %.3f, <= 2 in %.4f of the mixtures" % (d.mean(), (d <= 2).mean()))
+        assert (d <= 2).mean() > 0.97
+
+
+def test_second_device_keeps_current_device():
+    """A handle created on cuda:1 is used and destroyed while cuda:0 is current: the caller's device is
+    restored by every entry point and the results equal those of cuda:0."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    w = W.config3(5000)
+    ref = _gpu_flash(w, 1)
+    torch.cuda.set_device(1)
+    f = B.PTFlash.from_system(w.system)
+    torch.cuda.set_device(0)
+    d1 = torch.device("cuda:1")
+    z, P, T = (torch.from_numpy(a).to(d1) for a in (w.z, w.P, w.T))
+    with torch.cuda.device(1):
+        st = torch.cuda.current_stream().cuda_stream
+    out = f.flash(z, P, T, stream=st)
+    assert torch.cuda.current_device() == 0
+    f.stats()
+    assert torch.cuda.current_device() == 0
+    for k in ("phase", "beta", "x", "y"):
+        assert np.array_equal(out[k].cpu().numpy(), ref[k], equal_nan=True), k
+    f.close()
+    assert torch.cuda.current_device() == 0
+
+
+def _ulps(y, ref):
+    """|y - ref| in units of the spacing of doubles at ref (ref: numpy longdouble)."""
+    r64 = ref.astype(np.float64)
+    return np.abs((y.astype(np.longdouble) - ref) / np.spacing(np.abs(r64)).astype(np.longdouble)).astype(np.float64)
+
+
+def test_math_routines_against_libm():
+    """The lean exp / log / reciprocal routines of csrc/ptflash_math.cuh through ptflash_math_probe against libm in
+    extended precision: <= 2 ulp on the stated ranges, and the documented behaviour at the clamps."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(20220503)
+    M = 400_000
+    L = np.longdouble
+
+    def run(fn, x):
+        xd = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float64)).to(dev)
+        yd = torch.empty_like(xd)
+        B.ptflash_math_probe(fn, xd.numel(), xd, yd)
+        torch.cuda.synchronize()
+        return yd.cpu().numpy()
+
+    lognormal = np.exp(rng.uniform(-700.0, 700.0, M))
+    cases = {
+        "exp_fast": (np.concatenate([rng.uniform(-708.0, 709.0, M), rng.uniform(-1e-3, 1e-3, 1000), [0.0, -708.0, 709.0, 1e-300]]),
+                     lambda x: np.exp(x.astype(L))),
+        "exp_tab": (np.concatenate([rng.uniform(-700.0, 709.0, M), rng.uniform(-1e-3, 1e-3, 1000), [0.0, -700.0, 709.0]]),
+                    lambda x: np.exp(x.astype(L))),
+        "log_fast": (np.concatenate([lognormal, rng.uniform(0.5, 2.0, M), [1.0, np.sqrt(2.0), np.nextafter(np.sqrt(2.0), 2), 2.2250738585072014e-308, 1.7e308]]),
+                     lambda x: np.log(x.astype(L))),
+        "log1p_fast": (np.concatenate([rng.uniform(0.0, 1.0, M), np.exp(rng.uniform(-40, 0, M)) * 0.999, [0.0, 0.41421356237309503, 0.4142135623730951, 0.9999999999999999]]),
+                       lambda x: np.log1p(x.astype(L))),
+        "rcp_fast": (np.concatenate([np.exp(rng.uniform(-300, 300, M)) * rng.choice([-1.0, 1.0], M), [1.0, -1.0, 3.0]]),
+                     lambda x: L(1) / x.astype(L)),
+        "div_fast_1": (np.exp(rng.uniform(-300, 300, M)), lambda x: L(1) / x.astype(L)),
+        "rsqrt_fast": (np.exp(rng.uniform(-600, 600, M)), lambda x: L(1) / np.sqrt(x.astype(L))),
+        "sqrt_fast": (np.concatenate([np.exp(rng.uniform(-600, 600, M)), [0.0, 1.0, 4.0]]), lambda x: np.sqrt(x.astype(L))),
+    }
+    # exp_tab: table value (0.5 ulp) x degree-5 polynomial x product rounding; log: reciprocal + series + two-term ln 2 sum
+    bound = {"exp_tab": 2.5, "log_fast": 2.5, "log1p_fast": 2.5, "exp_fast": 1.0, "rcp_fast": 1.0, "div_fast_1": 1.0, "rsqrt_fast": 1.0, "sqrt_fast": 1.0}
+    worst = {}
+    for fn, (x, ref) in cases.items():
+        y = run(fn, x)
+        r = ref(x)
+        ok = r != 0
+        u = np.zeros(len(x))
+        u[ok] = _ulps(y[ok], r[ok])
+        assert np.all(np.isfinite(y)), fn
+        assert np.all(y[~ok] == 0.0), fn
+        print(f"{fn}: max {u.max():.3f} ulp, mean {u.mean():.3f} ulp over {len(x)} arguments")
+        worst[fn] = (float(u.max()), float(x[np.argmax(u)]))
+    for fn, (u, x) in worst.items():
+        assert u <= bound.get(fn, 2.0), (fn, u, x)
+    # ~2^-40 reciprocal used inside self-correcting iterations
+    x = np.exp(rng.uniform(-300, 300, M))
+    assert np.abs(run("rcp_nr1", x) * x - 1.0).max() < 2.0 ** -38
+    # clamps: exp_fast below -708 and exp_tab below -700 return the value at the clamp (finite, normal), never 0 or NaN
+    lo = np.array([-708.0, -709.0, -745.0, -1000.0, -1e300])
+    assert np.all(run("exp_fast", lo) == run("exp_fast", np.full(5, -708.0)))
+    lo = np.array([-700.0, -701.0, -745.0, -1000.0, -1e300])
+    assert np.all(run("exp_tab", lo) == run("exp_tab", np.full(5, -700.0)))
+    assert np.all(run("exp_tab", lo) > 2.2250738585072014e-308)
+    # sqrt_fast(0) = 0 exactly; rcp_fast(0) is documented as NaN (the kernels never divide by an exact zero)
+    assert run("sqrt_fast", np.zeros(3)).tolist() == [0.0, 0.0, 0.0]
+    assert np.all(np.isnan(run("rcp_fast", np.zeros(3))))
+
+
+MAX_ATTRIBUTED_MISSES = 3    # per 10^6 mixtures (configs 2-4): two-phase mixtures above 1e-8, each attributed (see adjudicate)
+
+
+def _full_size(oracle_mod, w, g, o, lnK0=None, flags=None, max_misses=MAX_ATTRIBUTED_MISSES, excuse=None):
+    """Invariants on every mixture + element-by-element oracle parity on every mixture (the oracle flashes ~1e6
+    mixtures per second on the box's host cores).  Misses above 1e-8 are adjudicated, listed and bounded."""
+    N = w.N
     assert set(np.unique(g["phase"])) <= {1, 2}
     two = g["phase"] == 2
-    assert 0.28 < two.mean() < 0.31
     b = g["beta"]
     assert np.all((b[two] > 0) & (b[two] < 1)) and np.all(np.isin(b[~two], (0.0, 1.0)))
     assert np.abs(w.z - b * g["y"] - (1 - b) * g["x"])[:, two].max() < 1e-10          # (1a)
-    assert np.abs(g["x"].sum(0) - 1).max() < 1e-9 and np.abs(g["y"].sum(0) - 1).max() < 1e-9   # (1b); worst case is a Newton finish with beta within 1e-5 of 0 or 1 (x = (z - nV)/(1 - beta))
+    # (1b); worst case is a Newton finish with beta within 1e-5 of 0 or 1 (x = (z - nV)/(1 - beta))
+    assert np.abs(g["x"].sum(0) - 1).max() < 1e-9 and np.abs(g["y"].sum(0) - 1).max() < 1e-9
     assert (g["status"] & 3).sum() == 0                                                   # no iteration cap hit
-    idx = np.sort(np.random.default_rng(5).choice(N, 30000, replace=False))
-    ws = W.Workload("sample", w.system, w.P[idx], w.T[idx], np.ascontiguousarray(w.z[:, idx]))
-    o = oracle_mod.Oracle.from_system(w.system).flash(ws.z, ws.P, ws.T)
-    gs = {k: (v[..., idx] if isinstance(v, np.ndarray) else v) for k, v in g.items()}
-    check(ws, gs, o)
+    rep = compare(w, g, o, excuse=excuse)
+    print({k: v for k, v in rep.items() if k not in ("messages", "bad", "band")})
+    for n in rep["band"]:
+        print(f"  in-band label mismatch n={n}: tpd_min oracle {o['tpd_min'][n]:.3e} gpu {g['tpd_min'][n]:.3e}")
+    assert rep["n_hard"] == 0, "\n".join(rep["messages"])
+    assert rep["in_band"] <= max(1, int(np.ceil(MAX_BAND_PER_MILLION * N / 1e6)))
+    assert rep["max_err_single"] == 0.0 and rep["beta_convention_mismatch"] == 0
+    rows = adjudicate(oracle_mod, w, g, o, rep["bad"], lnK0, flags)
+    for r in rows:
+        print("  miss above 1e-8:", r)
+    assert all(r["attributed"] != "BUG" for r in rows), "a miss above 1e-8 that neither the oracle's rounding nor conditioning explains"
+    assert len(rows) <= max_misses
+    rep["misses"] = rows
+    return rep
+
+
+@pytest.mark.parametrize("cfg,N", [(2, 1_000_000), (3, 1_000_000), (4, 1 << 20), (4, 1 << 22)])
+def test_full_size_parity(oracle_mod, cfg, N):
+    """BASELINE sizes (configs[1..3]; config 3 at 1e6 is the launch configuration bench.py times; at these sizes the
+    persistent Newton kernels refill their lanes ~40 times): EVERY mixture against the oracle."""
+    w = W.CONFIGS[cfg](N)
+    g = _gpu_flash(w, 1)
+    o = oracle_mod.Oracle.from_system(w.system).flash(w.z, w.P, w.T)
+    rep = _full_size(oracle_mod, w, g, o)
+    assert 0.10 < rep["two_phase"] / N < 0.35
+    assert (g["iters"] == o["iters"]).mean() > 0.98
+
+
+def test_full_size_config5_warm_and_cold(oracle_mod):
+    """BASELINE configs[4] at its stated size (1e6 mixtures within 5 % of their phase boundary; PTFLASH_TEST_CONFIG5_N
+    overrides): warm (caller lnK0 + skip-stability flags) and cold calls, every mixture against the oracle."""
+    import config5
+    N = int(os.environ.get("PTFLASH_TEST_CONFIG5_N", "1000000"))
+    orc = oracle_mod.Oracle.from_system(W.system_co2_10())
+    w, lnK0, flags, info = config5.build_cached(orc, N)
+    o_cold = info["cold"]
+    o_warm = orc.flash(w.z, w.P, w.T, lnK0=lnK0, flags=flags)
+    g_cold = _gpu_flash(w, 1)
+    g_warm = _gpu_flash(w, 1, lnK0=lnK0, flags=flags)
+    # every mixture of this workload is within 5 % of its phase boundary, where G is flat: more conditioning-limited misses
+    # than in configs 2-4 (each one adjudicated against the long double oracle and listed)
+    rc = _full_size(oracle_mod, w, g_cold, o_cold, max_misses=max(3, int(20e-6 * N)))
+    restarted, o_restarted = (g_warm["status"] & 64) != 0, (o_warm["status"] & 64) != 0
+    # Which hints fail is a property of the iteration path next to the boundary: both sides follow C21 and run the eta
+    # search of B.4a on hinted splits, so the sets agree up to borderline cases.  A mixture restarted on one side only is
+    # compared after the restart all the same (the cold answer); it is left out only if the LABELS differ, i.e. the hinted
+    # split found two phases on one side where the cold stability analysis (the other side) says single phase.
+    differ = restarted != o_restarted
+    assert differ.sum() <= max(3, 1e-5 * N)
+    excuse = differ & (g_warm["phase"] != o_warm["phase"])
+    assert excuse.sum() <= max(1, 2e-5 * N)
+    rw = _full_size(oracle_mod, w, g_warm, o_warm, lnK0, flags, max_misses=max(3, int(20e-6 * N)), excuse=excuse)
+    assert 0.4 < rc["two_phase"] / N < 0.6
+    two = (g_warm["phase"] == 2) & (g_cold["phase"] == 2)
+    print("config5 N=%d: two-phase %.3f, restarts gpu %d oracle %d; mean iters (two-phase) warm %.2f cold %.2f" %
+          (N, rc["two_phase"] / N, restarted.sum(), o_restarted.sum(), g_warm["iters"][two].mean(), g_cold["iters"][two].mean()))
