@@ -19,7 +19,7 @@ _LIBS = {"double": _HERE / "libptflash_oracle.so", "long double": _HERE / "libpt
 
 OPT_NAMES = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band",
              "probe_iters", "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters",
-             "use_newton", "ss_cap", "hint_ss_cap", "eta_growth", "eta_ratio", "split_trivial_tol"]
+             "use_newton", "ss_cap", "hint_ss_cap", "eta_growth", "eta_ratio", "split_trivial_tol", "stability_only"]
 
 
 def build(real: str = "double", force: bool = False) -> Path:
@@ -125,6 +125,23 @@ class Oracle:
         ok = self.lib.orc_rachford_rice(C.c_int(len(K)), _dp(K), _dp(z), C.byref(th))
         return (th.value if ok else None)
 
+    def rr_dtheta_dK(self, K, z, theta):
+        """Eq. 13: d theta / d K_i at a root (theta, K) of the Rachford-Rice equation."""
+        K, z = _f64(K), _f64(z)
+        out = np.zeros(len(K))
+        self.lib.orc_rr_dtheta_dK(C.c_int(len(K)), _dp(K), _dp(z), C.c_double(theta), _dp(out))
+        return out
+
+    def rr_batch(self, lnK, z):
+        """lnK, z [nc, N] -> dict(theta [N], x, y, dtheta_dK [nc, N], ok [N]); no window -> NaN, ok = 0."""
+        lnK, z = _f64(lnK), _f64(z)
+        nc, N = z.shape
+        out = dict(theta=np.empty(N), x=np.empty((nc, N)), y=np.empty((nc, N)), dtheta_dK=np.empty((nc, N)),
+                   ok=np.empty(N, dtype=np.int32))
+        self.lib.orc_rr_batch(C.c_int(nc), C.c_int64(N), _dp(lnK), _dp(z), _dp(out["theta"]), _dp(out["x"]), _dp(out["y"]),
+                              _dp(out["dtheta_dK"]), out["ok"].ctypes.data_as(C.POINTER(C.c_int32)))
+        return out
+
     def rr_f(self, K, z, theta):
         K, z = _f64(K), _f64(z)
         return self.lib.orc_rr_f(C.c_int(len(K)), _dp(K), _dp(z), C.c_double(theta))
@@ -159,7 +176,7 @@ class Oracle:
             phase=np.empty(N, dtype=np.int32), iters=np.empty(N, dtype=np.int32),
             tpd_min=np.empty(N), lnK=np.empty((nc, N)), status=np.empty(N, dtype=np.int32),
             stab_iters=np.empty(N, dtype=np.int32), probe_case=np.empty(N, dtype=np.int32),
-            diag=np.empty((3, N)), stage=np.empty((9, N), dtype=np.int32),
+            diag=np.empty((3, N)), stage=np.empty((13, N), dtype=np.int32), dbeta_dK=np.empty((nc, N)),
         )
         l0 = _f64(lnK0) if lnK0 is not None else None
         fl = np.ascontiguousarray(flags, dtype=np.uint8) if flags is not None else None
@@ -169,7 +186,7 @@ class Oracle:
             fl.ctypes.data_as(C.POINTER(C.c_uint8)) if fl is not None else None, _dp(self._opts(opts)),
             _dp(out["beta"]), _dp(out["x"]), _dp(out["y"]), ip(out["phase"]), ip(out["iters"]),
             _dp(out["tpd_min"]), _dp(out["lnK"]), ip(out["status"]), ip(out["stab_iters"]),
-            ip(out["probe_case"]), _dp(out["diag"]), ip(out["stage"]), C.c_int(nthreads))
+            ip(out["probe_case"]), _dp(out["diag"]), ip(out["stage"]), _dp(out["dbeta_dK"]), C.c_int(nthreads))
         out["threads"] = used
         return out
 

@@ -66,12 +66,14 @@ struct Opts {
                           //      (reading C22: a Newton iteration sliding into x = y "converges" -- its gradient vanishes
                           //      with |ln K| -- at |ln K| ~ 1e-8, theta ~ 1e-9; genuine solutions of the workloads have
                           //      max|ln K| > 3e-2)
+  double stability_only;  // [17] 1 = stop after the label (probe + stability analysis, no phase split): the mode the
+                          //      paper uses to label 10^6 samples for its classifier                  0
 };
 static Opts default_opts() {
-  Opts o = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 30, 8, 1.5, 1e-5};
+  Opts o = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 30, 8, 1.5, 1e-5, 0};
   return o;
 }
-#define NOPTS 17
+#define NOPTS 18
 static Opts opts_from(const double* p) {
   Opts o = default_opts();
   if (p) std::memcpy(&o, p, sizeof(double) * NOPTS);
@@ -318,6 +320,23 @@ static void phases_from_theta(int nc, const real* K, const real* z, real th, rea
     sx += x[i]; sy += y[i];
   }
   for (int i = 0; i < nc; ++i) { x[i] /= sx; y[i] /= sy; }
+}
+
+// d theta / d K_i at a root of f_RR by the implicit-function theorem, eq. 13 PAPER.md:281-286:
+//   d theta / d K = -[d f_RR / d theta]^-1 d f_RR / d K,  with f_RR of eq. 7 differentiated term by term:
+//   d f / d K_i = z_i / (1 + (K_i - 1) theta) - (K_i - 1) z_i theta / (1 + (K_i - 1) theta)^2,
+//   d f / d theta = - sum_i (K_i - 1)^2 z_i / (1 + (K_i - 1) theta)^2.        Components with z_i = 0 get 0 (C12).
+static void rr_dtheta_dK(int nc, const real* K, const real* z, real th, real* dth) {
+  real dfdth = 0;
+  for (int i = 0; i < nc; ++i)
+    if (z[i] > (real)0) { const real den = (real)1 + (K[i] - (real)1) * th; dfdth -= (K[i] - (real)1) * (K[i] - (real)1) * z[i] / (den * den); }
+  for (int i = 0; i < nc; ++i) {
+    if (z[i] > (real)0) {
+      const real den = (real)1 + (K[i] - (real)1) * th;
+      const real dfdK = z[i] / den - (K[i] - (real)1) * z[i] * th / (den * den);
+      dth[i] = -dfdK / dfdth;
+    } else dth[i] = 0;
+  }
 }
 
 static inline real xlnx_term(real c, real t) { return (c > (real)0) ? c * t : (real)0; }
@@ -714,8 +733,10 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
 struct FlashOut {
   int phase, iters, status, stab_iters, probe_case;
   real beta, x[MAXC], y[MAXC], lnK[MAXC], tpd_min, Zfeed, dc, rate;
+  real dbeta_dK[MAXC];   // eq. 13 at the reported (beta, K = y / x); NaN unless two phases
   // per-stage counts (the columns of the paper's profiler, Table 4), summed over a warm restart
   int stab_ss[2], stab_tr[2], stab_newton_trials, split_ss, split_tr, split_entered, split_newton;
+  int stab_entered_tr[2], stab_capped[2];   // per start: went on to the trust-region stage / hit an iteration cap
 };
 
 static void flash_one(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij,
@@ -726,7 +747,8 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
   out.beta = nan; out.tpd_min = nan; out.Zfeed = nan; out.dc = 0; out.rate = 0;
   out.stab_ss[0] = out.stab_ss[1] = out.stab_tr[0] = out.stab_tr[1] = 0;
   out.stab_newton_trials = out.split_ss = out.split_tr = out.split_entered = out.split_newton = 0;
-  for (int i = 0; i < nc; ++i) { out.x[i] = nan; out.y[i] = nan; out.lnK[i] = nan; }
+  out.stab_entered_tr[0] = out.stab_entered_tr[1] = out.stab_capped[0] = out.stab_capped[1] = 0;
+  for (int i = 0; i < nc; ++i) { out.x[i] = nan; out.y[i] = nan; out.lnK[i] = nan; out.dbeta_dK[i] = nan; }
   // O0 validate
   bool ok = std::isfinite((double)P) && std::isfinite((double)T) && P > (real)0 && T > (real)0;
   real sz = 0;
@@ -794,6 +816,8 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
       out.stab_iters = sv.ss_iters + sv.tr_iters + sl.ss_iters + sl.tr_iters;
       out.stab_ss[0] = sv.ss_iters; out.stab_ss[1] = sl.ss_iters; out.stab_tr[0] = sv.tr_iters; out.stab_tr[1] = sl.tr_iters;
       out.stab_newton_trials = (sv.entered_newton ? 1 : 0) + (sl.entered_newton ? 1 : 0);
+      out.stab_entered_tr[0] = sv.entered_newton ? 1 : 0; out.stab_entered_tr[1] = sl.entered_newton ? 1 : 0;
+      out.stab_capped[0] = sv.capped ? 1 : 0; out.stab_capped[1] = sl.capped ? 1 : 0;
       if (sv.capped || sl.capped) out.status |= ST_STAB_CAP;
       // O7 label
       tpd_min = 0;
@@ -812,6 +836,17 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
     unstable = true; tpd_min = nan; out.probe_case = 4;
   }
   out.tpd_min = tpd_min;
+
+  if (o.stability_only != 0) {
+    // Stability-only mode ("determine stability (no need for phase split calculations)"): the label of
+    // Fig. 2 up to the entry of the phase split.  phase = 2 means "unstable" (a split would be attempted), 1 "stable";
+    // x = y = z; beta is the single-phase convention for a stable feed and NaN for an unstable one (not computed);
+    // lnK is the K that would seed the split (probe iterate, or the stability trial's).
+    out.phase = unstable ? 2 : 1;
+    out.beta = unstable ? nan : ((Zf > (real)1 / (real)3) ? (real)1 : (real)0);
+    for (int i = 0; i < nc; ++i) { out.x[i] = z[i]; out.y[i] = z[i]; out.lnK[i] = unstable ? ((z[i] > (real)0) ? lnK[i] : (real)0) : (real)0; }
+    return;
+  }
 
   bool two = false;
   if (unstable) {
@@ -836,6 +871,10 @@ static void flash_one(int nc, const double* Tc, const double* Pc, const double* 
         out.beta = (real)1 - sp.theta;
         for (int i = 0; i < nc; ++i) { out.x[i] = sp.y[i]; out.y[i] = sp.x[i]; out.lnK[i] = -sp.lnK[i]; }
       }
+      // derivative output, eq. 13, at the reported solution (K = y / x solves f_RR(beta, K) = 0)
+      real Kr[MAXC];
+      for (int i = 0; i < nc; ++i) Kr[i] = (z[i] > (real)0) ? out.y[i] / out.x[i] : (real)1;
+      rr_dtheta_dK(nc, Kr, z, out.beta, out.dbeta_dK);
     } else if (!(sp.status & ST_SPLIT_FAILED)) out.status |= ST_SPLIT_FAILED;
   }
   if (!two && skip_stab) {
@@ -922,6 +961,32 @@ int orc_rachford_rice(int nc, const double* K, const double* z, double* theta) {
   *theta = (double)th;
   return ok ? 1 : 0;
 }
+// eq. 13: d theta / d K at (theta, K)
+void orc_rr_dtheta_dK(int nc, const double* K, const double* z, double theta, double* dth) {
+  real k[MAXC], zz[MAXC], d[MAXC];
+  for (int i = 0; i < nc; ++i) { k[i] = (real)K[i]; zz[i] = (real)z[i]; }
+  rr_dtheta_dK(nc, k, zz, (real)theta, d);
+  for (int i = 0; i < nc; ++i) dth[i] = (double)d[i];
+}
+// Batched Rachford-Rice (what the paper's initializer training calls): per mixture theta from (lnK, z),
+// x, y (eq. 7 / PAPER.md:83) and d theta / d K (eq. 13).  lnK, z, x, y, dth are [nc][N]; no window -> theta = NaN, ok = 0.
+void orc_rr_batch(int nc, int64_t N, const double* lnK, const double* z, double* theta, double* x, double* y, double* dth, int32_t* ok) {
+  const real nan = std::numeric_limits<real>::quiet_NaN();
+  for (int64_t n = 0; n < N; ++n) {
+    real k[MAXC], zz[MAXC], xx[MAXC], yy[MAXC], d[MAXC], th = nan, sz = 0;
+    for (int i = 0; i < nc; ++i) { k[i] = r_exp((real)lnK[(int64_t)i * N + n]); zz[i] = (real)z[(int64_t)i * N + n]; sz += zz[i]; }
+    for (int i = 0; i < nc; ++i) zz[i] /= sz;
+    const bool good = rachford_rice(nc, k, zz, &th);
+    if (good) { phases_from_theta(nc, k, zz, th, xx, yy); rr_dtheta_dK(nc, k, zz, th, d); }
+    theta[n] = good ? (double)th : (double)nan;
+    if (ok) ok[n] = good ? 1 : 0;
+    for (int i = 0; i < nc; ++i) {
+      if (x) x[(int64_t)i * N + n] = good ? (double)xx[i] : (double)nan;
+      if (y) y[(int64_t)i * N + n] = good ? (double)yy[i] : (double)nan;
+      if (dth) dth[(int64_t)i * N + n] = good ? (double)d[i] : (double)nan;
+    }
+  }
+}
 double orc_rr_f(int nc, const double* K, const double* z, double theta) {
   real k[MAXC], zz[MAXC];
   for (int i = 0; i < nc; ++i) { k[i] = (real)K[i]; zz[i] = (real)z[i]; }
@@ -970,7 +1035,7 @@ int orc_flash_batch(int nc, const double* Tc, const double* Pc, const double* om
                     const double* lnK0, const uint8_t* flags, const double* opts,
                     double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
                     double* out_tpd_min, double* out_lnK, int32_t* out_status, int32_t* out_stab_iters,
-                    int32_t* out_probe_case, double* out_diag, int32_t* out_stage, int nthreads) {
+                    int32_t* out_probe_case, double* out_diag, int32_t* out_stage, double* out_dbeta_dK, int nthreads) {
   Opts o = opts_from(opts);
   int used = 1;
 #ifdef _OPENMP
@@ -994,10 +1059,11 @@ int orc_flash_batch(int nc, const double* Tc, const double* Pc, const double* om
     if (out_probe_case) out_probe_case[n] = fo.probe_case;
     if (out_diag) { out_diag[n] = (double)fo.Zfeed; out_diag[N + n] = (double)fo.dc; out_diag[2 * N + n] = (double)fo.rate; }
     if (out_stage) {
-      const int v[9] = {fo.stab_ss[0], fo.stab_ss[1], fo.stab_tr[0], fo.stab_tr[1], fo.stab_newton_trials, fo.split_ss, fo.split_tr,
-                        fo.split_entered, fo.split_newton};
-      for (int k = 0; k < 9; ++k) out_stage[(int64_t)k * N + n] = v[k];
+      const int v[13] = {fo.stab_ss[0], fo.stab_ss[1], fo.stab_tr[0], fo.stab_tr[1], fo.stab_newton_trials, fo.split_ss, fo.split_tr,
+                         fo.split_entered, fo.split_newton, fo.stab_entered_tr[0], fo.stab_entered_tr[1], fo.stab_capped[0], fo.stab_capped[1]};
+      for (int k = 0; k < 13; ++k) out_stage[(int64_t)k * N + n] = v[k];
     }
+    if (out_dbeta_dK) for (int i = 0; i < nc; ++i) out_dbeta_dK[(int64_t)i * N + n] = (double)fo.dbeta_dK[i];
   }
   return used;
 }

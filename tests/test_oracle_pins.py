@@ -571,3 +571,163 @@ def test_path_sensitivity_set(sys10):
     for n in uns:
         tpd, neg, ns = S.adjudicate(sys10, w.P[n], w.T[n], w.z[:, n])
         assert neg >= 1 and tpd <= base["tpd_min"][n] + 1e-10
+
+
+# ------------------------------------------------------------------------------------------------
+# eq. 13: d theta / d K by the implicit-function theorem
+# ------------------------------------------------------------------------------------------------
+def test_rr_derivative_binary_closed_form(sys2):
+    # binary: f_RR = 0 has the closed-form root theta = -(z1 (K1-1) + z2 (K2-1)) / ((K1-1)(K2-1)); differentiate it by hand
+    for K1, K2, z1 in [(3.0, 0.2, 0.4), (1.5, 0.6, 0.5), (12.0, 0.01, 0.3)]:
+        z2 = 1.0 - z1
+        a, b = K1 - 1.0, K2 - 1.0
+        th = -(z1 * a + z2 * b) / (a * b)
+        d1 = -z1 / (a * b) + (z1 * a + z2 * b) / (a * a * b)     # d theta / d K1
+        d2 = -z2 / (a * b) + (z1 * a + z2 * b) / (a * b * b)     # d theta / d K2
+        got = sys2.rr_dtheta_dK([K1, K2], [z1, z2], th)
+        assert np.allclose(got, [d1, d2], rtol=1e-13, atol=0)
+
+
+def test_rr_derivative_matches_finite_differences_of_the_solver(sys10):
+    # the derivative of the SOLVER's root (bisection to rounding) by central differences: pins sign, index and the
+    # [d f / d theta]^-1 factor of eq. 13 against the definition of theta(K) itself
+    rng = np.random.default_rng(13)
+    for _ in range(20):
+        z = rng.dirichlet(np.ones(10))
+        lnK = rng.normal(0.0, 1.5, 10)
+        K = np.exp(lnK)
+        th = sys10.rachford_rice(K, z)
+        if th is None:
+            continue
+        got = sys10.rr_dtheta_dK(K, z, th)
+        for i in range(10):
+            h = 1e-6 * K[i]
+            Kp, Km = K.copy(), K.copy()
+            Kp[i] += h
+            Km[i] -= h
+            fd = (sys10.rachford_rice(Kp, z) - sys10.rachford_rice(Km, z)) / (2 * h)
+            assert abs(got[i] - fd) <= 1e-6 * max(1.0, abs(fd)), (i, got[i], fd)
+    # a z_i = 0 component does not move theta (C12)
+    z = np.array([0.5, 0.5, 0, 0, 0, 0, 0, 0, 0, 0.0])
+    K = np.array([2.0, 0.5, 7, 7, 7, 7, 7, 7, 7, 7.0])
+    d = sys10.rr_dtheta_dK(K, z, sys10.rachford_rice(K, z))
+    assert np.all(d[2:] == 0.0) and d[0] > 0 and d[1] > 0      # theta grows with every K_i (f_RR grows with K_i, falls with theta)
+
+
+def test_rr_batch_and_flash_derivative_output(oracle_mod, sys10):
+    w = W.config3(3000)
+    o = sys10.flash(w.z, w.P, w.T)
+    two = o["phase"] == 2
+    assert two.sum() > 500
+    # the flash's derivative output is eq. 13 at its own reported (beta, K = y/x): re-evaluate through the scalar entry,
+    # and check it against the batched Rachford-Rice solve started from the reported ln K
+    rb = sys10.rr_batch(o["lnK"][:, two], w.z[:, two])
+    assert np.all(rb["ok"] == 1)
+    assert np.abs(rb["theta"] - o["beta"][two]).max() < 1e-9
+    assert np.abs(rb["x"] - o["x"][:, two]).max() < 1e-9 and np.abs(rb["y"] - o["y"][:, two]).max() < 1e-9
+    d = o["dbeta_dK"][:, two]
+    assert np.all(np.isfinite(d)) and np.all(d >= 0)
+    assert np.allclose(rb["dtheta_dK"], d, rtol=1e-6, atol=1e-12)
+    assert np.all(np.isnan(o["dbeta_dK"][:, ~two]))
+    # no window -> NaN and ok = 0
+    lnK = np.full((10, 4), 0.3)
+    rb = sys10.rr_batch(lnK, w.z[:, :4])
+    assert np.all(rb["ok"] == 0) and np.all(np.isnan(rb["theta"]))
+
+
+# ------------------------------------------------------------------------------------------------
+# stability-only mode and the Table-4 counters
+# ------------------------------------------------------------------------------------------------
+def test_stability_only_mode_is_the_label_of_the_full_flash(sys10):
+    w = W.config3(4000)
+    full = sys10.flash(w.z, w.P, w.T)
+    so = sys10.flash(w.z, w.P, w.T, opts={"stability_only": 1})
+    # "unstable" in stability-only mode <=> the full flash entered the phase split (it ends two-phase unless the split
+    # failed, which the full flash reports with status bit 8)
+    entered = full["stage"][7] > 0
+    assert np.array_equal(so["phase"] == 2, entered)
+    failed = (full["status"] & 8) != 0
+    assert np.array_equal(full["phase"] == 2, entered & ~failed)
+    assert np.array_equal(so["tpd_min"], full["tpd_min"], equal_nan=True)
+    assert np.array_equal(so["stab_iters"], full["stab_iters"]) and np.array_equal(so["probe_case"], full["probe_case"])
+    assert np.array_equal(so["x"], w.z / w.z.sum(0)) and np.array_equal(so["y"], so["x"])
+    assert np.all(np.isnan(so["beta"][so["phase"] == 2])) and np.all(np.isin(so["beta"][so["phase"] == 1], (0.0, 1.0)))
+    assert np.all(so["iters"] <= 3) and np.all(so["stage"][5:9] == 0)        # no split work at all
+    # the K seed of an unstable mixture starts a split that reaches the full flash's answer
+    n = int(np.nonzero((so["phase"] == 2) & (full["phase"] == 2))[0][0])
+    sp = sys10.phase_split(w.P[n], w.T[n], so["x"][:, n], so["lnK"][:, n])
+    assert sp["two_phase"] and abs(min(sp["theta"], 1 - sp["theta"]) - min(full["beta"][n], 1 - full["beta"][n])) < 1e-9
+
+
+def test_stage_counters_are_consistent(sys10):
+    w = W.config3(4000)
+    o = sys10.flash(w.z, w.P, w.T)
+    st, pc = o["stage"], o["probe_case"]
+    went = (pc == 1) | (pc == 2)
+    assert np.array_equal(o["stab_iters"], st[0] + st[1] + st[2] + st[3])
+    assert np.array_equal(st[4], st[9] + st[10])                               # trials that entered the trust-region stage
+    assert np.all((st[0] + st[1] > 0) == went) and np.all(st[0:4, ~went] == 0)
+    assert np.all(st[0] <= 9) and np.all(st[1] <= 9)                            # SS cap of PAPER.md:79
+    assert np.all(st[2][st[9] == 0] == 0) and np.all(st[3][st[10] == 0] == 0)   # no trust-region iterations without entering
+    assert np.all(st[11:13] == 0) and np.all((o["status"] & 1) == 0)            # nothing capped on this workload
+    assert np.array_equal(st[7] > 0, (pc == 3) | (went & (o["tpd_min"] < 0)))
+
+
+# ------------------------------------------------------------------------------------------------
+# the paper's own case studies (section 2.3-2.4, Tables 1-3, D.6)
+# ------------------------------------------------------------------------------------------------
+def test_paper_workloads_follow_tables_1_to_3():
+    s = W.system_paper9()
+    assert s.names[0] == "CH4" and s.nc == 9
+    assert s.Pc[0] == 4.6 and s.Tc[6] == 604.5 and s.omega[8] == 0.039          # Table 1 PAPER.md:121-129 (MPa, K)
+    k = s.kij.copy()
+    assert k[0, 7] == 0.0882 == k[7, 0]
+    k[0, 7] = k[7, 0] = 0.0
+    assert not k.any()
+    w = W.paper9(8000)
+    assert np.all((w.P > 5) & (w.P < 25)) and np.all((w.T > 200) & (w.T < 600)) and np.allclose(w.z.sum(0), 1, atol=1e-14)
+    for t, kind in enumerate(W.PAPER_FLUIDS):
+        z = w.z[:, t::4]
+        for i, (lo, hi) in enumerate(W.PAPER_FLUID_RANGES[kind]):                # Table 2
+            assert np.all(z[i] >= lo - 1e-12) and np.all(z[i] <= hi + 1e-12), (kind, i)
+        # Appendix D's typical composition of the type lies inside the type's ranges (consistency of Tables 2 and D.6)
+        for i, (lo, hi) in enumerate(W.PAPER_FLUID_RANGES[kind]):
+            assert lo - 1e-12 <= W.PAPER_TYPICAL[kind][i] <= hi + 5e-4, (kind, i)
+    acc = W.paper9(40000).meta["acceptance"]
+    assert acc["wet_gas"] > acc["volatile_oil"] > acc["gas_condensate"] > acc["black_oil"] > 5e-4
+    # prefix / offset property
+    assert np.array_equal(W.paper9(300, offset=500).z, w.z[:, 500:800])
+    for name, nc in (("paper2", 2), ("paper4", 4)):
+        v = W.CONFIGS[name](2000)
+        assert v.system.nc == nc and np.all((v.P > 0.1) & (v.P < 10)) and np.all((v.T > 200) & (v.T < 500))
+        assert np.allclose(v.z.sum(0), 1, atol=1e-14) and not v.system.kij.any()
+
+
+@pytest.mark.parametrize("name,N", [("paper2", 3000), ("paper4", 3000), ("paper9", 4000)])
+def test_flash_invariants_on_paper_workloads(oracle_mod, name, N):
+    w = W.CONFIGS[name](N)
+    orc = oracle_mod.Oracle.from_system(w.system)
+    o = orc.flash(w.z, w.P, w.T)
+    two = o["phase"] == 2
+    assert 0.05 < two.mean() < 0.8
+    b, x, y = o["beta"][two], o["x"][:, two], o["y"][:, two]
+    assert np.all((b > 0) & (b < 1))
+    assert np.abs(b * y + (1 - b) * x - w.z[:, two]).max() < 1e-12               # (1a)
+    assert np.abs(x.sum(0) - 1).max() < 1e-12 and np.abs(y.sum(0) - 1).max() < 1e-12   # (1b)
+    idx = np.nonzero(two)[0][:: max(1, two.sum() // 60)]
+    for n in idx:                                                               # (2) iso-fugacity
+        lx, Zx = orc.lnphi(w.P[n], w.T[n], o["x"][:, n])
+        ly, Zy = orc.lnphi(w.P[n], w.T[n], o["y"][:, n])
+        assert np.abs(np.log(o["x"][:, n]) + lx - np.log(o["y"][:, n]) - ly).max() < 1e-8
+        assert Zy >= Zx
+    if name == "paper9":
+        # Table 4's shape (SURVEY.md section 4 says the absolute shares are NOT a pin): the probe proves
+        # a large share unstable, and a minority of the stability trials needs the trust-region stage
+        assert 0.2 < (o["probe_case"] == 3).mean() < 0.5
+        # pressure in MPa with Pc in MPa == pressure in bar with Pc in bar (the gas constant cancels)
+        s = w.system
+        orc_bar = oracle_mod.Oracle(s.Tc, s.Pc * 10.0, s.omega, s.kij)
+        o2 = orc_bar.flash(w.z[:, :500], w.P[:500] * 10.0, w.T[:500])
+        assert np.array_equal(o2["phase"], o["phase"][:500])
+        t2 = o2["phase"] == 2
+        assert np.abs(o2["beta"][t2] - o["beta"][:500][t2]).max() < 1e-9
