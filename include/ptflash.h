@@ -99,12 +99,18 @@ typedef struct ptflash_io {
   double* out_lnK;           /* optional out [nc][N]: converged ln K (0 for single phase) */
   int32_t* out_status;       /* optional out [N]: PTFLASH_ST_* bits */
   int32_t* out_stab_iters;   /* optional out [N]: stability iterations (SS + Newton, both starts) */
+  double* out_dbeta_dK;      /* optional out [nc][N]: d beta / d K_i at the reported solution (K = y / x), by the implicit-function
+                                formula of eq. 13: -[d f_RR / d beta]^-1 d f_RR / d K_i; 0 for a z_i = 0
+                                component; NaN unless out_phase == 2 */
 } ptflash_io_t;
 int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream);
 
-/* End-to-end variant with HOST buffers (same meaning and layout as ptflash_flash; pinned memory recommended):
- * copies inputs host->device, runs the flash, copies results device->host on `stream`, then synchronises.
- * Staging buffers belong to the handle. */
+/* End-to-end variant with HOST buffers (same meaning and layout as ptflash_flash; pinned memory needed for the copies to be
+ * asynchronous): the batch is cut into PTFLASH_OPT_HOST_CHUNKS chunks of consecutive mixtures, each copied host->device,
+ * flashed and copied back device->host on an internal stream of its own (strided slices of the SoA arrays), so that the
+ * transfers of one chunk overlap the kernels of the others; all of it starts after the work already queued on `stream`,
+ * and the call returns after everything has completed (it synchronises).  Staging buffers, the chunks' workspaces and
+ * streams belong to the handle; ptflash_get_stats then reports the sums over the chunks. */
 int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T,
                        double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
                        void* stream);
@@ -134,12 +140,31 @@ enum {
   PTFLASH_OPT_STAGE_PROFILE = 14,  /* [0] 1 = record a CUDA event between the stage kernels (engine 1), see ptflash_get_stage_ms */
   PTFLASH_OPT_TOL_NEWTON_STEP_STAB = 15, /* the same for the stability Newton, whose result enters only through tm (itself
                                             second order in the error of W) and the K seed [1e-6] */
-  PTFLASH_OPT_HINT_SS_CAP = 16,    /* [30] a PTFLASH_FLAG_SKIP_STABILITY split whose successive substitution is still outside
+  PTFLASH_OPT_HINT_SS_CAP = 16,    /* [12] a PTFLASH_FLAG_SKIP_STABILITY split whose successive substitution is still outside
                                       0 < theta < 1 after this many iterations is dropped and the mixture re-flashed from
                                       Wilson (PTFLASH_ST_WARM_RESTART; reading C21) */
   PTFLASH_OPT_SPLIT_TRIVIAL_TOL = 17, /* [1e-5] the phase split has collapsed into the trivial solution x = y when max_i |ln K_i| < tol
                                       (-> PTFLASH_ST_SPLIT_FAILED, or a warm restart); reading C22 */
-  PTFLASH_NUM_OPTS = 18
+  PTFLASH_OPT_STABILITY_ONLY = 18, /* [0] 1 = stop after the label: probe + stability analysis, no phase split -- the mode the paper
+                                      uses to label 10^6 samples for its classifier.  out_phase = 1 stable / 2
+                                      unstable; x = y = z; out_beta = the single-phase convention for a stable feed, NaN for an
+                                      unstable one; out_lnK = the K that would seed the split; out_tpd_min as usual;
+                                      a PTFLASH_FLAG_SKIP_STABILITY mixture is reported unstable without any work */
+  PTFLASH_OPT_HOST_CHUNKS = 19,    /* [8] ptflash_flash_host cuts the batch into at most this many chunks (1..8, none below 32768
+                                      mixtures), each on a stream of its own, so that the PCIe copies of one chunk overlap the
+                                      kernels of the others */
+  PTFLASH_OPT_HINT_ETA_SEARCH = 20, /* [0] 0 = a split entered through PTFLASH_FLAG_SKIP_STABILITY takes the truncated
+                                      modified-Cholesky step of every other split (one factorisation per trust-region iteration);
+                                      1 = it takes the restricted step of B.4a by the eta search, the oracle's path, so that the
+                                      SAME hints fail and PTFLASH_ST_WARM_RESTART agrees with the oracle mixture by mixture (with
+                                      0 the answers are the same, but ~2 hints per 1000 mixtures next to the phase boundary fail
+                                      or survive differently: which hints fail is a property of the iteration path); costs
+                                      1.4x on the warm-start workload */
+  PTFLASH_OPT_HINT_TR_CAP = 21,    /* [15] a PTFLASH_FLAG_SKIP_STABILITY split that has not converged after this many trust-region
+                                      iterations is dropped and the mixture re-flashed from Wilson (PTFLASH_ST_WARM_RESTART;
+                                      DESIGN.md reading C21): converging hinted splits of the warm-start workload need <= 11, failing
+                                      ones wander until the cap */
+  PTFLASH_NUM_OPTS = 22
 };
 int ptflash_set_option(ptflash_handle_t h, int key, double value);
 int ptflash_get_option(ptflash_handle_t h, int key, double* value);
@@ -155,13 +180,38 @@ typedef struct ptflash_stats {
   int64_t n_split_newton;   /* phase splits that needed the trust-region stage */
   int64_t n_two_phase;
   int64_t kernel_launches;  /* kernels launched by the last call */
+  /* The remaining columns of Table 4; index [0] = vapour-like start, [1] = liquid-like start.
+   * "# of samples": ss stages n_stability (each start) and n_split, tr stages n_stab_tr[] and n_split_newton.
+   * "Convergence": a stability trial / phase split that does not go on to the trust-region stage ended within the SS
+   * cap (n_stability - n_stab_tr[k], n_split - n_split_newton); a trust-region stage converged unless it hit its cap
+   * (n_stab_capped[k], n_split_capped); the probe's figure is n_probe_case3 / n_total (footnote 1 of Table 4).
+   * "Max number of iterations": the max_* fields. */
+  int64_t n_stab_tr[2];      /* stability trials that went on to the trust-region stage, per start (sum = n_stab_newton) */
+  int64_t n_stab_capped[2];  /* stability trials that hit an iteration cap, per start */
+  int64_t n_split_capped;    /* phase splits that hit an iteration cap */
+  int64_t n_warm_restarts;   /* PTFLASH_FLAG_SKIP_STABILITY hints that failed and were re-flashed cold (PTFLASH_ST_WARM_RESTART) */
+  int32_t max_probe_iters, max_stab_ss_iters[2], max_stab_tr_iters[2], max_split_ss_iters, max_split_tr_iters;
+  int32_t reserved_;
 } ptflash_stats_t;
 int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out);
 
+/* Batched Rachford-Rice solve with its derivative -- what the paper's initializer training evaluates for every sample
+ * (PAPER.md:279-286): theta from (K, z) by eq. 7 (solver of App. C: Newton on h_RR inside a
+ * shrinking sign bracket on (alpha_l, alpha_r), negative flash allowed), x_i = z_i / (1 + (K_i - 1) theta), y_i = K_i x_i
+ * (normalised), and d theta / d K_i = -[d f_RR / d theta]^-1 d f_RR / d K_i (eq. 13) at the solution.
+ *   lnK, z [nc][N]      DEVICE inputs (ln K so that the caller's network output is used as is; z is normalised internally)
+ *   out_theta [N]       DEVICE; NaN where there is no window (all K_i >= 1 or all <= 1 over the z_i > 0 components) or the
+ *                       input is invalid (non-finite, z_i < 0, |ln K_i| > 700 -- cf. the overflow reported at PAPER.md:363)
+ *   out_x, out_y, out_dtheta_dK [nc][N]   DEVICE, each may be NULL; NaN where out_theta is NaN; 0 derivative for z_i = 0
+ * Asynchronous on `stream`; the caller owns all buffers.  Returns PTFLASH_OK / EINVAL / ECUDA. */
+int ptflash_rachford_rice(ptflash_handle_t h, int64_t N, const double* lnK, const double* z, double* out_theta,
+                          double* out_x, double* out_y, double* out_dtheta_dK, void* stream);
+
 /* Stage times of the last call made with PTFLASH_OPT_STAGE_PROFILE = 1 (engine 1), measured with CUDA events recorded
  * on the call's stream between the stage kernels -- the per-stage "time" row of the paper's profiler (Table 4
- * PAPER.md:332-345).  Order (first pass): init, probe, stab_ss, stab_newton, stab_decide, split_ss, split_newton;
- * a second pass (warm restarts) appends its six stages.  Writes up to `cap` values (milliseconds) to HOST array `ms`,
+ * PAPER.md:332-345).  Order: init, probe, stab_ss, stab_newton, stab_decide, split_ss, split_newton; a call with
+ * PTFLASH_FLAG_* flags inserts three stages after init -- split_ss and split_newton of the hinted mixtures, and the re-queueing
+ * of the failed hints -- so that the hints that fail take the cold path in the same pass.  Writes up to `cap` values (milliseconds) to HOST array `ms`,
  * returns the number written (0 if profiling was off), or PTFLASH_EINVAL / PTFLASH_ECUDA.  Synchronises the stream. */
 #define PTFLASH_NUM_STAGES 7
 int ptflash_get_stage_ms(ptflash_handle_t h, float* ms, int cap);

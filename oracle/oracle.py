@@ -19,7 +19,7 @@ _LIBS = {"double": _HERE / "libptflash_oracle.so", "long double": _HERE / "libpt
 
 OPT_NAMES = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band",
              "probe_iters", "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters",
-             "use_newton", "ss_cap", "hint_ss_cap", "eta_growth", "eta_ratio", "split_trivial_tol", "stability_only"]
+             "use_newton", "ss_cap", "hint_ss_cap", "eta_growth", "eta_ratio", "split_trivial_tol", "stability_only", "hint_tr_cap"]
 
 
 def build(real: str = "double", force: bool = False) -> Path:

@@ -58,7 +58,7 @@ struct Opts {
   double use_newton;      // [11] 1; 0 = pure successive substitution everywhere (used by pins)
   double ss_cap;          // [12] cap on SS iterations when use_newton == 0                               100000
   double hint_ss_cap;     // [13] a skip-stability hint whose split SS is still outside 0 < theta < 1 after this
-                          //      many iterations is dropped (reading C21)                  30
+                          //      many iterations is dropped (reading C21)                  12
   double eta_growth;      // [14] restricted step (C11): geometric growth factor of eta                            8
   double eta_ratio;       // [15] restricted step (C11): the bisection of eta stops at this bracket ratio          1.5
                           //      ([14], [15] exist so that tests/oracle_path_sensitivity.py can perturb the schedule)
@@ -68,12 +68,15 @@ struct Opts {
                           //      max|ln K| > 3e-2)
   double stability_only;  // [17] 1 = stop after the label (probe + stability analysis, no phase split): the mode the
                           //      paper uses to label 10^6 samples for its classifier                  0
+  double hint_tr_cap;     // [18] a skip-stability hint whose split has not converged after this many trust-region iterations
+                          //      is dropped (reading C21: on the warm-start workload converging hinted splits need at most
+                          //      11, failing ones wander until the cap)                                                   15
 };
 static Opts default_opts() {
-  Opts o = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 30, 8, 1.5, 1e-5, 0};
+  Opts o = {1e-10, 1e-12, 1e-10, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 12, 8, 1.5, 1e-5, 0, 15};
   return o;
 }
-#define NOPTS 18
+#define NOPTS 19
 static Opts opts_from(const double* p) {
   Opts o = default_opts();
   if (p) std::memcpy(&o, p, sizeof(double) * NOPTS);
@@ -650,7 +653,7 @@ static void phase_split(const Setup& s, const real* z, const real* lnK_in, const
     };
     eval();
     real Delta = (real)0.25;   // n^V lives in the box (0, z), |n^V| < 1; Delta is capped at 1 (C11)
-    const int kmax = (int)o.split_tr_iters;
+    const int kmax = hinted ? std::min((int)o.split_tr_iters, (int)o.hint_tr_cap) : (int)o.split_tr_iters;   // C21
     for (int it = 0; it < kmax; ++it) {
       // Reading C8: the gradient test does not end the iteration by itself.  Near a critical point (d_c -> 0, eq. 14
       // PAPER.md:318) and next to the phase boundary the Hessian is nearly singular, so a gradient below 1e-12 does not

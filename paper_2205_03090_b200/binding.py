@@ -17,10 +17,10 @@ PTFLASH_OK, PTFLASH_EINVAL, PTFLASH_ECUDA = 0, -1, -2
 ST_STAB_CAP, ST_SPLIT_CAP, ST_BAND, ST_SPLIT_FAILED, ST_LNK0_REJECTED = 1, 2, 4, 8, 32
 FLAG_SKIP_STABILITY, FLAG_USE_LNK0 = 1, 2
 OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band", "probe_iters",
-           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol"]
+           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol", "stability_only", "host_chunks", "hint_eta_search", "hint_tr_cap"]
 EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
            "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_get_stage_ms", "ptflash_fp64_peak",
-           "ptflash_last_error", "ptflash_version", "ptflash_math_probe"]
+           "ptflash_last_error", "ptflash_version", "ptflash_math_probe", "ptflash_rachford_rice"]
 
 
 class PTFlashError(RuntimeError):
@@ -31,16 +31,26 @@ class _Io(C.Structure):
     _fields_ = [("N", C.c_int64), ("z", C.c_void_p), ("P", C.c_void_p), ("T", C.c_void_p), ("lnK0", C.c_void_p),
                 ("flags", C.c_void_p), ("out_beta", C.c_void_p), ("out_x", C.c_void_p), ("out_y", C.c_void_p),
                 ("out_phase", C.c_void_p), ("out_iters", C.c_void_p), ("out_tpd_min", C.c_void_p),
-                ("out_lnK", C.c_void_p), ("out_status", C.c_void_p), ("out_stab_iters", C.c_void_p)]
+                ("out_lnK", C.c_void_p), ("out_status", C.c_void_p), ("out_stab_iters", C.c_void_p),
+                ("out_dbeta_dK", C.c_void_p)]
 
 
 class Stats(C.Structure):
-    _fields_ = [(k, C.c_int64) for k in ("n_total", "n_invalid", "n_probe_case1", "n_probe_case2", "n_probe_case3",
-                                         "n_stability", "n_stab_newton", "n_split", "n_split_newton", "n_two_phase",
-                                         "kernel_launches")]
+    _fields_ = ([(k, C.c_int64) for k in ("n_total", "n_invalid", "n_probe_case1", "n_probe_case2", "n_probe_case3",
+                                          "n_stability", "n_stab_newton", "n_split", "n_split_newton", "n_two_phase",
+                                          "kernel_launches")]
+                + [("n_stab_tr", C.c_int64 * 2), ("n_stab_capped", C.c_int64 * 2), ("n_split_capped", C.c_int64),
+                   ("n_warm_restarts", C.c_int64), ("max_probe_iters", C.c_int32), ("max_stab_ss_iters", C.c_int32 * 2),
+                   ("max_stab_tr_iters", C.c_int32 * 2), ("max_split_ss_iters", C.c_int32), ("max_split_tr_iters", C.c_int32),
+                   ("reserved_", C.c_int32)])
 
     def as_dict(self):
-        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+        d = {}
+        for k, _ in self._fields_:
+            v = getattr(self, k)
+            if k != "reserved_":
+                d[k] = int(v) if isinstance(v, int) else [int(e) for e in v]
+        return d
 
 
 def load_library():
@@ -75,6 +85,8 @@ def load_library():
     L.ptflash_fp64_peak.argtypes = [C.c_int, dp, dp, vp]
     L.ptflash_math_probe.restype = C.c_int
     L.ptflash_math_probe.argtypes = [C.c_int, i64, vp, vp, vp]
+    L.ptflash_rachford_rice.restype = C.c_int
+    L.ptflash_rachford_rice.argtypes = [vp, i64] + [vp] * 7
     L.ptflash_last_error.restype = C.c_char_p
     L.ptflash_version.restype = C.c_char_p
     _lib = L
@@ -128,10 +140,10 @@ def ptflash_flash(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=No
 
 
 def ptflash_flash_ex(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=None, lnK0=None, flags=None,
-                     out_tpd_min=None, out_lnK=None, out_status=None, out_stab_iters=None, stream=None):
+                     out_tpd_min=None, out_lnK=None, out_status=None, out_stab_iters=None, out_dbeta_dK=None, stream=None):
     io = _Io(int(N), *[(_ptr(t).value if t is not None else None) for t in
                        (z, P, T, lnK0, flags, out_beta, out_x, out_y, out_phase, out_iters, out_tpd_min, out_lnK,
-                        out_status, out_stab_iters)])
+                        out_status, out_stab_iters, out_dbeta_dK)])
     _check(load_library().ptflash_flash_ex(h, C.byref(io), _stream(stream)), "ptflash_flash_ex")
 
 
@@ -139,6 +151,11 @@ def ptflash_flash_host(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_ite
     _check(load_library().ptflash_flash_host(h, int(N), _ptr(z), _ptr(P), _ptr(T), _ptr(out_beta), _ptr(out_x),
                                              _ptr(out_y), _ptr(out_phase), _ptr(out_iters), _stream(stream)),
            "ptflash_flash_host")
+
+
+def ptflash_rachford_rice(h, N, lnK, z, out_theta, out_x=None, out_y=None, out_dtheta_dK=None, stream=None):
+    _check(load_library().ptflash_rachford_rice(h, int(N), _ptr(lnK), _ptr(z), _ptr(out_theta), _ptr(out_x), _ptr(out_y),
+                                                _ptr(out_dtheta_dK), _stream(stream)), "ptflash_rachford_rice")
 
 
 def ptflash_destroy(h):
@@ -218,6 +235,17 @@ class PTFlash:
     def stage_ms(self):
         return ptflash_get_stage_ms(self.h)
 
+    def rachford_rice(self, lnK, z, stream=None):
+        """lnK, z [nc, N] CUDA float64 -> dict(theta [N], x, y, dtheta_dK [nc, N])."""
+        import torch
+        assert z.is_cuda and z.dtype == torch.float64 and z.shape[0] == self.nc and lnK.shape == z.shape
+        N = z.shape[1]
+        f64 = dict(dtype=torch.float64, device=z.device)
+        out = dict(theta=torch.empty(N, **f64), x=torch.empty(self.nc, N, **f64), y=torch.empty(self.nc, N, **f64),
+                   dtheta_dK=torch.empty(self.nc, N, **f64))
+        ptflash_rachford_rice(self.h, N, lnK, z, out["theta"], out["x"], out["y"], out["dtheta_dK"], stream=stream)
+        return out
+
     def flash(self, z, P, T, lnK0=None, flags=None, extended=True, stream=None):
         """z [nc, N], P [N], T [N]: CUDA float64 tensors -> dict of CUDA tensors."""
         import torch
@@ -230,10 +258,11 @@ class PTFlash:
                    phase=torch.empty(N, **i32), iters=torch.empty(N, **i32))
         if extended:
             out.update(tpd_min=torch.empty(N, **f64), lnK=torch.empty(self.nc, N, **f64),
-                       status=torch.empty(N, **i32), stab_iters=torch.empty(N, **i32))
+                       status=torch.empty(N, **i32), stab_iters=torch.empty(N, **i32), dbeta_dK=torch.empty(self.nc, N, **f64))
             ptflash_flash_ex(self.h, N, z, P, T, out["beta"], out["x"], out["y"], out["phase"], out["iters"],
                              lnK0=lnK0, flags=flags, out_tpd_min=out["tpd_min"], out_lnK=out["lnK"],
-                             out_status=out["status"], out_stab_iters=out["stab_iters"], stream=stream)
+                             out_status=out["status"], out_stab_iters=out["stab_iters"], out_dbeta_dK=out["dbeta_dK"],
+                             stream=stream)
         else:
             ptflash_flash(self.h, N, z, P, T, out["beta"], out["x"], out["y"], out["phase"], out["iters"], stream=stream)
         return out

@@ -2,6 +2,7 @@
 // workspace ownership, option table, host-buffer variant and the FP64 roofline probe.  No torch types,
 // no CPU fallback: every numerical step runs in the kernels of ptflash_nc.cu.
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -12,6 +13,7 @@
 
 namespace {
 
+#define PTF_MAX_HOST_CHUNKS 8
 thread_local std::string g_err;
 void set_err(const std::string& s) { g_err = s; }
 bool cuda_ok(cudaError_t e, const char* what) {
@@ -20,7 +22,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 
-const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 30, 1e-5};
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 12, 1e-5, 0, 8, 0, 15};
 
 }  // namespace
 
@@ -49,6 +51,15 @@ struct ptflash_handle_s {
   cudaEvent_t ev_fork, ev_join;
   bool aux_made;
   int cta_cache[4];   // resident CTAs per SM of the persistent kernels on this handle's device (0 = not queried yet)
+  // ptflash_flash_host pipeline: child handles (same component system, own workspace / streams / counters), one per chunk
+  // in flight, each with a stream of its own on which its chunk's H2D copies, kernels and D2H copies are ordered
+  ptflash_handle_s* child[PTF_MAX_HOST_CHUNKS];
+  cudaStream_t child_stream[PTF_MAX_HOST_CHUNKS];
+  cudaEvent_t child_done[PTF_MAX_HOST_CHUNKS];
+  cudaEvent_t host_begin;
+  int n_child;
+  bool host_stats;       // the last call was a chunked ptflash_flash_host: statistics are the sum over the children
+  int host_chunks_used;
 };
 
 namespace {
@@ -82,11 +93,25 @@ ptf::Opt make_opt(const double* o) {
   r.ss_cap = (int)o[PTFLASH_OPT_SS_CAP];
   r.hint_ss_cap = (int)o[PTFLASH_OPT_HINT_SS_CAP];
   r.split_trivial_tol = o[PTFLASH_OPT_SPLIT_TRIVIAL_TOL];
+  r.stability_only = (int)o[PTFLASH_OPT_STABILITY_ONLY];
+  r.hint_eta_search = (int)o[PTFLASH_OPT_HINT_ETA_SEARCH];
+  r.hint_tr_cap = (int)o[PTFLASH_OPT_HINT_TR_CAP];
   r.prof_events = nullptr;
   r.prof_count = nullptr;
   r.aux_stream = r.ev_fork = r.ev_join = nullptr;
   r.cta_cache = nullptr;
   return r;
+}
+
+ptf::launch_rr_fn pick_rr(int nc) {
+  using namespace ptf;
+#define PTF_CASE(NC) case NC: return launch_rr_##NC;
+  switch (nc) {
+    PTF_CASE(2) PTF_CASE(3) PTF_CASE(4) PTF_CASE(5) PTF_CASE(6) PTF_CASE(7) PTF_CASE(8) PTF_CASE(9)
+    PTF_CASE(10) PTF_CASE(11) PTF_CASE(12) PTF_CASE(13) PTF_CASE(14) PTF_CASE(15) PTF_CASE(16)
+  }
+#undef PTF_CASE
+  return nullptr;
 }
 
 ptf::launch_fn pick_launcher(int nc, int engine) {
@@ -181,6 +206,13 @@ int ptflash_destroy(ptflash_handle_t h) {
   if (h->events_made)
     for (int i = 0; i < PTF_MAX_STAGE_EVENTS; ++i) cudaEventDestroy(h->events[i]);
   if (h->aux_made) { cudaStreamDestroy(h->aux_stream); cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join); }
+  for (int c = 0; c < h->n_child; ++c) {
+    cudaStreamSynchronize(h->child_stream[c]);
+    ptflash_destroy(h->child[c]);
+    cudaStreamDestroy(h->child_stream[c]);
+    cudaEventDestroy(h->child_done[c]);
+  }
+  if (h->n_child) cudaEventDestroy(h->host_begin);
   delete h;
   return rc;
 }
@@ -195,10 +227,13 @@ int ptflash_set_option(ptflash_handle_t h, int key, double value) {
     case PTFLASH_OPT_PROBE_MARGIN: case PTFLASH_OPT_BAND:
       ok = value >= 0.0 && value < 1.0; break;
     case PTFLASH_OPT_PROBE_ITERS: case PTFLASH_OPT_STAB_SS_ITERS: case PTFLASH_OPT_STAB_TR_ITERS: case PTFLASH_OPT_SPLIT_SS_ITERS:
-    case PTFLASH_OPT_SPLIT_TR_ITERS: case PTFLASH_OPT_SS_CAP: case PTFLASH_OPT_HINT_SS_CAP:
+    case PTFLASH_OPT_SPLIT_TR_ITERS: case PTFLASH_OPT_SS_CAP: case PTFLASH_OPT_HINT_SS_CAP: case PTFLASH_OPT_HINT_TR_CAP:
       ok = value >= 0.0 && value <= 1.0e9 && value == std::floor(value); break;   // iteration counts
-    case PTFLASH_OPT_USE_NEWTON: case PTFLASH_OPT_ENGINE: case PTFLASH_OPT_STAGE_PROFILE:
+    case PTFLASH_OPT_USE_NEWTON: case PTFLASH_OPT_ENGINE: case PTFLASH_OPT_STAGE_PROFILE: case PTFLASH_OPT_STABILITY_ONLY:
+    case PTFLASH_OPT_HINT_ETA_SEARCH:
       ok = value == 0.0 || value == 1.0; break;                   // switches
+    case PTFLASH_OPT_HOST_CHUNKS:
+      ok = value >= 1.0 && value <= (double)PTF_MAX_HOST_CHUNKS && value == std::floor(value); break;
     default: break;
   }
   if (!ok) { set_err("ptflash_set_option: value out of range for this option"); return PTFLASH_EINVAL; }
@@ -235,6 +270,7 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
   d.beta = io->out_beta; d.x = io->out_x; d.y = io->out_y;
   d.phase = io->out_phase; d.iters = io->out_iters;
   d.tpd_min = io->out_tpd_min; d.lnK = io->out_lnK; d.status = io->out_status; d.stab_iters = io->out_stab_iters;
+  d.dbeta_dK = io->out_dbeta_dK;
   if (engine) {
     const size_t need = ptf::staged_workspace_bytes(h->sys.nc, io->N);
     if (!ensure(&h->ws, &h->ws_bytes, need, st, "cudaMalloc(workspace)")) return PTFLASH_ECUDA;
@@ -270,6 +306,7 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
   h->used = true;
   h->last_N = io->N;
   h->last_launches = launches;
+  h->host_stats = false;
   return PTFLASH_OK;
 }
 
@@ -282,6 +319,11 @@ int ptflash_flash(ptflash_handle_t h, int64_t N, const double* z, const double* 
   return ptflash_flash_ex(h, &io, stream);
 }
 
+// Host-buffer variant.  The batch is cut into chunks of consecutive mixtures; chunk c is handled by child handle c on a
+// stream of its own: H2D copies of its slices of z, P, T (the SoA slices are strided: cudaMemcpy2DAsync) -> the flash kernels
+// -> D2H copies of its results.  Streams of different chunks overlap, so the PCIe transfers of one chunk hide under the
+// kernels of the others (PCIe is full duplex: H2D and D2H use different copy engines).  The device buffers are chunk-local
+// SoA ([nc][Nc]), so each chunk is an ordinary ptflash_flash call.
 int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T, double* out_beta,
                        double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters, void* stream) {
   g_err.clear();
@@ -293,30 +335,86 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
   DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
   const int nc = h->sys.nc;
-  const size_t nd = (size_t)N;
-  // device staging: z, P, T, beta, x, y (doubles), phase, iters (int32)
-  const size_t n_dbl = nd * (size_t)(nc + 2 + 1 + 2 * nc);
-  const size_t need = n_dbl * sizeof(double) + 2 * nd * sizeof(int32_t);
-  if (!ensure(&h->stage, &h->stage_bytes, need, st, "cudaMalloc(staging)")) return PTFLASH_ECUDA;
-  double* dz = (double*)h->stage;
-  double* dP = dz + nd * nc;
-  double* dT = dP + nd;
-  double* dbeta = dT + nd;
-  double* dx = dbeta + nd;
-  double* dy = dx + nd * nc;
-  int32_t* dphase = (int32_t*)(dy + nd * nc);
-  int32_t* diters = dphase + nd;
-  if (!cuda_ok(cudaMemcpyAsync(dz, z, nd * nc * sizeof(double), cudaMemcpyHostToDevice, st), "H2D z")) return PTFLASH_ECUDA;
-  if (!cuda_ok(cudaMemcpyAsync(dP, P, nd * sizeof(double), cudaMemcpyHostToDevice, st), "H2D P")) return PTFLASH_ECUDA;
-  if (!cuda_ok(cudaMemcpyAsync(dT, T, nd * sizeof(double), cudaMemcpyHostToDevice, st), "H2D T")) return PTFLASH_ECUDA;
-  const int rc = ptflash_flash(h, N, dz, dP, dT, dbeta, dx, dy, dphase, out_iters ? diters : nullptr, stream);
-  if (rc != PTFLASH_OK) return rc;
-  if (!cuda_ok(cudaMemcpyAsync(out_beta, dbeta, nd * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H beta")) return PTFLASH_ECUDA;
-  if (!cuda_ok(cudaMemcpyAsync(out_x, dx, nd * nc * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H x")) return PTFLASH_ECUDA;
-  if (!cuda_ok(cudaMemcpyAsync(out_y, dy, nd * nc * sizeof(double), cudaMemcpyDeviceToHost, st), "D2H y")) return PTFLASH_ECUDA;
-  if (!cuda_ok(cudaMemcpyAsync(out_phase, dphase, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st), "D2H phase")) return PTFLASH_ECUDA;
-  if (out_iters && !cuda_ok(cudaMemcpyAsync(out_iters, diters, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st), "D2H iters")) return PTFLASH_ECUDA;
+  // chunks: at most PTFLASH_OPT_HOST_CHUNKS, none smaller than 32768 mixtures (below that a call is latency bound)
+  int chunks = (int)h->opts[PTFLASH_OPT_HOST_CHUNKS];
+  while (chunks > 1 && N / chunks < 32768) --chunks;
+  while (h->n_child < chunks) {
+    const int c = h->n_child;
+    ptflash_handle_s* k = new ptflash_handle_s();
+    std::memset(k, 0, sizeof(*k));
+    k->device = h->device;
+    k->sys = h->sys;
+    if (!cuda_ok(cudaMallocHost((void**)&k->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete k; return PTFLASH_ECUDA; }
+    std::memset(k->counters_host, 0, sizeof(ptf::StageCounters));
+    if (!cuda_ok(cudaStreamCreateWithFlags(&h->child_stream[c], cudaStreamNonBlocking), "cudaStreamCreate")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaEventCreateWithFlags(&h->child_done[c], cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+    if (c == 0 && !cuda_ok(cudaEventCreateWithFlags(&h->host_begin, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+    h->child[c] = k;
+    h->n_child = c + 1;
+  }
+  // work queued on the caller's stream before this call completes before any chunk starts
+  if (!cuda_ok(cudaEventRecord(h->host_begin, st), "cudaEventRecord")) return PTFLASH_ECUDA;
+  const int64_t per = ((N + chunks - 1) / chunks + 31) & ~(int64_t)31;
+  const size_t hp = (size_t)N * sizeof(double);   // pitch of the host SoA arrays
+  int launches = 0;
+  for (int c = 0; c < chunks; ++c) {
+    const int64_t n0 = (int64_t)c * per;
+    const int64_t nn = (n0 + per <= N ? per : N - n0);
+    if (nn <= 0) { chunks = c; break; }
+    ptflash_handle_s* k = h->child[c];
+    std::memcpy(k->opts, h->opts, sizeof(k->opts));
+    cudaStream_t cs = h->child_stream[c];
+    const size_t nd = (size_t)nn, dp = nd * sizeof(double);
+    const size_t need = nd * (size_t)(nc + 2 + 1 + 2 * nc) * sizeof(double) + 2 * nd * sizeof(int32_t);
+    if (!ensure(&k->stage, &k->stage_bytes, need, cs, "cudaMalloc(staging)")) return PTFLASH_ECUDA;
+    double* dz = (double*)k->stage;
+    double* dP = dz + nd * nc;
+    double* dT = dP + nd;
+    double* dbeta = dT + nd;
+    double* dx = dbeta + nd;
+    double* dy = dx + nd * nc;
+    int32_t* dphase = (int32_t*)(dy + nd * nc);
+    int32_t* diters = dphase + nd;
+    if (!cuda_ok(cudaStreamWaitEvent(cs, h->host_begin, 0), "cudaStreamWaitEvent")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaMemcpy2DAsync(dz, dp, z + n0, hp, dp, (size_t)nc, cudaMemcpyHostToDevice, cs), "H2D z")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaMemcpyAsync(dP, P + n0, dp, cudaMemcpyHostToDevice, cs), "H2D P")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaMemcpyAsync(dT, T + n0, dp, cudaMemcpyHostToDevice, cs), "H2D T")) return PTFLASH_ECUDA;
+    const int rc = ptflash_flash(k, nn, dz, dP, dT, dbeta, dx, dy, dphase, out_iters ? diters : nullptr, cs);
+    if (rc != PTFLASH_OK) return rc;
+    launches += k->last_launches;
+    if (!cuda_ok(cudaMemcpyAsync(out_beta + n0, dbeta, dp, cudaMemcpyDeviceToHost, cs), "D2H beta")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaMemcpy2DAsync(out_x + n0, hp, dx, dp, dp, (size_t)nc, cudaMemcpyDeviceToHost, cs), "D2H x")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaMemcpy2DAsync(out_y + n0, hp, dy, dp, dp, (size_t)nc, cudaMemcpyDeviceToHost, cs), "D2H y")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaMemcpyAsync(out_phase + n0, dphase, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, cs), "D2H phase")) return PTFLASH_ECUDA;
+    if (out_iters && !cuda_ok(cudaMemcpyAsync(out_iters + n0, diters, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, cs), "D2H iters")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaEventRecord(h->child_done[c], cs), "cudaEventRecord")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaStreamWaitEvent(st, h->child_done[c], 0), "cudaStreamWaitEvent")) return PTFLASH_ECUDA;   // join
+  }
   if (!cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
+  h->last_stream = st;
+  h->used = true;
+  h->last_N = N;
+  h->last_launches = launches;
+  h->host_stats = true;
+  h->host_chunks_used = chunks;
+  return PTFLASH_OK;
+}
+
+int ptflash_rachford_rice(ptflash_handle_t h, int64_t N, const double* lnK, const double* z, double* out_theta,
+                          double* out_x, double* out_y, double* out_dtheta_dK, void* stream) {
+  g_err.clear();
+  if (!h) { set_err("ptflash_rachford_rice: null handle"); return PTFLASH_EINVAL; }
+  if (N < 0) { set_err("ptflash_rachford_rice: N < 0"); return PTFLASH_EINVAL; }
+  if (N == 0) return PTFLASH_OK;
+  if (!lnK || !z || !out_theta) { set_err("ptflash_rachford_rice: null required pointer"); return PTFLASH_EINVAL; }
+  ptf::launch_rr_fn fn = pick_rr(h->sys.nc);
+  if (!fn) { set_err("ptflash_rachford_rice: no kernel for this nc"); return PTFLASH_EINVAL; }
+  DeviceGuard guard(h->device);
+  ptf::RrIo io;
+  io.N = N; io.lnK = lnK; io.z = z; io.theta = out_theta; io.x = out_x; io.y = out_y; io.dth = out_dtheta_dK;
+  if (fn(io, (cudaStream_t)stream) < 0) { cuda_ok(cudaGetLastError(), "rachford-rice kernel"); if (g_err.empty()) set_err("kernel launch failed"); return PTFLASH_ECUDA; }
+  h->last_stream = (cudaStream_t)stream;
+  h->used = true;
   return PTFLASH_OK;
 }
 
@@ -326,7 +424,20 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
   if (!h->used) return PTFLASH_OK;
   DeviceGuard guard(h->device);
   if (!cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
-  const ptf::StageCounters& c = *h->counters_host;
+  ptf::StageCounters sum;
+  if (h->host_stats) {
+    // chunked host call: sums (and maxima) over the chunks' child handles, all complete after the synchronise above
+    std::memset(&sum, 0, sizeof(sum));
+    for (int k = 0; k < h->host_chunks_used; ++k) {
+      const long long* a = (const long long*)h->child[k]->counters_host;
+      long long* b = (long long*)&sum;
+      const size_t n_add = offsetof(ptf::StageCounters, max_probe) / sizeof(long long), n_all = sizeof(sum) / sizeof(long long);
+      for (size_t i = 0; i < n_all; ++i) b[i] = (i < n_add) ? b[i] + a[i] : (a[i] > b[i] ? a[i] : b[i]);
+    }
+  } else {
+    sum = *h->counters_host;
+  }
+  const ptf::StageCounters& c = sum;
   out->n_total = h->last_N;
   out->kernel_launches = h->last_launches;
   if ((int)h->opts[PTFLASH_OPT_ENGINE]) {
@@ -339,6 +450,17 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
     out->n_split = c.n_split;
     out->n_split_newton = c.n_split_newton;
     out->n_two_phase = c.n_two_phase;
+    for (int k = 0; k < 2; ++k) {
+      out->n_stab_tr[k] = c.n_stab_tr[k];
+      out->n_stab_capped[k] = c.n_stab_capped[k];
+      out->max_stab_ss_iters[k] = (int32_t)c.max_stab_ss[k];
+      out->max_stab_tr_iters[k] = (int32_t)c.max_stab_tr[k];
+    }
+    out->n_split_capped = c.n_split_capped;
+    out->n_warm_restarts = c.n_restart;
+    out->max_probe_iters = (int32_t)c.max_probe;
+    out->max_split_ss_iters = (int32_t)c.max_split_ss;
+    out->max_split_tr_iters = (int32_t)c.max_split_tr;
   }
   return PTFLASH_OK;
 }

@@ -25,7 +25,9 @@ namespace ptf {
 // ------------------------------------------------------------------------------------------------
 struct Opt {
   double tol_ss, tol_newton_g, tol_newton_step, tol_newton_step_stab, probe_margin, trivial_tol, band, split_trivial_tol;
-  int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap, hint_ss_cap;
+  int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap, hint_ss_cap, hint_tr_cap;
+  int stability_only;   // 1: stop after the label; no phase split
+  int hint_eta_search;  // 1: splits entered through a skip-stability hint run the eta search of B.4a (the oracle's path)
   // host only: cudaEvent_t[PTF_MAX_STAGE_EVENTS] recorded between the stage kernels when stage profiling is on (else null)
   void* prof_events;
   int* prof_count;   // host only: number of events recorded by the last launch
@@ -58,6 +60,7 @@ struct Io {
   int32_t *phase, *iters;
   double *tpd_min, *lnK;
   int32_t *status, *stab_iters;
+  double* dbeta_dK;   // optional [nc][N]: d beta / d K_i at the solution (eq. 13)
 };
 
 enum : int { ST_STAB_CAP = 1, ST_SPLIT_CAP = 2, ST_BAND = 4, ST_SPLIT_FAILED = 8, ST_LNK0_REJECTED = 32, ST_WARM_RESTART = 64,

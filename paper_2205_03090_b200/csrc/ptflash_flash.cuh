@@ -5,6 +5,7 @@
 // and the run-to-completion kernel (engine 0): one thread = one mixture from load to store.
 #pragma once
 #include "ptflash_device.cuh"
+#include "ptflash_math.cuh"
 
 namespace ptf {
 
@@ -291,7 +292,7 @@ __device__ __noinline__ void split_ss(const Sys<NC>& S, const Opt& o, const MixC
 // Needs x, y, theta = RR(exp(st.lnK), z) on entry with 0 < theta < 1.
 template <int NC>
 __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const MixCtx<NC>& m, SplitState<NC>& st,
-                                          double (&x)[NC], double (&y)[NC]) {
+                                          double (&x)[NC], double (&y)[NC], bool hinted = false) {
   double Mx[NC * NC], My[NC * NC], H[NC * NC], Lc[NC * NC];
   double nV[NC], gt[NC], D[NC], sstep[NC], lpx[NC], lpy[NC], Sx[NC], Sy[NC];
   Eos ex, ey;
@@ -325,8 +326,9 @@ __device__ __noinline__ void split_newton(const Sys<NC>& S, const Opt& o, const 
   eval();
   double Delta = 0.25;
   bool converged = false;
+  const int tr_cap = hinted ? min(o.split_tr_iters, o.hint_tr_cap) : o.split_tr_iters;   // reading C21
 #pragma unroll 1
-  for (int itn = 0; itn < o.split_tr_iters; ++itn) {
+  for (int itn = 0; itn < tr_cap; ++itn) {
     // reading C8: a gradient below the target triggers one last full Newton step (applied if admissible), see DESIGN.md
     const bool last = gmax < o.tol_newton_g;
     if (!last) st.iters++;
@@ -421,7 +423,7 @@ __device__ __forceinline__ void phase_split(const Sys<NC>& S, const Opt& o, cons
 #pragma unroll
   for (int i = 0; i < NC; ++i) st.lnK[i] = lnK[i];
   split_ss<NC>(S, o, m, st, x, y, hinted);
-  if (st.go_newton) split_newton<NC>(S, o, m, st, x, y);
+  if (st.go_newton) split_newton<NC>(S, o, m, st, x, y, hinted);
   split_finish<NC>(st, res);
 #pragma unroll
   for (int i = 0; i < NC; ++i) lnK[i] = st.lnK[i];
@@ -482,6 +484,22 @@ __device__ __forceinline__ bool start_lnK(const Sys<NC>& S, const Io& io, int64_
     for (int i = 0; i < NC; ++i) lnKs[i] = l0[i];
   } else status |= ST_LNK0_REJECTED;
   return have0;
+}
+
+// Does the Rachford-Rice equation (eq. 7) for K = exp(lnK) have its root inside 0 < theta < 1?  f_RR is strictly decreasing
+// on its window, so this is f_RR(0) > 0 and f_RR(1) < 0 (which also implies that the window exists: some K_i > 1, some < 1).
+// Used for the first Rachford-Rice of the probe.
+template <int NC>
+__device__ __forceinline__ bool rr_root_inside01(const double (&z)[NC], const double (&lnK)[NC]) {
+  double f0 = 0.0, f1 = 0.0;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    const bool a = z[i] > 0.0;
+    const double K = exp_fast(a ? lnK[i] : 0.0);   // z_i = 0: K = 1 drops out of both sums
+    f0 = fma(z[i], K - 1.0, f0);
+    f1 = fma(z[i] * (K - 1.0), rcp_fast(K), f1);
+  }
+  return f0 > 0.0 && f1 < 0.0;
 }
 
 // Probe of section 2.2.3: probe_iters phase-split SS iterations from lnK, then the
@@ -552,6 +570,7 @@ __device__ __forceinline__ void store_invalid(const Io& io, int64_t n) {
     io.x[(int64_t)i * io.N + n] = nan;
     io.y[(int64_t)i * io.N + n] = nan;
     if (io.lnK) io.lnK[(int64_t)i * io.N + n] = nan;
+    if (io.dbeta_dK) io.dbeta_dK[(int64_t)i * io.N + n] = nan;
   }
   if (io.iters) io.iters[n] = 0;
   if (io.tpd_min) io.tpd_min[n] = nan;
@@ -584,6 +603,52 @@ __device__ __forceinline__ void store_result(const Io& io, int64_t n, bool two, 
     io.x[(int64_t)i * io.N + n] = two ? (swap ? y[i] : x[i]) : z[i];
     io.y[(int64_t)i * io.N + n] = two ? (swap ? x[i] : y[i]) : z[i];
     if (io.lnK) io.lnK[(int64_t)i * io.N + n] = two ? (swap ? -lnK[i] : lnK[i]) : 0.0;
+  }
+  if (io.iters) io.iters[n] = iters;
+  if (io.tpd_min) io.tpd_min[n] = tpd_min;
+  if (io.status) io.status[n] = status;
+  if (io.stab_iters) io.stab_iters[n] = stab_iters;
+  if (io.dbeta_dK) {
+    // eq. 13 PAPER.md:281-286 at the reported solution: with 1 + (K_i - 1) beta = z_i / x_i the two partial derivatives of
+    // f_RR (eq. 7) become  d f / d K_i = x_i^2 / z_i  and  d f / d beta = - sum_j (y_j - x_j)^2 / z_j,  so
+    // d beta / d K_i = (x_i^2 / z_i) / sum_j (y_j - x_j)^2 / z_j   (unchanged by the x <-> y exchange of C23 up to K -> 1/K,
+    // which is why it is formed from the compositions as reported).  Single phase: NaN.
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    if (two) {
+      double den = 0.0;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const double dxy = y[i] - x[i];
+        if (z[i] > 0.0) den = fma(dxy * dxy, 1.0 / z[i], den);
+      }
+      const double iden = 1.0 / den;
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        const double xr = swap ? y[i] : x[i];
+        io.dbeta_dK[(int64_t)i * io.N + n] = (z[i] > 0.0) ? xr * xr / z[i] * iden : 0.0;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < NC; ++i) io.dbeta_dK[(int64_t)i * io.N + n] = nan;
+    }
+  }
+}
+
+// Stability-only mode (PTFLASH_OPT_STABILITY_ONLY; "determine stability (no need for phase split
+// calculations)"): the store of a mixture labelled UNSTABLE -- phase = 2, x = y = z, beta = NaN (not computed), lnK = the K
+// that would seed the phase split (probe iterate, caller's estimate, or the stability trial's).
+template <int NC>
+__device__ __forceinline__ void store_unstable_label(const Io& io, int64_t n, const double (&z)[NC], const double (&lnK)[NC],
+                                                     int iters, int status, double tpd_min, int stab_iters) {
+  const double nan = __longlong_as_double(0x7ff8000000000000LL);
+  io.beta[n] = nan;
+  io.phase[n] = 2;
+#pragma unroll
+  for (int i = 0; i < NC; ++i) {
+    io.x[(int64_t)i * io.N + n] = z[i];
+    io.y[(int64_t)i * io.N + n] = z[i];
+    if (io.lnK) io.lnK[(int64_t)i * io.N + n] = (z[i] > 0.0) ? lnK[i] : 0.0;
+    if (io.dbeta_dK) io.dbeta_dK[(int64_t)i * io.N + n] = nan;
   }
   if (io.iters) io.iters[n] = iters;
   if (io.tpd_min) io.tpd_min[n] = tpd_min;
@@ -633,6 +698,10 @@ __device__ void flash_one(const Sys<NC>& S, const Opt& o, const Io& io, int64_t 
     } else {
       unstable = true;
       tpd_min = nan;
+    }
+    if (o.stability_only) {
+      if (unstable) { store_unstable_label<NC>(io, n, m.z, lnK, iters, status, tpd_min, stab_iters); return; }
+      break;
     }
     int split_status = 0;
     if (unstable) {

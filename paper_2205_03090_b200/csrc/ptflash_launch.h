@@ -28,19 +28,31 @@ inline Sys<NC> narrow(const SysHost& h) {
 // Stage counters of the staged engine (first bytes of the workspace; mirrored to the host after each call).
 struct StageCounters {
   long long n_invalid, n_case1, n_case2, n_case3, n_stab, n_stab_newton, n_split, n_split_newton, n_two_phase;
-  long long reserved[7];
+  long long n_restart;                         // skip-stability hints that failed and were re-flashed cold (C21)
+  // the columns of the paper's profiler (Table 4) that are not queue lengths; [0] vapour-like, [1] liquid-like
+  long long n_stab_tr[2], n_stab_capped[2];    // stability trials that went on to the trust-region stage / hit an iteration cap
+  long long n_split_capped;                    // phase splits that hit an iteration cap
+  long long max_probe, max_stab_ss[2], max_stab_tr[2], max_split_ss, max_split_tr;   // largest iteration counts per stage
 };
 
 // Launchers return the number of kernels launched (>= 0) or -1 on error.
 //   launch_mono_<NC>   engine 0: one run-to-completion kernel (workspace unused)
 //   launch_staged_<NC> engine 1: staged persistent kernels with work queues in `workspace`
 typedef int (*launch_fn)(const SysHost&, const Opt&, const Io&, void* workspace, cudaStream_t);
+// arguments of the batched Rachford-Rice kernel (ptflash_rr.cuh)
+struct RrIo {
+  int64_t N;
+  const double *lnK, *z;          // [nc][N]
+  double *theta, *x, *y, *dth;    // [N], [nc][N] x 3 (x, y, dth optional)
+};
+typedef int (*launch_rr_fn)(const RrIo&, cudaStream_t);
 size_t staged_workspace_bytes(int nc, int64_t N);
 int run_fp64_peak(int iters, double* flops_per_s, double* elapsed_ms, cudaStream_t st);
 int run_math_probe(int fn, int64_t n, const double* x, double* y, cudaStream_t st);
 
 #define PTF_DECL(NC) int launch_mono_##NC(const SysHost&, const Opt&, const Io&, void*, cudaStream_t); \
-  int launch_staged_##NC(const SysHost&, const Opt&, const Io&, void*, cudaStream_t);
+  int launch_staged_##NC(const SysHost&, const Opt&, const Io&, void*, cudaStream_t); \
+  int launch_rr_##NC(const RrIo&, cudaStream_t);
 PTF_DECL(2) PTF_DECL(3) PTF_DECL(4) PTF_DECL(5) PTF_DECL(6) PTF_DECL(7) PTF_DECL(8) PTF_DECL(9)
 PTF_DECL(10) PTF_DECL(11) PTF_DECL(12) PTF_DECL(13) PTF_DECL(14) PTF_DECL(15) PTF_DECL(16)
 #undef PTF_DECL

@@ -4,6 +4,7 @@
 #include "ptflash_flash.cuh"
 #include "ptflash_staged.cuh"
 #include "ptflash_stage2.cuh"
+#include "ptflash_rr.cuh"
 
 #ifndef PTF_NC
 #error "compile with -DPTF_NC=<2..16>"
@@ -18,6 +19,7 @@ namespace ptf {
 // development build that left this component count out
 int PTF_CAT(launch_mono_, PTF_NC)(const SysHost&, const Opt&, const Io&, void*, cudaStream_t) { return -1; }
 int PTF_CAT(launch_staged_, PTF_NC)(const SysHost&, const Opt&, const Io&, void*, cudaStream_t) { return -1; }
+int PTF_CAT(launch_rr_, PTF_NC)(const RrIo&, cudaStream_t) { return -1; }
 }  // namespace ptf
 #else
 
@@ -37,6 +39,8 @@ int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& i
 #endif
   return launch_staged<PTF_NC>(hs, o, io, ws, st);
 }
+
+int PTF_CAT(launch_rr_, PTF_NC)(const RrIo& io, cudaStream_t st) { return launch_rr<PTF_NC>(io, st); }
 
 }  // namespace ptf
 #endif

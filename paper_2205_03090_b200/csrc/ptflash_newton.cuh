@@ -171,6 +171,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
   double tm = 0.0, rmax_acc = 0.0, pred = 0.0, Delta = 1.0, Delta_cap = 8.0, snorm = 0.0, Zw = 0.0, kept_sn = 0.0;
   EtaSearch es;
   es.start(1.0e-3);
+  int my_max = 0;   // Table-4 counter, published after the loop
 
 #pragma unroll 1
   while (true) {
@@ -377,9 +378,17 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
       w.sumW[(int64_t)sidx * N + n] = sumW;
       w.tflags[(int64_t)sidx * N + n] = (fin_conv ? TF_CONVERGED : 0) | (fin_exact ? TF_EXACT : 0) |
                                         (fin_cap ? TF_CAPPED : 0) | TF_BETA | (iters << TF_ITER_SHIFT);
+      if (fin_cap) atomicAdd((unsigned long long*)&w.ctr->n_stab_capped[sidx], 1ull);   // rare
+      {
+        // running maxima of the trust-region iteration count per start, two 16-bit fields of one register
+        const int sh = sidx << 4, it = min(tr_it, 65535);
+        if (it > ((my_max >> sh) & 0xffff)) my_max = (my_max & ~(0xffff << sh)) | (it << sh);
+      }
       busy = false;
     }
   }
+  flush_max(my_max & 0xffff, &w.ctr->max_stab_tr[0]);
+  flush_max((my_max >> 16) & 0xffff, &w.ctr->max_stab_tr[1]);
 }
 
 // ---- K6: phase-split trust-region Newton on G (B.4-B.5), persistent warps with lane refill --------
@@ -410,6 +419,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   int* ticket = &w.qcount[part ? Q_TICKET_SPLIT_B : Q_TICKET_SPLIT];
   bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false, polish = false;
   bool eta_mode = false;   // this lane's item runs the eta search of B.4a instead of the truncated modified-Cholesky step
+  int tr_cap = 0;          // trust-region iteration cap of the lane's item (smaller for a skip-stability hint, reading C21)
   int n = 0, tr_it = 0, status = 0;
   unsigned act = 0u;
   PT3<NC> q;
@@ -420,6 +430,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   Eos ex, ey;   // cubic scalars of the two phases at the evaluated point (Z doubles as the warm start)
   ex.A = ex.B = ex.Z = ex.q = ex.L = ex.lnZmB = 0.0;
   ey = ex;
+  int my_max = 0;   // Table-4 counter, published after the loop
 
 #pragma unroll 1
   while (true) {
@@ -431,7 +442,11 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           const double P = io.P[n], Tk = io.T[n];
           { const double iT = rcp_fast(Tk); q.sT = sqrt_fast(Tk); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
           act = (unsigned)w.actmask[n];
-          eta_mode = (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED);
+          {
+            const bool hinted = (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED);
+            eta_mode = o.hint_eta_search && hinted;
+            tr_cap = hinted ? min(o.split_tr_iters, o.hint_tr_cap) : o.split_tr_iters;
+          }
 #pragma unroll
           for (int i = 0; i < NC; ++i) {
             sn[i * T] = w.lnK[(int64_t)i * N + n];   // k2_split_ss left n^V here
@@ -532,7 +547,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         // to the phase boundary the Hessian is nearly singular and the gradient does not bound the error of n^V -- it
         // triggers one last full Newton step (polish), applied without another evaluation if it is admissible.
         polish = gmax < o.tol_newton_g;
-        if (!polish && tr_it >= o.split_tr_iters) { finish = true; status |= ST_SPLIT_CAP; }
+        if (!polish && tr_it >= tr_cap) { finish = true; status |= ST_SPLIT_CAP; }
         else {
           if (!polish) tr_it++;
           es.start(1.0e-3 * rcp_fast(theta * (1.0 - theta)));
@@ -696,9 +711,12 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         for (int i = 0; i < NC; ++i) lnK[i] = 0.0;
       }
       store_split<NC>(io, w, n, z, fin_conv, trivial, theta, tr_it, status, x, y, lnK, ex.Z, ey.Z);
+      if (status & ST_SPLIT_CAP) atomicAdd((unsigned long long*)&w.ctr->n_split_capped, 1ull);   // rare
+      my_max = max(my_max, tr_it);
       busy = false;
     }
   }
+  flush_max(my_max, &w.ctr->max_split_tr);
 }
 
 }  // namespace ptf

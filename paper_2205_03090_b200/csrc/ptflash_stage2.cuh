@@ -31,9 +31,10 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
   exp_tab_init(s_exp);
   const int64_t cnt = w.qcount[Q_PROBE];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
+  int my_max = 0;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    int pcase = 0, n = 0;
+    int pcase = 0, n = 0, iters = 0;
     if (in) {
       n = w.q_probe[idx];
       double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
@@ -44,7 +45,6 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
       int status = w.status[n] & ST_WARM_RESTART, fl = 0;
       start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
       double theta = -1.0e300, Zx = 0.0, Zy = 0.0;
-      int iters = 0;
       pcase = 2;
 #pragma unroll 1
       for (int it = 0; it < o.probe_iters; ++it) {
@@ -93,9 +93,11 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
     count_add(pcase == 1, &w.ctr->n_case1);
     count_add(pcase == 2, &w.ctr->n_case2);
     count_add(pcase == 3, &w.ctr->n_case3);
+    my_max = max(my_max, iters);
     queue_push(pcase == 1 || pcase == 2, &w.qcount[Q_STAB], w.q_stab, n);
     queue_push(pcase == 3, &w.qcount[Q_SPLIT], w.q_split, n);
   }
+  flush_max(my_max, &w.ctr->max_probe);
 }
 
 // ---- K2: stability SS -----------------------------------------------------------------------------
@@ -119,10 +121,12 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
   const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
+  // Table-4 counters: a thread always works on the same start (the grid stride is even, so idx & 1 == threadIdx.x & 1)
+  int my_tr = 0, my_cap = 0, my_max = 0;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    bool need_newton = false;
-    int item = 0;
+    bool need_newton = false, capped = false;
+    int item = 0, iters = 0;
     if (in) {
       const int n = w.q_stab[idx >> 1];
       const int sidx = (int)(idx & 1);  // 0 vapour-like, 1 liquid-like
@@ -146,8 +150,7 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
       Eos e;
       e.Z = 0.0;
       const int ss_max = o.use_newton ? o.stab_ss_iters : o.ss_cap;
-      bool converged = false, capped = false;
-      int iters = 0;
+      bool converged = false;
       double tm = 0.0, sumW = 1.0;
 #pragma unroll 1
       for (int k = 0; k <= ss_max; ++k) {
@@ -193,7 +196,19 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
       w.tflags[(int64_t)sidx * N + n] = (converged ? TF_CONVERGED : 0) | (capped ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
       if (need_newton) w.Zw[(int64_t)sidx * N + n] = e.Z;
     }
+    my_tr += need_newton ? 1 : 0;
+    my_cap += capped ? 1 : 0;
+    my_max = max(my_max, iters);
     queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
+  }
+  {
+    const bool odd = threadIdx.x & 1;
+    flush_add(odd ? 0 : my_tr, &w.ctr->n_stab_tr[0]);
+    flush_add(odd ? my_tr : 0, &w.ctr->n_stab_tr[1]);
+    flush_add(odd ? 0 : my_cap, &w.ctr->n_stab_capped[0]);
+    flush_add(odd ? my_cap : 0, &w.ctr->n_stab_capped[1]);
+    flush_max(odd ? 0 : my_max, &w.ctr->max_stab_ss[0]);
+    flush_max(odd ? my_max : 0, &w.ctr->max_stab_ss[1]);
   }
 }
 
@@ -256,10 +271,11 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
   const int64_t cnt = w.qcount[part ? Q_SPLIT_B : Q_SPLIT];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
+  int my_max = 0;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
     bool go_newton = false;
-    int n = 0;
+    int n = 0, k = 0, status = 0;
     if (in) {
       n = q_in[idx];
       double z[NC], lnK[NC], x[NC], y[NC], lpx[NC], lpy[NC];
@@ -273,7 +289,6 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
       const bool hinted = (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED);
       double Zx = w.Zxy[n], Zy = w.Zxy[N + n];   // roots of the stage that produced lnK (0: none)
       bool converged = false, failed = false, final_rr = false;
-      int k = 0, status = 0;
       // One copy of exp + Rachford-Rice + the two lnphi evaluations: the Rachford-Rice that makes x, y consistent with
       // the converged lnK is the top of one more trip (final_rr).
 #pragma unroll 1
@@ -334,8 +349,11 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         store_split<NC>(io, w, n, z, converged, failed, theta, k, status, x, y, lnK, Zx, Zy);
       }
     }
+    my_max = max(my_max, k);
+    count_add((status & ST_SPLIT_CAP) != 0, &w.ctr->n_split_capped);   // rare: no atomic unless a lane hit the cap
     queue_push(go_newton, &w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON], part ? w.q_split_newton_b : w.q_split_newton, n);
   }
+  flush_max(my_max, &w.ctr->max_split_ss);
 }
 
 }  // namespace ptf
@@ -388,10 +406,21 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   cudaStream_t aux = (cudaStream_t)o.aux_stream;
   const bool fork = aux != nullptr && ev == nullptr;
   w.decide_part = 1;
-  const int passes = (io.flags && io.lnK0) ? 2 : 1;   // pass 1: cold re-flash of mixtures whose skip-stability hint failed
+  // Warm-start call (caller flags): the hinted splits run first; the hints that fail (reading C21) are appended to the probe
+  // queue and take the cold path together with the mixtures that came without a hint -- one pass, no second sweep
+  // (in stability-only mode a hint is a verdict, not a split: nothing to run).
+  if (io.flags && io.lnK0 && !o.stability_only) {
+    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0);
+    mark();
+    k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
+    mark();
+    k_requeue_failed_hints<<<1, 1024, 0, st>>>(w);
+    mark();
+    launches += 3;
+  }
+  const int passes = 1;
   for (int pass = 0; pass < passes; ++pass) {
     w.pass = pass;
-    if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
     k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
     k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
@@ -400,6 +429,14 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     mark();
     k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
     mark();
+    if (o.stability_only) {
+      k_label_only<NC><<<gN, threads, 0, st>>>(io, w);
+      mark();
+      k_finalize_counters<<<1, 32, 0, st>>>(w);
+      mark();
+      launches += 6;
+      break;
+    }
     if (fork) {
       cudaEventRecord((cudaEvent_t)o.ev_fork, st);
       cudaStreamWaitEvent(aux, (cudaEvent_t)o.ev_fork, 0);

@@ -107,6 +107,24 @@ __device__ __forceinline__ void count_add(bool pred, long long* ctr) {
   if (mask && (int)(threadIdx.x & 31) == __ffs(mask) - 1) atomicAdd((unsigned long long*)ctr, (unsigned long long)__popc(mask));
 }
 
+// running maximum of an iteration count (Table 4's "max number of iterations" row)
+__device__ __forceinline__ void count_max(bool pred, int v, long long* ctr) {
+  const unsigned active = __activemask();
+  const int m = __reduce_max_sync(active, pred ? v : 0);
+  if (m > 0 && (int)(threadIdx.x & 31) == __ffs(active) - 1) atomicMax((unsigned long long*)ctr, (unsigned long long)m);
+}
+
+// The same for kernels that see many items per thread: the thread keeps its own maximum / count in a register and the warp
+// publishes once, after its loop (all lanes converged), so the hot loop carries a compare instead of an atomic.
+__device__ __forceinline__ void flush_max(int v, long long* ctr) {
+  const int m = __reduce_max_sync(0xffffffffu, v);
+  if (m > 0 && (threadIdx.x & 31) == 0) atomicMax((unsigned long long*)ctr, (unsigned long long)m);
+}
+__device__ __forceinline__ void flush_add(int v, long long* ctr) {
+  const int m = __reduce_add_sync(0xffffffffu, v);
+  if (m > 0 && (threadIdx.x & 31) == 0) atomicAdd((unsigned long long*)ctr, (unsigned long long)m);
+}
+
 // context of a mixture already validated by K1a
 template <int NC>
 __device__ __forceinline__ void reload_ctx(const Sys<NC>& S, const Io& io, const Work& w, int n, bool need_ref, MixCtx<NC>& m,
@@ -186,18 +204,8 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
       } else if (o.probe_iters == 0) {
         dest = 1;
       } else {
-        // first Rachford-Rice of the probe: theta in (0,1) <=> window exists, f(0) > 0 and f(1) < 0
-        double f0 = 0.0, f1 = 0.0, Kmax = 0.0, Kmin = 1.0e300;
-#pragma unroll
-        for (int i = 0; i < NC; ++i) {
-          const bool a = m.z[i] > 0.0;
-          const double K = exp_fast(a ? lnKs[i] : 0.0);   // z_i = 0: K = 1 drops out of every term below
-          Kmax = dmax(Kmax, K);
-          Kmin = dmin(Kmin, K);
-          f0 = fma(m.z[i], K - 1.0, f0);
-          f1 = fma(m.z[i] * (K - 1.0), rcp_fast(K), f1);
-        }
-        dest = (Kmax > 1.0 && Kmin < 1.0 && f0 > 0.0 && f1 < 0.0) ? 0 : 1;
+        // first Rachford-Rice of the probe: theta in (0,1) <=> f(0) > 0 and f(1) < 0
+        dest = rr_root_inside01<NC>(m.z, lnKs) ? 0 : 1;
       }
     }
     count_add(dest == 1, &w.ctr->n_case1);
@@ -215,13 +223,13 @@ __global__ void __launch_bounds__(128) k_probe(const __grid_constant__ Sys<NC> S
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    int pcase = 0, n = 0;
+    int pcase = 0, n = 0, iters = 0;
     if (in) {
       n = w.q_probe[idx];
       MixCtx<NC> m;
       double P, T;
       reload_ctx<NC>(S, io, w, n, true, m, P, T);
-      int status = w.status[n] & ST_WARM_RESTART, fl = 0, iters = 0;
+      int status = w.status[n] & ST_WARM_RESTART, fl = 0;
       double lnK[NC];
       start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
       double tpd_min = 0.0;
@@ -236,9 +244,20 @@ __global__ void __launch_bounds__(128) k_probe(const __grid_constant__ Sys<NC> S
     count_add(pcase == 1, &w.ctr->n_case1);
     count_add(pcase == 2, &w.ctr->n_case2);
     count_add(pcase == 3, &w.ctr->n_case3);
+    count_max(in, iters, &w.ctr->max_probe);
     queue_push(pcase == 1 || pcase == 2, &w.qcount[Q_STAB], w.q_stab, n);
     queue_push(pcase == 3, &w.qcount[Q_SPLIT], w.q_split, n);
   }
+}
+
+// Table-4 counters of the stability SS stage (called by all lanes of the warp)
+__device__ __forceinline__ void stab_ss_counters(const Work& w, bool in, int sidx, bool need_newton, bool capped, int iters) {
+  count_add(in && need_newton && sidx == 0, &w.ctr->n_stab_tr[0]);
+  count_add(in && need_newton && sidx == 1, &w.ctr->n_stab_tr[1]);
+  count_add(in && capped && sidx == 0, &w.ctr->n_stab_capped[0]);
+  count_add(in && capped && sidx == 1, &w.ctr->n_stab_capped[1]);
+  count_max(in && sidx == 0, iters, &w.ctr->max_stab_ss[0]);
+  count_max(in && sidx == 1, iters, &w.ctr->max_stab_ss[1]);
 }
 
 // ---- K2 -------------------------------------------------------------------------------------------
@@ -260,8 +279,8 @@ __global__ void __launch_bounds__(128) k_stab_ss(const __grid_constant__ Sys<NC>
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    bool need_newton = false;
-    int item = 0;
+    bool need_newton = false, capped = false;
+    int item = 0, ss_iters = 0;
     if (in) {
       const int n = w.q_stab[idx >> 1];
       const int sidx = (int)(idx & 1);  // 0 vapour-like, 1 liquid-like
@@ -276,8 +295,11 @@ __global__ void __launch_bounds__(128) k_stab_ss(const __grid_constant__ Sys<NC>
       stab_init<NC>(m, lnKs, sidx ? -1.0 : 1.0, st);
       stab_ss<NC>(S, o, m, st);
       need_newton = !st.converged && o.use_newton;
+      capped = st.capped;
+      ss_iters = st.iters;
       store_trial<NC>(io, w, n, sidx, st);
     }
+    stab_ss_counters(w, in, item & 1, need_newton, capped, ss_iters);
     queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
   }
 }
@@ -297,10 +319,15 @@ __global__ void __launch_bounds__(128) k_stab_newton(const __grid_constant__ Sys
 #pragma unroll
     for (int i = 0; i < NC; ++i) st.lnW[i] = w.lnW[((int64_t)sidx * NC + i) * io.N + n];
     st.tm = 0.0; st.sumW = 1.0;
-    st.iters = w.tflags[(int64_t)sidx * io.N + n] >> TF_ITER_SHIFT;
+    const int it0 = w.tflags[(int64_t)sidx * io.N + n] >> TF_ITER_SHIFT;
+    st.iters = it0;
     st.converged = false; st.stationary_exact = false; st.capped = false;
     stab_newton<NC>(S, o, m, st);
     store_trial<NC>(io, w, n, sidx, st);
+    count_add(st.capped && sidx == 0, &w.ctr->n_stab_capped[0]);
+    count_add(st.capped && sidx == 1, &w.ctr->n_stab_capped[1]);
+    count_max(sidx == 0, st.iters - it0, &w.ctr->max_stab_tr[0]);
+    count_max(sidx == 1, st.iters - it0, &w.ctr->max_stab_tr[1]);
   }
 }
 
@@ -397,8 +424,8 @@ __global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    bool go_newton = false;
-    int n = 0;
+    bool go_newton = false, capped = false;
+    int n = 0, ss_iters = 0;
     if (in) {
       n = w.q_split[idx];
       MixCtx<NC> m;
@@ -410,6 +437,8 @@ __global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC
       double x[NC], y[NC];
       split_ss<NC>(S, o, m, st, x, y, (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED));
       go_newton = st.go_newton;
+      ss_iters = st.iters;
+      capped = (st.status & ST_SPLIT_CAP) != 0;
       if (go_newton) {
 #pragma unroll
         for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = st.lnK[i];
@@ -419,6 +448,8 @@ __global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC
         finish_split<NC>(S, io, w, n, m, st, x, y);
       }
     }
+    count_max(in, ss_iters, &w.ctr->max_split_ss);
+    count_add(capped, &w.ctr->n_split_capped);
     queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
   }
 }
@@ -438,8 +469,30 @@ __global__ void __launch_bounds__(128) k_split_newton(const __grid_constant__ Sy
     for (int i = 0; i < NC; ++i) { st.lnK[i] = w.lnK[(int64_t)i * io.N + n]; K[i] = exp(st.lnK[i]); }
     st.iters = 0; st.status = 0; st.converged = false; st.failed = false; st.go_newton = true;
     rr_solve<NC>(K, m.z, st.theta, x, y);  // the same Rachford-Rice that ended the SS stage
-    split_newton<NC>(S, o, m, st, x, y);
+    split_newton<NC>(S, o, m, st, x, y, (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED));
+    count_max(true, st.iters, &w.ctr->max_split_tr);
+    count_add((st.status & ST_SPLIT_CAP) != 0, &w.ctr->n_split_capped);
     finish_split<NC>(S, io, w, n, m, st, x, y);
+  }
+}
+
+// ---- stability-only mode --------------------------------------------------------------------------
+// PTFLASH_OPT_STABILITY_ONLY: the mixtures queued for the phase split (probe case 3, the caller's
+// "unstable" flag, or the stability verdict) are labelled instead of split; the stable ones were stored by k_stab_decide.
+template <int NC>
+__global__ void __launch_bounds__(128) k_label_only(const __grid_constant__ Io io, const __grid_constant__ Work w) {
+  const int64_t N = io.N;
+#pragma unroll 1
+  for (int part = 0; part < 2; ++part) {
+    const int* const q = part ? w.q_split_b : w.q_split;
+    const int64_t cnt = w.qcount[part ? Q_SPLIT_B : Q_SPLIT];
+    PTF_GRID_STRIDE(idx, cnt) {
+      const int n = q[idx];
+      double z[NC], lnK[NC];
+#pragma unroll
+      for (int i = 0; i < NC; ++i) { z[i] = w.zn[(int64_t)i * N + n]; lnK[i] = w.lnK[(int64_t)i * N + n]; }
+      store_unstable_label<NC>(io, n, z, lnK, w.iters[n], w.status[n] & ~ST_INTERNAL_SKIPPED, w.tpdmin[n], w.stabit[n]);
+    }
   }
 }
 
@@ -463,7 +516,24 @@ static __global__ void k_begin_pass2(const __grid_constant__ Work w) {
     w.qcount[Q_STAB] = 0; w.qcount[Q_STAB_NEWTON] = 0; w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0;
     w.qcount[Q_TICKET_STAB] = 0; w.qcount[Q_TICKET_SPLIT] = 0; w.qcount[Q_RETRY] = 0;
     w.qcount[Q_SPLIT_B] = 0; w.qcount[Q_SPLIT_NEWTON_B] = 0; w.qcount[Q_TICKET_SPLIT_B] = 0;
-    w.ctr->reserved[0] = cnt;   // number of warm restarts
+    w.ctr->n_restart += cnt;   // number of warm restarts
+  }
+}
+
+// Warm-start calls of the fast engine: the splits entered through a skip-stability hint run FIRST; the hints that failed
+// (Q_RETRY, reading C21) then join the probe queue of the mixtures without a hint, so the whole call stays one pass.
+// The split queues and tickets restart from zero for the probe- and stability-found splits that follow.
+static __global__ void k_requeue_failed_hints(const __grid_constant__ Work w) {
+  const int cnt = w.qcount[Q_RETRY], base = w.qcount[Q_PROBE];
+  for (int i = threadIdx.x; i < cnt; i += blockDim.x) w.q_probe[base + i] = w.q_retry[i];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    w.ctr->n_restart += cnt;
+    w.ctr->n_split += w.qcount[Q_SPLIT];
+    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON];
+    w.qcount[Q_PROBE] = base + cnt;
+    w.qcount[Q_RETRY] = 0;
+    w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0; w.qcount[Q_TICKET_SPLIT] = 0;
   }
 }
 
@@ -485,7 +555,7 @@ int launch_staged(const SysHost& hs, const Opt& o, const Io& io, void* workspace
   const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
   k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
   int launches = 1;
-  const int passes = (io.flags && io.lnK0) ? 2 : 1;
+  const int passes = (io.flags && io.lnK0 && !o.stability_only) ? 2 : 1;
   for (int pass = 0; pass < passes; ++pass) {
     w.pass = pass;
     if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
@@ -493,8 +563,13 @@ int launch_staged(const SysHost& hs, const Opt& o, const Io& io, void* workspace
     k_stab_ss<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
     k_stab_newton<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
     k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-    k_split_ss<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-    k_split_newton<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    if (o.stability_only) {
+      k_label_only<NC><<<gN, threads, 0, st>>>(io, w);
+      launches -= 1;
+    } else {
+      k_split_ss<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+      k_split_newton<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+    }
     k_finalize_counters<<<1, 32, 0, st>>>(w);
     launches += 7;
   }

@@ -13,9 +13,13 @@ P = P_b (1 + 0.05 (2u - 1)) clipped to [5, 300].
 """
 from __future__ import annotations
 
+import sys
+from pathlib import Path
+
 import numpy as np
 
-from paper_2205_03090_b200 import workloads as W
+sys.path.insert(0, str(Path(__file__).resolve().parents[1]))   # also runnable as a script (see the bottom of the file)
+from paper_2205_03090_b200 import workloads as W  # noqa: E402
 
 SEED = W.SEEDS[5]
 N_GRID = 28
@@ -103,3 +107,14 @@ def build_cached(oracle, N: int, cache_dir: str = ""):
     except OSError:
         pass
     return w, lnK0, flags, info
+
+
+if __name__ == "__main__":
+    # python tests/config5.py N OUT.npz -- writes the INPUTS of config 5 (P, T, z, lnK0, flags; no expected values) for
+    # `bench.py --config 5`, which runs this script in a process of its own so that the benchmark process never imports oracle/.
+    from oracle import oracle as O
+    O.build("double")
+    n_mix, out_path = int(sys.argv[1]), sys.argv[2]
+    w_, l0_, fl_, info_ = build(O.Oracle.from_system(W.system_co2_10()), n_mix, batch=min(65536, max(4096, n_mix // 8)))
+    np.savez(out_path, P=w_.P, T=w_.T, z=w_.z, lnK0=l0_, flags=fl_, two=info_["cold"]["phase"] == 2)
+    print(f"config 5: {n_mix} mixtures, two-phase share {info_['two_phase_fraction']:.4f}, acceptance {info_['acceptance']:.3f} -> {out_path}")

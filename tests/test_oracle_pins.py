@@ -508,14 +508,16 @@ def test_warm_start_and_skip_stability(sys10):
     assert np.array_equal(warm["phase"], cold["phase"])
     assert np.abs(warm["beta"] - cold["beta"])[two].max() < 1e-8
     assert warm["iters"][two].mean() < cold["iters"][two].mean()
-    # reading C21: a hint that fails (here: successive substitution still outside 0 < theta < 1 after hint_ss_cap = 30
-    # iterations, or a trivial / capped split) is dropped, reported (status bit 64) and the mixture flashed cold
+    # reading C21: a hint that fails (successive substitution still outside 0 < theta < 1 after hint_ss_cap = 12 iterations,
+    # no convergence within hint_tr_cap = 15 trust-region iterations, or a trivial split) is dropped, reported (status bit 64)
+    # and the mixture flashed cold
     restarted = (warm["status"] & 64) != 0
     assert restarted.sum() < 0.01 * two.sum() and not np.any(restarted & ~two)
     assert np.all(warm["stab_iters"][two & ~restarted] == 0)
     assert np.array_equal(warm["stab_iters"][restarted], cold["stab_iters"][restarted])
-    # the 30-iteration rule only cuts short splits that would fail anyway: with the rule off (cap = SS cap) the answers agree
-    slow = sys10.flash(w.z, w.P, w.T, lnK0=lnK0, flags=flags, nthreads=8, opts=dict(hint_ss_cap=100000))
+    # the two hint caps only cut short splits whose outcome does not change: with the rules off (caps = the general caps) the
+    # answers agree, and only hints that were dropped can survive
+    slow = sys10.flash(w.z, w.P, w.T, lnK0=lnK0, flags=flags, nthreads=8, opts=dict(hint_ss_cap=100000, hint_tr_cap=60))
     assert np.array_equal(slow["phase"], warm["phase"]) and np.abs(slow["beta"] - warm["beta"])[two].max() < 1e-8
     assert np.all(((slow["status"] & 64) != 0) <= restarted)
 
