@@ -115,6 +115,20 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
                        double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
                        void* stream);
 
+/* Pipelined host-buffer variant for a stream of batches (what a simulator or a data-generation loop submits): the call
+ * enqueues the H2D copies of the inputs, the flash kernels and the D2H copies of the results of ONE batch on an internal
+ * stream and returns without waiting.  Up to PTFLASH_HOST_DEPTH batches are in flight, each on a stream and a workspace of
+ * its own, so the copies of one batch run under the kernels of its neighbours (PCIe is full duplex); a call first waits for
+ * the batch submitted PTFLASH_HOST_DEPTH calls earlier.  The host buffers of a batch (pinned memory needed) must stay
+ * valid, and its outputs are defined, only after ptflash_host_wait -- or after PTFLASH_HOST_DEPTH later submissions.  Use
+ * distinct output buffers for batches that can be in flight together.  ptflash_get_stats reports the most recent batch.
+ * Returns PTFLASH_OK / EINVAL / ECUDA. */
+#define PTFLASH_HOST_DEPTH 3
+int ptflash_flash_host_async(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T,
+                             double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters);
+/* Blocks until every batch submitted with ptflash_flash_host_async has completed (its results are in the host buffers). */
+int ptflash_host_wait(ptflash_handle_t h);
+
 /* Synchronises the handle's last stream, frees constants and workspace.  NULL is a no-op. */
 int ptflash_destroy(ptflash_handle_t h);
 

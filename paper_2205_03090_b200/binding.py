@@ -20,7 +20,7 @@ OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial
            "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol", "stability_only", "host_chunks", "hint_eta_search", "hint_tr_cap"]
 EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
            "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_get_stage_ms", "ptflash_fp64_peak",
-           "ptflash_last_error", "ptflash_version", "ptflash_math_probe", "ptflash_rachford_rice"]
+           "ptflash_last_error", "ptflash_version", "ptflash_math_probe", "ptflash_rachford_rice", "ptflash_flash_host_async", "ptflash_host_wait"]
 
 
 class PTFlashError(RuntimeError):
@@ -71,6 +71,10 @@ def load_library():
     L.ptflash_flash_ex.argtypes = [vp, C.POINTER(_Io), vp]
     L.ptflash_flash_host.restype = C.c_int
     L.ptflash_flash_host.argtypes = [vp, i64] + [vp] * 9
+    L.ptflash_flash_host_async.restype = C.c_int
+    L.ptflash_flash_host_async.argtypes = [vp, i64] + [vp] * 8
+    L.ptflash_host_wait.restype = C.c_int
+    L.ptflash_host_wait.argtypes = [vp]
     L.ptflash_destroy.restype = C.c_int
     L.ptflash_destroy.argtypes = [vp]
     L.ptflash_set_option.restype = C.c_int
@@ -151,6 +155,15 @@ def ptflash_flash_host(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_ite
     _check(load_library().ptflash_flash_host(h, int(N), _ptr(z), _ptr(P), _ptr(T), _ptr(out_beta), _ptr(out_x),
                                              _ptr(out_y), _ptr(out_phase), _ptr(out_iters), _stream(stream)),
            "ptflash_flash_host")
+
+
+def ptflash_flash_host_async(h, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=None):
+    _check(load_library().ptflash_flash_host_async(h, int(N), _ptr(z), _ptr(P), _ptr(T), _ptr(out_beta), _ptr(out_x),
+                                                   _ptr(out_y), _ptr(out_phase), _ptr(out_iters)), "ptflash_flash_host_async")
+
+
+def ptflash_host_wait(h):
+    _check(load_library().ptflash_host_wait(h), "ptflash_host_wait")
 
 
 def ptflash_rachford_rice(h, N, lnK, z, out_theta, out_x=None, out_y=None, out_dtheta_dK=None, stream=None):

@@ -14,6 +14,7 @@
 namespace {
 
 #define PTF_MAX_HOST_CHUNKS 8
+#define PTF_HOST_DEPTH PTFLASH_HOST_DEPTH
 thread_local std::string g_err;
 void set_err(const std::string& s) { g_err = s; }
 bool cuda_ok(cudaError_t e, const char* what) {
@@ -60,6 +61,13 @@ struct ptflash_handle_s {
   int n_child;
   bool host_stats;       // the last call was a chunked ptflash_flash_host: statistics are the sum over the children
   int host_chunks_used;
+  // ptflash_flash_host_async: PTFLASH_HOST_DEPTH batches in flight, each on a child handle with a stream of its own
+  ptflash_handle_s* aslot[PTF_HOST_DEPTH];
+  cudaStream_t astream[PTF_HOST_DEPTH];
+  cudaEvent_t adone[PTF_HOST_DEPTH];
+  int n_aslot;
+  long long a_submitted;   // batches submitted so far
+  int a_last;              // slot of the most recent batch (-1: the last call was not an async one)
 };
 
 namespace {
@@ -190,6 +198,7 @@ ptflash_handle_t ptflash_create(int nc, const double* Tc, const double* Pc, cons
     }
   }
   std::memcpy(h->opts, kDefaultOpts, sizeof(kDefaultOpts));
+  h->a_last = -1;
   if (!cuda_ok(cudaMallocHost((void**)&h->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete h; return nullptr; }
   std::memset(h->counters_host, 0, sizeof(ptf::StageCounters));
   return h;
@@ -213,6 +222,12 @@ int ptflash_destroy(ptflash_handle_t h) {
     cudaEventDestroy(h->child_done[c]);
   }
   if (h->n_child) cudaEventDestroy(h->host_begin);
+  for (int c = 0; c < h->n_aslot; ++c) {
+    cudaStreamSynchronize(h->astream[c]);
+    ptflash_destroy(h->aslot[c]);
+    cudaStreamDestroy(h->astream[c]);
+    cudaEventDestroy(h->adone[c]);
+  }
   delete h;
   return rc;
 }
@@ -307,6 +322,7 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
   h->last_N = io->N;
   h->last_launches = launches;
   h->host_stats = false;
+  h->a_last = -1;
   return PTFLASH_OK;
 }
 
@@ -397,6 +413,79 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
   h->last_launches = launches;
   h->host_stats = true;
   h->host_chunks_used = chunks;
+  h->a_last = -1;
+  return PTFLASH_OK;
+}
+
+// Pipelined host-buffer variant: batch k's H2D copies, kernels and D2H copies are ordered on the stream of slot k mod DEPTH;
+// the slots' streams overlap, so the copies of one batch run under the kernels of its neighbours (PCIe is full duplex).
+int ptflash_flash_host_async(ptflash_handle_t h, int64_t N, const double* z, const double* P, const double* T, double* out_beta,
+                             double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters) {
+  g_err.clear();
+  if (!h) { set_err("ptflash_flash_host_async: null handle"); return PTFLASH_EINVAL; }
+  if (N < 0) { set_err("ptflash_flash_host_async: N < 0"); return PTFLASH_EINVAL; }
+  if (N == 0) return PTFLASH_OK;
+  if (N > PTFLASH_MAX_N) { set_err("ptflash_flash_host_async: N exceeds PTFLASH_MAX_N (2^30 - 1); split the batch"); return PTFLASH_EINVAL; }
+  if (!z || !P || !T || !out_beta || !out_x || !out_y || !out_phase) { set_err("ptflash_flash_host_async: null required pointer"); return PTFLASH_EINVAL; }
+  DeviceGuard guard(h->device);
+  const int nc = h->sys.nc;
+  const int slot = (int)(h->a_submitted % PTF_HOST_DEPTH);
+  while (h->n_aslot <= slot) {
+    const int c = h->n_aslot;
+    ptflash_handle_s* k = new ptflash_handle_s();
+    std::memset(k, 0, sizeof(*k));
+    k->device = h->device;
+    k->sys = h->sys;
+    k->a_last = -1;
+    if (!cuda_ok(cudaMallocHost((void**)&k->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete k; return PTFLASH_ECUDA; }
+    std::memset(k->counters_host, 0, sizeof(ptf::StageCounters));
+    if (!cuda_ok(cudaStreamCreateWithFlags(&h->astream[c], cudaStreamNonBlocking), "cudaStreamCreate")) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaEventCreateWithFlags(&h->adone[c], cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+    h->aslot[c] = k;
+    h->n_aslot = c + 1;
+  }
+  ptflash_handle_s* k = h->aslot[slot];
+  cudaStream_t cs = h->astream[slot];
+  // the slot's previous batch (DEPTH submissions ago) must have left its staging buffers
+  if (h->a_submitted >= PTF_HOST_DEPTH && !cuda_ok(cudaEventSynchronize(h->adone[slot]), "cudaEventSynchronize")) return PTFLASH_ECUDA;
+  std::memcpy(k->opts, h->opts, sizeof(k->opts));
+  const size_t nd = (size_t)N;
+  const size_t need = nd * (size_t)(nc + 2 + 1 + 2 * nc) * sizeof(double) + 2 * nd * sizeof(int32_t);
+  if (!ensure(&k->stage, &k->stage_bytes, need, cs, "cudaMalloc(staging)")) return PTFLASH_ECUDA;
+  double* dz = (double*)k->stage;
+  double* dP = dz + nd * nc;
+  double* dT = dP + nd;
+  double* dbeta = dT + nd;
+  double* dx = dbeta + nd;
+  double* dy = dx + nd * nc;
+  int32_t* dphase = (int32_t*)(dy + nd * nc);
+  int32_t* diters = dphase + nd;
+  if (!cuda_ok(cudaMemcpyAsync(dz, z, nd * nc * sizeof(double), cudaMemcpyHostToDevice, cs), "H2D z")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(dP, P, nd * sizeof(double), cudaMemcpyHostToDevice, cs), "H2D P")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(dT, T, nd * sizeof(double), cudaMemcpyHostToDevice, cs), "H2D T")) return PTFLASH_ECUDA;
+  const int rc = ptflash_flash(k, N, dz, dP, dT, dbeta, dx, dy, dphase, out_iters ? diters : nullptr, cs);
+  if (rc != PTFLASH_OK) return rc;
+  if (!cuda_ok(cudaMemcpyAsync(out_beta, dbeta, nd * sizeof(double), cudaMemcpyDeviceToHost, cs), "D2H beta")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(out_x, dx, nd * nc * sizeof(double), cudaMemcpyDeviceToHost, cs), "D2H x")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(out_y, dy, nd * nc * sizeof(double), cudaMemcpyDeviceToHost, cs), "D2H y")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaMemcpyAsync(out_phase, dphase, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, cs), "D2H phase")) return PTFLASH_ECUDA;
+  if (out_iters && !cuda_ok(cudaMemcpyAsync(out_iters, diters, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, cs), "D2H iters")) return PTFLASH_ECUDA;
+  if (!cuda_ok(cudaEventRecord(h->adone[slot], cs), "cudaEventRecord")) return PTFLASH_ECUDA;
+  h->a_submitted++;
+  h->a_last = slot;
+  h->used = true;
+  h->last_stream = cs;
+  h->last_N = N;
+  h->last_launches = k->last_launches;
+  h->host_stats = false;
+  return PTFLASH_OK;
+}
+
+int ptflash_host_wait(ptflash_handle_t h) {
+  if (!h) { set_err("ptflash_host_wait: null handle"); return PTFLASH_EINVAL; }
+  DeviceGuard guard(h->device);
+  for (int c = 0; c < h->n_aslot; ++c)
+    if (!cuda_ok(cudaStreamSynchronize(h->astream[c]), "cudaStreamSynchronize")) return PTFLASH_ECUDA;
   return PTFLASH_OK;
 }
 
@@ -434,6 +523,8 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
       const size_t n_add = offsetof(ptf::StageCounters, max_probe) / sizeof(long long), n_all = sizeof(sum) / sizeof(long long);
       for (size_t i = 0; i < n_all; ++i) b[i] = (i < n_add) ? b[i] + a[i] : (a[i] > b[i] ? a[i] : b[i]);
     }
+  } else if (h->a_last >= 0) {
+    sum = *h->aslot[h->a_last]->counters_host;   // the most recent pipelined batch
   } else {
     sum = *h->counters_host;
   }
@@ -453,7 +544,10 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
     for (int k = 0; k < 2; ++k) {
       out->n_stab_tr[k] = c.n_stab_tr[k];
       out->n_stab_capped[k] = c.n_stab_capped[k];
+      // trials that went on to the trust-region stage did all stab_ss_iters SS iterations (counted off the hot path)
       out->max_stab_ss_iters[k] = (int32_t)c.max_stab_ss[k];
+      if (c.n_stab_tr[k] > 0 && out->max_stab_ss_iters[k] < (int32_t)h->opts[PTFLASH_OPT_STAB_SS_ITERS])
+        out->max_stab_ss_iters[k] = (int32_t)h->opts[PTFLASH_OPT_STAB_SS_ITERS];
       out->max_stab_tr_iters[k] = (int32_t)c.max_stab_tr[k];
     }
     out->n_split_capped = c.n_split_capped;

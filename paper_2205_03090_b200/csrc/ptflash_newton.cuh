@@ -160,7 +160,8 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
   double* const sr = sp + NC * NEWTON_THREADS;   // residual r_i = ln W_i + lnphi_i(w) - d_i at the evaluated point
   double* const sdd = sr + NC * NEWTON_THREADS;  // d_i = ln z_i + lnphi_i(z) of the lane's mixture
   const int64_t N = io.N;
-  const int total = w.qcount[Q_STAB_NEWTON];
+  const int n_front = w.qcount[Q_STAB_NEWTON];           // trials expected to be long (k2_stab_ss): taken first
+  const int total = n_front + w.qcount[Q_STAB_NEWTON_E];  // the others sit at the end of the same array
   int* ticket = &w.qcount[Q_TICKET_STAB];
   // ---- lane state (scalars only) ----
   bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false;
@@ -180,7 +181,7 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
       const int64_t tk = take_ticket(!busy && !exhausted, ticket);
       if (tk >= 0) {
         if (tk < total) {
-          const int item = w.q_stab_newton[tk];
+          const int item = w.q_stab_newton[tk < n_front ? tk : 2 * N - 1 - (tk - n_front)];
           n = item >> 1;
           sidx = item & 1;
           const double P = io.P[n], T = io.T[n];
@@ -414,7 +415,8 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   double* const sD = sg + NC * T;    // D_i = z_i / (x_i y_i)
   double* const sS = sD + NC * T;    // S(x) [NC], S(y) [NC]
   const int64_t N = io.N;
-  const int total = w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON];
+  const int n_front = w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON];           // slow-SS splits (k2_split_ss): taken first
+  const int total = n_front + w.qcount[part ? Q_SPLIT_NEWTON_BE : Q_SPLIT_NEWTON_E];   // the others sit at the end of the array
   const int* const q_in = part ? w.q_split_newton_b : w.q_split_newton;
   int* ticket = &w.qcount[part ? Q_TICKET_SPLIT_B : Q_TICKET_SPLIT];
   bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false, polish = false;
@@ -438,7 +440,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       const int64_t tk = take_ticket(!busy && !exhausted, ticket);
       if (tk >= 0) {
         if (tk < total) {
-          n = q_in[tk];
+          n = q_in[tk < n_front ? tk : N - 1 - (tk - n_front)];
           const double P = io.P[n], Tk = io.T[n];
           { const double iT = rcp_fast(Tk); q.sT = sqrt_fast(Tk); q.spt = sqrt_fast(P) * iT; q.pt = P * iT; }
           act = (unsigned)w.actmask[n];

@@ -111,21 +111,26 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
 #define PTF_SS_MINB 4
 #endif
 constexpr double LNW_ZERO = -1000.0;
+// Longest-processing-time-first order of the Newton stage: a trial that is still further than this from the trivial solution
+// (max_i |ln W_i - ln z_i|) after the SS iterations is queued at the front.  On config 3 that is 13 % of the trials and it
+// contains every trial that needs >= 8 trust-region iterations (87 % of those with >= 5): started first, they no longer
+// form the tail of the persistent kernel.
+constexpr double STAB_HARD_DIST = 0.3;
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                const __grid_constant__ Io io, const __grid_constant__ Work w) {
   __shared__ double s_d[NC * 128];
+  __shared__ double s_lz[NC * 128];
   __shared__ double s_exp[PTF_EXP_TAB];
   exp_tab_init(s_exp);
   double* const sd = s_d + threadIdx.x;
+  double* const slz = s_lz + threadIdx.x;
   const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
-  // Table-4 counters: a thread always works on the same start (the grid stride is even, so idx & 1 == threadIdx.x & 1)
-  int my_tr = 0, my_cap = 0, my_max = 0;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    bool need_newton = false, capped = false;
+    bool need_newton = false, capped = false, hard = false;
     int item = 0, iters = 0;
     if (in) {
       const int n = w.q_stab[idx >> 1];
@@ -143,7 +148,9 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
         const double side = sidx ? -1.0 : 1.0;
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
-          lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], w.lnz[(int64_t)i * N + n]) : LNW_ZERO;
+          const double lz = w.lnz[(int64_t)i * N + n];
+          slz[i * 128] = lz;
+          lnW[i] = ((act >> i) & 1u) ? fma(side, lnKs[i], lz) : LNW_ZERO;
           sd[i * 128] = __ldg(&w.d[(int64_t)i * N + n]);
         }
       }
@@ -185,6 +192,12 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
         if (k == ss_max - 1 && o.use_newton) break;   // hand-over to the Newton stage after ss_max updates: no further evaluation needed here
       }
       need_newton = !converged && o.use_newton;
+      {
+        double dist = 0.0;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) dist = dmax(dist, ((act >> i) & 1u) ? fabs(lnW[i] - slz[i * 128]) : 0.0);
+        hard = dist > STAB_HARD_DIST;
+      }
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
         const bool a = (act >> i) & 1u;
@@ -196,19 +209,16 @@ __global__ void __launch_bounds__(128, PTF_SS_MINB) k2_stab_ss(const __grid_cons
       w.tflags[(int64_t)sidx * N + n] = (converged ? TF_CONVERGED : 0) | (capped ? TF_CAPPED : 0) | (iters << TF_ITER_SHIFT);
       if (need_newton) w.Zw[(int64_t)sidx * N + n] = e.Z;
     }
-    my_tr += need_newton ? 1 : 0;
-    my_cap += capped ? 1 : 0;
-    my_max = max(my_max, iters);
-    queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
-  }
-  {
-    const bool odd = threadIdx.x & 1;
-    flush_add(odd ? 0 : my_tr, &w.ctr->n_stab_tr[0]);
-    flush_add(odd ? my_tr : 0, &w.ctr->n_stab_tr[1]);
-    flush_add(odd ? 0 : my_cap, &w.ctr->n_stab_capped[0]);
-    flush_add(odd ? my_cap : 0, &w.ctr->n_stab_capped[1]);
-    flush_max(odd ? 0 : my_max, &w.ctr->max_stab_ss[0]);
-    flush_max(odd ? my_max : 0, &w.ctr->max_stab_ss[1]);
+    // Table-4 counters off the hot path: only a trial that ENDS here (converged within the SS cap, or capped in pure-SS
+    // mode: 0.7 % of the trials of config 3) touches a counter; the trials that go on are counted per start by k_stab_decide,
+    // and their SS iteration count is the cap itself (ptflash_get_stats folds that in)
+    if (in && !need_newton) {
+      atomicMax((unsigned long long*)&w.ctr->max_stab_ss[item & 1], (unsigned long long)iters);
+      if (capped) atomicAdd((unsigned long long*)&w.ctr->n_stab_capped[item & 1], 1ull);
+    }
+    // hard trials from the front of the array, the others from its end (the Newton stage takes the front first)
+    queue_push(need_newton && hard, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
+    queue_push_back(need_newton && !hard, &w.qcount[Q_STAB_NEWTON_E], w.q_stab_newton + 2 * N - 1, item);
   }
 }
 
@@ -252,6 +262,10 @@ struct EtaSearch {
   }
 };
 
+// Longest-processing-time-first order of the split Newton stage: a split whose last SS step contracted by less than this
+// factor is queued at the front.  On config 3 that is 4.5 % of the Newton items and every one that needs >= 6 iterations.
+constexpr double SPLIT_SLOW_RATE = 0.8;
+
 // ---- K5: phase-split SS ---------------------------------------------------------------------------
 template <int NC>
 __device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, const double (&z)[NC], bool converged,
@@ -274,7 +288,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
   int my_max = 0;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    bool go_newton = false;
+    bool go_newton = false, slow = false;
     int n = 0, k = 0, status = 0;
     if (in) {
       n = q_in[idx];
@@ -326,6 +340,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         for (int i = 0; i < NC; ++i)
           if (z[i] > 0.0) { const double nk = lpx[i] - lpy[i]; rk = dmax(rk, fabs(nk - lnK[i])); lnK[i] = nk; }
         ++k;
+        slow = r_prev > 0.0 && rk > SPLIT_SLOW_RATE * r_prev;
         if (rk < 1.0e-14) final_rr = true;
         else if (r_prev > 0.0 && rk < o.tol_ss) {
           const double rho = rk * rcp_fast(r_prev);   // linear-convergence error estimate eps = r rho / (1 - rho)
@@ -351,7 +366,11 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
     }
     my_max = max(my_max, k);
     count_add((status & ST_SPLIT_CAP) != 0, &w.ctr->n_split_capped);   // rare: no atomic unless a lane hit the cap
-    queue_push(go_newton, &w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON], part ? w.q_split_newton_b : w.q_split_newton, n);
+    // longest first: splits whose successive substitution was still contracting slowly (near-critical mixtures) are queued at
+    // the front of the array, the others from its end (the Newton stage takes the front first)
+    queue_push(go_newton && slow, &w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON], part ? w.q_split_newton_b : w.q_split_newton, n);
+    queue_push_back(go_newton && !slow, &w.qcount[part ? Q_SPLIT_NEWTON_BE : Q_SPLIT_NEWTON_E],
+                    (part ? w.q_split_newton_b : w.q_split_newton) + N - 1, n);
   }
   flush_max(my_max, &w.ctr->max_split_ss);
 }

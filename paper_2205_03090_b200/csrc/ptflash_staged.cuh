@@ -30,7 +30,9 @@ namespace ptf {
 // mixtures the stability analysis found unstable (Q_*_B).  Engine 1 runs part 0 on a second stream, concurrently with
 // the stability kernels; the plain stage kernels (launch_staged) use part 0 for both.
 enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_RETRY = 7,
-              Q_SPLIT_B = 8, Q_SPLIT_NEWTON_B = 9, Q_TICKET_SPLIT_B = 10, Q_COUNT = 11 };
+              Q_SPLIT_B = 8, Q_SPLIT_NEWTON_B = 9, Q_TICKET_SPLIT_B = 10,
+              Q_STAB_NEWTON_E = 11 /* fast engine: trials expected to be short, stored from the END of q_stab_newton */,
+              Q_SPLIT_NEWTON_E = 12, Q_SPLIT_NEWTON_BE = 13 /* the same for the two split queues */, Q_COUNT = 14 };
 enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_BETA = 8, TF_ITER_SHIFT = 8 + 0 };
 
 struct Work {
@@ -99,6 +101,19 @@ __device__ __forceinline__ void queue_push(bool pred, int* __restrict__ count, i
   if (lane == leader) base = atomicAdd(count, __popc(mask));
   base = __shfl_sync(active, base, leader);
   if (pred) queue[base + __popc(mask & ((1u << lane) - 1u))] = value;
+}
+
+// the same, filling the array downwards from `last` (two queues can share one array, one from each end)
+__device__ __forceinline__ void queue_push_back(bool pred, int* __restrict__ count, int* __restrict__ last, int value) {
+  const unsigned active = __activemask();
+  const unsigned mask = __ballot_sync(active, pred);
+  if (mask == 0u) return;
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(mask) - 1;
+  int base = 0;
+  if (lane == leader) base = atomicAdd(count, __popc(mask));
+  base = __shfl_sync(active, base, leader);
+  if (pred) last[-(int64_t)(base + __popc(mask & ((1u << lane) - 1u)))] = value;
 }
 
 __device__ __forceinline__ void count_add(bool pred, long long* ctr) {
@@ -338,6 +353,7 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
   const int64_t cnt = w.qcount[Q_STAB];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
+  int my_tr = 0;   // trials that came back from the trust-region stage: vapour-like in the low, liquid-like in the high half
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
     bool unstable = false;
@@ -354,6 +370,7 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
 #pragma unroll
       for (int i = 0; i < NC; ++i) { sv.lnW[i] = w.lnW[(int64_t)i * N + n]; sl.lnW[i] = w.lnW[((int64_t)NC + i) * N + n]; }
       const int fv = w.tflags[n], fl_ = w.tflags[N + n];
+      my_tr += ((fv & TF_BETA) ? 1 : 0) + ((fl_ & TF_BETA) ? 65536 : 0);
       // trials finished by the Newton stage come back as beta = 2 sqrt(W) (B.1a): ln W = 2 ln(beta / 2)
       if (fv & TF_BETA) {
 #pragma unroll
@@ -385,6 +402,8 @@ __global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys
     }
     queue_push(unstable, &w.qcount[w.decide_part ? Q_SPLIT_B : Q_SPLIT], w.decide_part ? w.q_split_b : w.q_split, n);
   }
+  flush_add(my_tr & 0xffff, &w.ctr->n_stab_tr[0]);
+  flush_add(my_tr >> 16, &w.ctr->n_stab_tr[1]);
 }
 
 // ---- K5 / K6 --------------------------------------------------------------------------------------
@@ -500,9 +519,9 @@ __global__ void __launch_bounds__(128) k_label_only(const __grid_constant__ Io i
 static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     w.ctr->n_stab += w.qcount[Q_STAB];
-    w.ctr->n_stab_newton += w.qcount[Q_STAB_NEWTON];
+    w.ctr->n_stab_newton += w.qcount[Q_STAB_NEWTON] + w.qcount[Q_STAB_NEWTON_E];
     w.ctr->n_split += w.qcount[Q_SPLIT] + w.qcount[Q_SPLIT_B];
-    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_B];
+    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_B] + w.qcount[Q_SPLIT_NEWTON_E] + w.qcount[Q_SPLIT_NEWTON_BE];
   }
 }
 
@@ -513,9 +532,10 @@ static __global__ void k_begin_pass2(const __grid_constant__ Work w) {
   __syncthreads();
   if (threadIdx.x == 0) {
     w.qcount[Q_PROBE] = cnt;
-    w.qcount[Q_STAB] = 0; w.qcount[Q_STAB_NEWTON] = 0; w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0;
+    w.qcount[Q_STAB] = 0; w.qcount[Q_STAB_NEWTON] = 0; w.qcount[Q_STAB_NEWTON_E] = 0; w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0;
     w.qcount[Q_TICKET_STAB] = 0; w.qcount[Q_TICKET_SPLIT] = 0; w.qcount[Q_RETRY] = 0;
     w.qcount[Q_SPLIT_B] = 0; w.qcount[Q_SPLIT_NEWTON_B] = 0; w.qcount[Q_TICKET_SPLIT_B] = 0;
+    w.qcount[Q_SPLIT_NEWTON_E] = 0; w.qcount[Q_SPLIT_NEWTON_BE] = 0;
     w.ctr->n_restart += cnt;   // number of warm restarts
   }
 }
@@ -530,10 +550,10 @@ static __global__ void k_requeue_failed_hints(const __grid_constant__ Work w) {
   if (threadIdx.x == 0) {
     w.ctr->n_restart += cnt;
     w.ctr->n_split += w.qcount[Q_SPLIT];
-    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON];
+    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_E];
     w.qcount[Q_PROBE] = base + cnt;
     w.qcount[Q_RETRY] = 0;
-    w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0; w.qcount[Q_TICKET_SPLIT] = 0;
+    w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0; w.qcount[Q_SPLIT_NEWTON_E] = 0; w.qcount[Q_TICKET_SPLIT] = 0;
   }
 }
 

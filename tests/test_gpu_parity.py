@@ -555,6 +555,40 @@ def test_parity_paper_workloads(oracle_mod, name, N):
           % (st["n_two_phase"] / N, st["n_probe_case3"] / N))
 
 
+def test_pipelined_host_call(oracle_mod):
+    """ptflash_flash_host_async / ptflash_host_wait: several batches in flight (different inputs, one output set per batch)
+    give bit-identical results to the device-buffer call, also when a slot is reused; sync host call alike (chunked)."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    N = 150_000
+    f = B.PTFlash.from_system(W.system_co2_10())
+    batches = [W.config3(N, offset=k * N) for k in range(5)]
+    ref = [_gpu_flash(w, 1) for w in batches]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    hin = [(pin(w.z), pin(w.P), pin(w.T)) for w in batches]
+    hout = [dict(beta=torch.empty(N, dtype=torch.float64).pin_memory(), x=torch.empty(10, N, dtype=torch.float64).pin_memory(),
+                 y=torch.empty(10, N, dtype=torch.float64).pin_memory(), phase=torch.empty(N, dtype=torch.int32).pin_memory(),
+                 iters=torch.empty(N, dtype=torch.int32).pin_memory()) for _ in batches]
+    for (z, P, T), o in zip(hin, hout):
+        B.ptflash_flash_host_async(f.h, N, z, P, T, o["beta"], o["x"], o["y"], o["phase"], o["iters"])
+    B.ptflash_host_wait(f.h)
+    for k, (o, r) in enumerate(zip(hout, ref)):
+        for key in ("beta", "x", "y", "phase", "iters"):
+            assert np.array_equal(o[key].numpy(), r[key], equal_nan=True), (k, key)
+    assert f.stats()["n_two_phase"] == int((ref[-1]["phase"] == 2).sum())
+    # the chunked synchronous call (4 chunks of 37,500 here) on the same handle
+    o = hout[0]
+    for key in o:
+        o[key].zero_()
+    z, P, T = hin[3]
+    B.ptflash_flash_host(f.h, N, z, P, T, o["beta"], o["x"], o["y"], o["phase"], o["iters"])
+    for key in ("beta", "x", "y", "phase", "iters"):
+        assert np.array_equal(o[key].numpy(), ref[3][key], equal_nan=True), key
+    st = f.stats()
+    assert st["n_total"] == N and st["n_two_phase"] == int((ref[3]["phase"] == 2).sum())
+    f.close()
+
+
 def test_second_device_keeps_current_device():
     """A handle created on cuda:1 is used and destroyed while cuda:0 is current: the caller's device is
     restored by every entry point and the results equal those of cuda:0."""
