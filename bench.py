@@ -47,7 +47,7 @@ WORKLOAD = WORKLOADS["3"]
 # DRAM bytes per launch.  They live in profiles/<tag>_flops.json, written by `bench.py --ncu-summary` from the ncu CSV of
 # that build together with a hash of the kernel sources; when the sources have changed since, the line says "flops_stale".
 STAGES = ("k_init", "k2_probe", "k2_stab_ss", "k3_stab_newton", "k_stab_decide", "k2_split_ss", "k3_split_newton")
-FLOPS_JSON = ROOT / "profiles" / "r02_flops.json"
+FLOPS_GLOB = "r02*_flops.json"   # the newest (by name) profile of this round; one is written per profiled build
 BYTES_PER_FLASH_NC10 = 272.0   # 8(nc+2) in + 8(2nc+1)+8 out, SURVEY.md section 8(d)
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # SMs x DFMA lanes/clk x 2 flop x max SM clock
 PAPER_TABLE4 = {"two_phase_share": 0.413442, "probe_proved_share": 0.3744, "seconds_per_1e6_on_RTX3080": 3.03,
@@ -68,10 +68,15 @@ def kernel_source_hash() -> str:
 def load_flops():
     """-> (per-stage flops per flash, total, traffic per call, traffic of the dominant kernel, stale?, source)"""
     try:
-        d = json.load(open(FLOPS_JSON))
+        cands = [json.load(open(f)) | {"file": f.name} for f in sorted((ROOT / "profiles").glob(FLOPS_GLOB))]
     except Exception:
         return None
-    d["stale"] = d.get("csrc_hash") != kernel_source_hash()
+    if not cands:
+        return None
+    h = kernel_source_hash()
+    match = [c for c in cands if c.get("csrc_hash") == h]
+    d = match[-1] if match else cands[-1]
+    d["stale"] = d.get("csrc_hash") != h
     return d
 
 
@@ -435,7 +440,7 @@ def main():
         achieved = fl["flops_per_flash"] * N / (ms_step * 1e-3) / 1e12
         roofline.update(achieved=achieved, frac=achieved / peak, flops_per_flash=fl["flops_per_flash"],
                         traffic=fl["traffic_call_bytes"] if N == 1_000_000 else None,
-                        flops_source=f"profiles/{FLOPS_JSON.name} (ncu count of build {fl['csrc_hash']})", flops_stale=bool(fl["stale"]))
+                        flops_source=f"profiles/{fl['file']} (ncu count of build {fl['csrc_hash']})", flops_stale=bool(fl["stale"]))
         if stage_ms:
             # the same figure per stage kernel; "dominant" = the kernel with the largest share of the step
             per = {}

@@ -33,11 +33,9 @@ int PTF_CAT(launch_mono_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io,
 }
 
 int PTF_CAT(launch_staged_, PTF_NC)(const SysHost& hs, const Opt& o, const Io& io, void* ws, cudaStream_t st) {
-  #if PTF_NC <= 12
-  // register-resident fast path (packed nc x nc systems fit the register file up to nc = 12)
-  if (o.use_newton) return launch_stage2<PTF_NC>(hs, o, io, ws, st);
-#endif
-  return launch_staged<PTF_NC>(hs, o, io, ws, st);
+  // every component count (2..16) and both modes (trust-region Newton / pure successive substitution) run the
+  // register-resident stage kernels; for nc >= 13 the Newton CTAs are limited by shared memory (one per SM at nc = 16)
+  return launch_stage2<PTF_NC>(hs, o, io, ws, st);
 }
 
 int PTF_CAT(launch_rr_, PTF_NC)(const RrIo& io, cudaStream_t st) { return launch_rr<PTF_NC>(io, st); }

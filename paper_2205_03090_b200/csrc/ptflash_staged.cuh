@@ -28,7 +28,7 @@ namespace ptf {
 
 // The phase split has two queue sets: part 0 = mixtures the probe (or the caller) sent straight to the split, part 1 =
 // mixtures the stability analysis found unstable (Q_*_B).  Engine 1 runs part 0 on a second stream, concurrently with
-// the stability kernels; the plain stage kernels (launch_staged) use part 0 for both.
+// the stability kernels.
 enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_RETRY = 7,
               Q_SPLIT_B = 8, Q_SPLIT_NEWTON_B = 9, Q_TICKET_SPLIT_B = 10,
               Q_STAB_NEWTON_E = 11 /* fast engine: trials expected to be short, stored from the END of q_stab_newton */,
@@ -122,14 +122,7 @@ __device__ __forceinline__ void count_add(bool pred, long long* ctr) {
   if (mask && (int)(threadIdx.x & 31) == __ffs(mask) - 1) atomicAdd((unsigned long long*)ctr, (unsigned long long)__popc(mask));
 }
 
-// running maximum of an iteration count (Table 4's "max number of iterations" row)
-__device__ __forceinline__ void count_max(bool pred, int v, long long* ctr) {
-  const unsigned active = __activemask();
-  const int m = __reduce_max_sync(active, pred ? v : 0);
-  if (m > 0 && (int)(threadIdx.x & 31) == __ffs(active) - 1) atomicMax((unsigned long long*)ctr, (unsigned long long)m);
-}
-
-// The same for kernels that see many items per thread: the thread keeps its own maximum / count in a register and the warp
+// Table 4's "max number of iterations" rows and the per-start counts: the thread keeps its own maximum / count in a register and the warp
 // publishes once, after its loop (all lanes converged), so the hot loop carries a compare instead of an atomic.
 __device__ __forceinline__ void flush_max(int v, long long* ctr) {
   const int m = __reduce_max_sync(0xffffffffu, v);
@@ -138,21 +131,6 @@ __device__ __forceinline__ void flush_max(int v, long long* ctr) {
 __device__ __forceinline__ void flush_add(int v, long long* ctr) {
   const int m = __reduce_add_sync(0xffffffffu, v);
   if (m > 0 && (threadIdx.x & 31) == 0) atomicAdd((unsigned long long*)ctr, (unsigned long long)m);
-}
-
-// context of a mixture already validated by K1a
-template <int NC>
-__device__ __forceinline__ void reload_ctx(const Sys<NC>& S, const Io& io, const Work& w, int n, bool need_ref, MixCtx<NC>& m,
-                                           double& P, double& T) {
-  load_feed<NC>(io, n, m.z, P, T);
-  eos_setup<NC>(S, P, T, m.sa, m.bi);
-  if (need_ref) {
-#pragma unroll
-    for (int i = 0; i < NC; ++i) {
-      m.lnz[i] = w.lnz[(int64_t)i * io.N + n];
-      m.d[i] = w.d[(int64_t)i * io.N + n];
-    }
-  }
 }
 
 #define PTF_GRID_STRIDE(idx, total) \
@@ -227,122 +205,6 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
     queue_push(dest == 0, &w.qcount[Q_PROBE], w.q_probe, n);
     queue_push(dest == 1, &w.qcount[Q_STAB], w.q_stab, n);
     queue_push(dest == 2, &w.qcount[Q_SPLIT], w.q_split, n);
-  }
-}
-
-// ---- K1b ------------------------------------------------------------------------------------------
-template <int NC>
-__global__ void __launch_bounds__(128) k_probe(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                               const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  const int64_t cnt = w.qcount[Q_PROBE];
-  const int64_t pad = (cnt + 31) & ~(int64_t)31;
-  PTF_GRID_STRIDE(idx, pad) {
-    const bool in = idx < cnt;
-    int pcase = 0, n = 0, iters = 0;
-    if (in) {
-      n = w.q_probe[idx];
-      MixCtx<NC> m;
-      double P, T;
-      reload_ctx<NC>(S, io, w, n, true, m, P, T);
-      int status = w.status[n] & ST_WARM_RESTART, fl = 0;
-      double lnK[NC];
-      start_lnK<NC>(S, io, n, P, T, lnK, fl, status);
-      double tpd_min = 0.0;
-      pcase = probe<NC>(S, o, m, lnK, tpd_min, iters);
-      w.iters[n] += iters;
-      if (pcase == 3) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = lnK[i];
-        w.tpdmin[n] = tpd_min;
-      }
-    }
-    count_add(pcase == 1, &w.ctr->n_case1);
-    count_add(pcase == 2, &w.ctr->n_case2);
-    count_add(pcase == 3, &w.ctr->n_case3);
-    count_max(in, iters, &w.ctr->max_probe);
-    queue_push(pcase == 1 || pcase == 2, &w.qcount[Q_STAB], w.q_stab, n);
-    queue_push(pcase == 3, &w.qcount[Q_SPLIT], w.q_split, n);
-  }
-}
-
-// Table-4 counters of the stability SS stage (called by all lanes of the warp)
-__device__ __forceinline__ void stab_ss_counters(const Work& w, bool in, int sidx, bool need_newton, bool capped, int iters) {
-  count_add(in && need_newton && sidx == 0, &w.ctr->n_stab_tr[0]);
-  count_add(in && need_newton && sidx == 1, &w.ctr->n_stab_tr[1]);
-  count_add(in && capped && sidx == 0, &w.ctr->n_stab_capped[0]);
-  count_add(in && capped && sidx == 1, &w.ctr->n_stab_capped[1]);
-  count_max(in && sidx == 0, iters, &w.ctr->max_stab_ss[0]);
-  count_max(in && sidx == 1, iters, &w.ctr->max_stab_ss[1]);
-}
-
-// ---- K2 -------------------------------------------------------------------------------------------
-template <int NC>
-__device__ __forceinline__ void store_trial(const Io& io, const Work& w, int n, int sidx, const StabState<NC>& st) {
-  const int64_t N = io.N;
-#pragma unroll
-  for (int i = 0; i < NC; ++i) w.lnW[((int64_t)sidx * NC + i) * N + n] = st.lnW[i];
-  w.tm[(int64_t)sidx * N + n] = st.tm;
-  w.sumW[(int64_t)sidx * N + n] = st.sumW;
-  w.tflags[(int64_t)sidx * N + n] = (st.converged ? TF_CONVERGED : 0) | (st.stationary_exact ? TF_EXACT : 0) |
-                                    (st.capped ? TF_CAPPED : 0) | (st.iters << TF_ITER_SHIFT);
-}
-
-template <int NC>
-__global__ void __launch_bounds__(128) k_stab_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                 const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  const int64_t cnt = 2 * (int64_t)w.qcount[Q_STAB];
-  const int64_t pad = (cnt + 31) & ~(int64_t)31;
-  PTF_GRID_STRIDE(idx, pad) {
-    const bool in = idx < cnt;
-    bool need_newton = false, capped = false;
-    int item = 0, ss_iters = 0;
-    if (in) {
-      const int n = w.q_stab[idx >> 1];
-      const int sidx = (int)(idx & 1);  // 0 vapour-like, 1 liquid-like
-      item = (n << 1) | sidx;
-      MixCtx<NC> m;
-      double P, T;
-      reload_ctx<NC>(S, io, w, n, true, m, P, T);
-      int status = w.status[n] & ST_WARM_RESTART, fl = 0;
-      double lnKs[NC];
-      start_lnK<NC>(S, io, n, P, T, lnKs, fl, status);
-      StabState<NC> st;
-      stab_init<NC>(m, lnKs, sidx ? -1.0 : 1.0, st);
-      stab_ss<NC>(S, o, m, st);
-      need_newton = !st.converged && o.use_newton;
-      capped = st.capped;
-      ss_iters = st.iters;
-      store_trial<NC>(io, w, n, sidx, st);
-    }
-    stab_ss_counters(w, in, item & 1, need_newton, capped, ss_iters);
-    queue_push(need_newton, &w.qcount[Q_STAB_NEWTON], w.q_stab_newton, item);
-  }
-}
-
-// ---- K3 -------------------------------------------------------------------------------------------
-template <int NC>
-__global__ void __launch_bounds__(128) k_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                     const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  const int64_t cnt = w.qcount[Q_STAB_NEWTON];
-  PTF_GRID_STRIDE(idx, cnt) {
-    const int item = w.q_stab_newton[idx];
-    const int n = item >> 1, sidx = item & 1;
-    MixCtx<NC> m;
-    double P, T;
-    reload_ctx<NC>(S, io, w, n, true, m, P, T);
-    StabState<NC> st;
-#pragma unroll
-    for (int i = 0; i < NC; ++i) st.lnW[i] = w.lnW[((int64_t)sidx * NC + i) * io.N + n];
-    st.tm = 0.0; st.sumW = 1.0;
-    const int it0 = w.tflags[(int64_t)sidx * io.N + n] >> TF_ITER_SHIFT;
-    st.iters = it0;
-    st.converged = false; st.stationary_exact = false; st.capped = false;
-    stab_newton<NC>(S, o, m, st);
-    store_trial<NC>(io, w, n, sidx, st);
-    count_add(st.capped && sidx == 0, &w.ctr->n_stab_capped[0]);
-    count_add(st.capped && sidx == 1, &w.ctr->n_stab_capped[1]);
-    count_max(sidx == 0, st.iters - it0, &w.ctr->max_stab_tr[0]);
-    count_max(sidx == 1, st.iters - it0, &w.ctr->max_stab_tr[1]);
   }
 }
 
@@ -427,74 +289,6 @@ __device__ __forceinline__ void finish_common(const Io& io, const Work& w, int n
   queue_push(retry, &w.qcount[Q_RETRY], w.q_retry, n);
 }
 
-template <int NC>
-__device__ __forceinline__ void finish_split(const Sys<NC>& S, const Io& io, const Work& w, int n, const MixCtx<NC>& m,
-                                             const SplitState<NC>& st, const double (&x)[NC], const double (&y)[NC]) {
-  SplitRes sp;
-  split_finish<NC>(st, sp);
-  const bool swap = sp.two_phase && phase_swap_by_Z<NC>(S, m, x, y);
-  finish_common<NC>(io, w, n, m.z, sp.two_phase, sp.theta, sp.iters, sp.status & ~ST_SPLIT_FAILED, x, y, st.lnK, swap);
-}
-
-template <int NC>
-__global__ void __launch_bounds__(128) k_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                  const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  const int64_t cnt = w.qcount[Q_SPLIT];
-  const int64_t pad = (cnt + 31) & ~(int64_t)31;
-  PTF_GRID_STRIDE(idx, pad) {
-    const bool in = idx < cnt;
-    bool go_newton = false, capped = false;
-    int n = 0, ss_iters = 0;
-    if (in) {
-      n = w.q_split[idx];
-      MixCtx<NC> m;
-      double P, T;
-      reload_ctx<NC>(S, io, w, n, false, m, P, T);
-      SplitState<NC> st;
-#pragma unroll
-      for (int i = 0; i < NC; ++i) st.lnK[i] = w.lnK[(int64_t)i * io.N + n];
-      double x[NC], y[NC];
-      split_ss<NC>(S, o, m, st, x, y, (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED));
-      go_newton = st.go_newton;
-      ss_iters = st.iters;
-      capped = (st.status & ST_SPLIT_CAP) != 0;
-      if (go_newton) {
-#pragma unroll
-        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * io.N + n] = st.lnK[i];
-        w.iters[n] += st.iters;
-        w.status[n] |= st.status;
-      } else {
-        finish_split<NC>(S, io, w, n, m, st, x, y);
-      }
-    }
-    count_max(in, ss_iters, &w.ctr->max_split_ss);
-    count_add(capped, &w.ctr->n_split_capped);
-    queue_push(go_newton, &w.qcount[Q_SPLIT_NEWTON], w.q_split_newton, n);
-  }
-}
-
-template <int NC>
-__global__ void __launch_bounds__(128) k_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
-                                                      const __grid_constant__ Io io, const __grid_constant__ Work w) {
-  const int64_t cnt = w.qcount[Q_SPLIT_NEWTON];
-  PTF_GRID_STRIDE(idx, cnt) {
-    const int n = w.q_split_newton[idx];
-    MixCtx<NC> m;
-    double P, T;
-    reload_ctx<NC>(S, io, w, n, false, m, P, T);
-    SplitState<NC> st;
-    double K[NC], x[NC], y[NC];
-#pragma unroll
-    for (int i = 0; i < NC; ++i) { st.lnK[i] = w.lnK[(int64_t)i * io.N + n]; K[i] = exp(st.lnK[i]); }
-    st.iters = 0; st.status = 0; st.converged = false; st.failed = false; st.go_newton = true;
-    rr_solve<NC>(K, m.z, st.theta, x, y);  // the same Rachford-Rice that ended the SS stage
-    split_newton<NC>(S, o, m, st, x, y, (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED));
-    count_max(true, st.iters, &w.ctr->max_split_tr);
-    count_add((st.status & ST_SPLIT_CAP) != 0, &w.ctr->n_split_capped);
-    finish_split<NC>(S, io, w, n, m, st, x, y);
-  }
-}
-
 // ---- stability-only mode --------------------------------------------------------------------------
 // PTFLASH_OPT_STABILITY_ONLY: the mixtures queued for the phase split (probe case 3, the caller's
 // "unstable" flag, or the stability verdict) are labelled instead of split; the stable ones were stored by k_stab_decide.
@@ -525,21 +319,6 @@ static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
   }
 }
 
-// second pass: the retry queue becomes the probe queue, every other queue and ticket restarts from zero
-static __global__ void k_begin_pass2(const __grid_constant__ Work w) {
-  const int cnt = w.qcount[Q_RETRY];
-  for (int i = threadIdx.x; i < cnt; i += blockDim.x) w.q_probe[i] = w.q_retry[i];
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    w.qcount[Q_PROBE] = cnt;
-    w.qcount[Q_STAB] = 0; w.qcount[Q_STAB_NEWTON] = 0; w.qcount[Q_STAB_NEWTON_E] = 0; w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0;
-    w.qcount[Q_TICKET_STAB] = 0; w.qcount[Q_TICKET_SPLIT] = 0; w.qcount[Q_RETRY] = 0;
-    w.qcount[Q_SPLIT_B] = 0; w.qcount[Q_SPLIT_NEWTON_B] = 0; w.qcount[Q_TICKET_SPLIT_B] = 0;
-    w.qcount[Q_SPLIT_NEWTON_E] = 0; w.qcount[Q_SPLIT_NEWTON_BE] = 0;
-    w.ctr->n_restart += cnt;   // number of warm restarts
-  }
-}
-
 // Warm-start calls of the fast engine: the splits entered through a skip-stability hint run FIRST; the hints that failed
 // (Q_RETRY, reading C21) then join the probe queue of the mixtures without a hint, so the whole call stays one pass.
 // The split queues and tickets restart from zero for the probe- and stability-found splits that follow.
@@ -555,45 +334,6 @@ static __global__ void k_requeue_failed_hints(const __grid_constant__ Work w) {
     w.qcount[Q_RETRY] = 0;
     w.qcount[Q_SPLIT] = 0; w.qcount[Q_SPLIT_NEWTON] = 0; w.qcount[Q_SPLIT_NEWTON_E] = 0; w.qcount[Q_TICKET_SPLIT] = 0;
   }
-}
-
-template <int NC>
-int launch_staged(const SysHost& hs, const Opt& o, const Io& io, void* workspace, cudaStream_t st) {
-  const Sys<NC> s = narrow<NC>(hs);
-  Work w;
-  carve_workspace(NC, io.N, (char*)workspace, &w);
-  if (cudaMemsetAsync(workspace, 0, align256(sizeof(StageCounters)) + align256(Q_COUNT * sizeof(int)), st) != cudaSuccess) return -1;
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  const int threads = 128;
-  auto grid_for = [&](int64_t items) {
-    const int64_t need = (items + threads - 1) / threads;
-    const int64_t cap = (int64_t)sms * 16;
-    return (unsigned)(need < cap ? (need > 0 ? need : 1) : cap);
-  };
-  const unsigned gN = grid_for(io.N), g2N = grid_for(2 * io.N);
-  k_init<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-  int launches = 1;
-  const int passes = (io.flags && io.lnK0 && !o.stability_only) ? 2 : 1;
-  for (int pass = 0; pass < passes; ++pass) {
-    w.pass = pass;
-    if (pass) { k_begin_pass2<<<1, 1024, 0, st>>>(w); ++launches; }
-    k_probe<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-    k_stab_ss<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
-    k_stab_newton<NC><<<g2N, threads, 0, st>>>(s, o, io, w);
-    k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-    if (o.stability_only) {
-      k_label_only<NC><<<gN, threads, 0, st>>>(io, w);
-      launches -= 1;
-    } else {
-      k_split_ss<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-      k_split_newton<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-    }
-    k_finalize_counters<<<1, 32, 0, st>>>(w);
-    launches += 7;
-  }
-  return cudaGetLastError() == cudaSuccess ? launches : -1;
 }
 
 }  // namespace ptf

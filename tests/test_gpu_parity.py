@@ -215,21 +215,23 @@ def test_invalid_and_degenerate_inputs(oracle_mod):
             assert g["stats"]["n_invalid"] == 6
 
 
-@pytest.mark.parametrize("names", [["C1", "C3", "nC10"], None])
-def test_other_component_counts(oracle_mod, names):
-    """nc = 3 (fast path) and nc = 16 (largest supported; engine 1 falls back to the local-memory Newton kernels)."""
-    if names is None:
-        names = W.HC8 + ["CO2", "N2"]
-        s10 = W.system_co2_10()
-        # 16 components: duplicate six alkanes with perturbed constants
-        Tc = np.concatenate([s10.Tc, s10.Tc[2:8] * 1.03]); Pc = np.concatenate([s10.Pc, s10.Pc[2:8] * 0.97])
-        om = np.concatenate([s10.omega, s10.omega[2:8] + 0.01])
-        kij = np.zeros((16, 16)); kij[:10, :10] = s10.kij
-        kij[10:, 8] = kij[8, 10:] = 0.12; kij[10:, 9] = kij[9, 10:] = 0.10
-        system = W.System([f"c{i}" for i in range(16)], Tc, Pc, om, kij)
-    else:
-        system = W.make_system(names)
-    nc, N = system.nc, 3000
+def _system_16(nc):
+    """Up to 16 components: the CO2-rich ten plus six alkanes duplicated with perturbed constants, truncated to nc."""
+    s10 = W.system_co2_10()
+    Tc = np.concatenate([s10.Tc, s10.Tc[2:8] * 1.03]); Pc = np.concatenate([s10.Pc, s10.Pc[2:8] * 0.97])
+    om = np.concatenate([s10.omega, s10.omega[2:8] + 0.01])
+    kij = np.zeros((16, 16)); kij[:10, :10] = s10.kij
+    kij[10:, 8] = kij[8, 10:] = 0.12; kij[10:, 9] = kij[9, 10:] = 0.10
+    return W.System([f"c{i}" for i in range(nc)], Tc[:nc], Pc[:nc], om[:nc], np.ascontiguousarray(kij[:nc, :nc]))
+
+
+@pytest.mark.parametrize("nc", [3, 13, 16])
+def test_other_component_counts(oracle_mod, nc):
+    """nc = 3, 13 and 16 (the largest supported): every component count runs the register-resident stage kernels of
+    engine 1 (10 launches per call: k_init, k2_probe, k2_stab_ss, k3_stab_newton, k_stab_decide, 2 x k2_split_ss,
+    2 x k3_split_newton, k_finalize_counters); for nc >= 13 the Newton CTAs are sized by shared memory."""
+    system = W.make_system(["C1", "C3", "nC10"]) if nc == 3 else _system_16(nc)
+    N = 3000
     n = np.arange(N)
     T = 220.0 + 300.0 * W.uniform(77, n, 0)
     P = 2.0 + 200.0 * W.uniform(77, n, 1)
@@ -237,18 +239,25 @@ def test_other_component_counts(oracle_mod, names):
     w = W.Workload("nc%d" % nc, system, P, T, np.ascontiguousarray(z))
     o = oracle_mod.Oracle.from_system(system).flash(w.z, w.P, w.T)
     for engine in (1, 0):
-        rep = check(w, _gpu_flash(w, engine), o)
+        g = _gpu_flash(w, engine)
+        rep = check(w, g, o)
         assert rep["two_phase"] > 100
+        if engine == 1:
+            assert g["stats"]["kernel_launches"] == 10 and g["stats"]["n_stab_newton"] > 0 and g["stats"]["n_split_newton"] > 0
 
 
-def test_pure_successive_substitution_mode(oracle_mod):
-    """use_newton = 0: every stage runs plain successive substitution (the north_star's SSI path)."""
-    w = W.config1(600)
-    opts = dict(use_newton=0, ss_cap=20000)
+@pytest.mark.parametrize("cfg,N", [(1, 600), (3, 1500)])
+def test_pure_successive_substitution_mode(oracle_mod, cfg, N):
+    """use_newton = 0: every stage runs plain successive substitution (the north_star's SSI path) on the same
+    register-resident stage kernels; the Newton stages find empty queues."""
+    w = W.CONFIGS[cfg](N)
+    opts = dict(use_newton=0, ss_cap=100000)
     o = oracle_mod.Oracle.from_system(w.system).flash(w.z, w.P, w.T, opts=opts)
     for engine in (1, 0):
         g = _gpu_flash(w, engine, **opts)
         check(w, g, o)
+        if engine == 1:
+            assert g["stats"]["n_stab_newton"] == 0 and g["stats"]["n_split_newton"] == 0
 
 
 def test_host_buffers_stream_and_stats(oracle_mod):
