@@ -276,6 +276,8 @@ def main():
     workload = WORKLOADS[args.config]
     nc = w.system.nc
     f = B.PTFlash.from_system(w.system, engine=args.engine)
+    for kv in filter(None, os.environ.get("PTFLASH_BENCH_OPTS", "").split(",")):   # development only: option overrides for experiments
+        f.set_option(kv.split("=")[0], float(kv.split("=")[1]))
     z, P, T = (torch.from_numpy(a).to(dev) for a in (w.z, w.P, w.T))
     f64 = dict(dtype=torch.float64, device=dev)
     i32 = dict(dtype=torch.int32, device=dev)

@@ -142,8 +142,17 @@ template <int NC>
 constexpr int newton_lrows() { return (NC - 1) * (NC - 2) / 2; }            // rows 1 .. NC-2 of the strict lower triangle
 template <int NC>
 constexpr int stabn_smem_doubles() { return newton_lrows<NC>() + 4 * NC; }   // per thread: L, beta, pending step, residual r, d
+// B200: 228 KB of shared memory per SM, 1 KB reserved per CTA, at most 227 KB per CTA; the 255-register kernels fit 2 CTAs
+constexpr int newton_ctas_by_smem(int doubles_per_thread) {
+  const int bytes = doubles_per_thread * NEWTON_THREADS * 8;
+  const int n = bytes > 232448 ? 0 : 233472 / (bytes + 1024);
+  return n > 2 ? 2 : n;
+}
+// the split kernel keeps the feed z in shared memory where that does not cost a resident CTA (else it is re-read through L1)
 template <int NC>
-constexpr int splitn_smem_doubles() { return newton_lrows<NC>() + 6 * NC; }  // per thread: L, n^V, pending step, g, D, S(x), S(y)
+constexpr bool split_z_in_smem() { return newton_ctas_by_smem(newton_lrows<NC>() + 7 * NC) == newton_ctas_by_smem(newton_lrows<NC>() + 6 * NC); }
+template <int NC>                                                              // per thread: L, n^V, pending step, g, D, S(x), S(y) [, z]
+constexpr int splitn_smem_doubles() { return newton_lrows<NC>() + (split_z_in_smem<NC>() ? 7 : 6) * NC; }
 
 // ---- K3: stability trust-region Newton (B.1-B.3), persistent warps with lane refill --------------
 template <int NC, bool KIJ0>
@@ -414,6 +423,8 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   double* const sg = sp + NC * T;    // gradient (B.5a) at the evaluated point
   double* const sD = sg + NC * T;    // D_i = z_i / (x_i y_i)
   double* const sS = sD + NC * T;    // S(x) [NC], S(y) [NC]
+  constexpr bool ZS = split_z_in_smem<NC>();
+  double* const sz = sS + 2 * NC * T;   // normalised feed z of the lane's mixture (read many times per trip), if it fits (ZS)
   const int64_t N = io.N;
   const int n_front = w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON];           // slow-SS splits (k2_split_ss): taken first
   const int total = n_front + w.qcount[part ? Q_SPLIT_NEWTON_BE : Q_SPLIT_NEWTON_E];   // the others sit at the end of the array
@@ -453,6 +464,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           for (int i = 0; i < NC; ++i) {
             sn[i * T] = w.lnK[(int64_t)i * N + n];   // k2_split_ss left n^V here
             sp[i * T] = 0.0;
+            if (ZS) sz[i * T] = __ldg(&w.zn[(int64_t)i * N + n]);
           }
           tr_it = 0;
           status = 0;
@@ -491,7 +503,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           const double v = sn[i * T] + sp[i * T];
-          c[i] = ph ? v * it : (__ldg(&w.zn[(int64_t)i * N + n]) - v) * il;
+          c[i] = ph ? v * it : ((ZS ? sz[i * T] : __ldg(&w.zn[(int64_t)i * N + n])) - v) * il;
         }
         Eos e;
         e.Z = ph ? ey.Z : ex.Z;
@@ -511,7 +523,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
             const double g = sg[i * T] + f;
             sg[i * T] = g;
             gmax = dmax(gmax, fabs(g));
-            sD[i * T] = a ? __ldg(&w.zn[(int64_t)i * N + n]) * rcp_fast(sD[i * T] * c[i]) : 1.0;
+            sD[i * T] = a ? (ZS ? sz[i * T] : __ldg(&w.zn[(int64_t)i * N + n])) * rcp_fast(sD[i * T] * c[i]) : 1.0;
           }
         }
       }
@@ -620,7 +632,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           s2 = fma(st[i], st[i], s2);
           sgd = fma(st[i], sg[i * T], sgd);
           const double ni = sn[i * T];
-          const double room = a ? dmax(st[i] < 0.0 ? ni : __ldg(&w.zn[(int64_t)i * N + n]) - ni, 1.0e-300) : 1.0;
+          const double room = a ? dmax(st[i] < 0.0 ? ni : (ZS ? sz[i * T] : __ldg(&w.zn[(int64_t)i * N + n])) - ni, 1.0e-300) : 1.0;
           over = dmax(over, fabs(st[i]) * rcp_fast(room));
         }
         const double sl = sqrt_fast(s2);
@@ -644,7 +656,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         sgd = fma(st[i], sg[i * T], sgd);
         if ((act >> i) & 1u) {
           const double nv = sn[i * T] + st[i];
-          if (!(nv > 0.0) || !(nv < __ldg(&w.zn[(int64_t)i * N + n]))) good = false;
+          if (!(nv > 0.0) || !(nv < (ZS ? sz[i * T] : __ldg(&w.zn[(int64_t)i * N + n])))) good = false;
         }
       }
       const double sl = sqrt_fast(s2);
@@ -676,7 +688,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         for (int i = 0; i < NC; ++i) {
           if ((act >> i) & 1u) {
             const double ni = sn[i * T];
-            smax = dmax(smax, fabs(sp[i * T]) * rcp_fast(dmin(ni, __ldg(&w.zn[(int64_t)i * N + n]) - ni)));
+            smax = dmax(smax, fabs(sp[i * T]) * rcp_fast(dmin(ni, (ZS ? sz[i * T] : __ldg(&w.zn[(int64_t)i * N + n])) - ni)));
           }
         }
         if (exact && smax < o.tol_newton_step) {
@@ -693,7 +705,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       double z[NC], x[NC], y[NC], lnK[NC];
       theta = 0.0;
 #pragma unroll
-      for (int i = 0; i < NC; ++i) { z[i] = __ldg(&w.zn[(int64_t)i * N + n]); y[i] = sn[i * T]; theta += y[i]; }
+      for (int i = 0; i < NC; ++i) { z[i] = (ZS ? sz[i * T] : __ldg(&w.zn[(int64_t)i * N + n])); y[i] = sn[i * T]; theta += y[i]; }
       {
         const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
 #pragma unroll

@@ -88,6 +88,8 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_probe(const __grid_con
         w.tpdmin[n] = tpd_min;
         w.Zxy[n] = Zx;
         w.Zxy[io.N + n] = Zy;
+      } else {
+        w.stabit[n] = -1;   // goes through the stability analysis (k_stab_decide walks the batch by this mark)
       }
     }
     count_add(pcase == 1, &w.ctr->n_case1);
