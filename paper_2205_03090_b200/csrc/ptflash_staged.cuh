@@ -137,8 +137,11 @@ __device__ __forceinline__ void flush_add(int v, long long* ctr) {
   for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (total); idx += (int64_t)gridDim.x * blockDim.x)
 
 // ---- K1a ------------------------------------------------------------------------------------------
+#ifndef PTF_INIT_MINB
+#define PTF_INIT_MINB 4
+#endif
 template <int NC>
-__global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+__global__ void __launch_bounds__(128, PTF_INIT_MINB) k_init(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                               const __grid_constant__ Io io, const __grid_constant__ Work w) {
   const int64_t Npad = (io.N + 31) & ~(int64_t)31;  // whole warps stay together for the ballots
   PTF_GRID_STRIDE(idx, Npad) {
@@ -210,8 +213,11 @@ __global__ void __launch_bounds__(128) k_init(const __grid_constant__ Sys<NC> S,
 }
 
 // ---- K4 -------------------------------------------------------------------------------------------
+#ifndef PTF_DECIDE_MINB
+#define PTF_DECIDE_MINB 4
+#endif
 template <int NC>
-__global__ void __launch_bounds__(128) k_stab_decide(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
+__global__ void __launch_bounds__(128, PTF_DECIDE_MINB) k_stab_decide(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                      const __grid_constant__ Io io, const __grid_constant__ Work w) {
   // The kernel is bound by memory traffic, so it walks the batch in mixture order (full, coalesced sectors) and skips the
   // mixtures that did not go through the stability analysis, instead of gathering through q_stab (whose order follows the
