@@ -178,7 +178,15 @@ enum {
                                       iterations is dropped and the mixture re-flashed from Wilson (PTFLASH_ST_WARM_RESTART;
                                       DESIGN.md reading C21): converging hinted splits of the warm-start workload need <= 11, failing
                                       ones wander until the cap */
-  PTFLASH_NUM_OPTS = 22
+  PTFLASH_OPT_EARLY_SPLIT_SS = 22, /* [0] 1 = the successive-substitution stage of the phase split of the mixtures the probe found
+                                      unstable starts right after the probe, next to the stability analysis of the others, instead
+                                      of after it.  Scheduling only, same results.  It pays on workloads with "crawlers" -- splits
+                                      still outside 0 < theta < 1 after split_ss_iters iterations, which continue the substitution
+                                      (reading C13) for hundreds of iterations on a stream of their own: started early,
+                                      that serial chain ends under the rest of the call (paper's 9-component workload: 4.8 -> 4.0 ms
+                                      per 1e6); without crawlers it costs ~5 % (the early stage no longer fills the machine next to
+                                      the latency-bound tail of the stability-found splits) */
+  PTFLASH_NUM_OPTS = 23
 };
 int ptflash_set_option(ptflash_handle_t h, int key, double value);
 int ptflash_get_option(ptflash_handle_t h, int key, double* value);

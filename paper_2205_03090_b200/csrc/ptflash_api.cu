@@ -23,7 +23,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 
-const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 12, 1e-5, 0, 8, 0, 15};
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 12, 1e-5, 0, 8, 0, 15, 0};
 
 }  // namespace
 
@@ -48,8 +48,8 @@ struct ptflash_handle_s {
   bool events_made;
   int n_events;
   // second stream + fork/join events of the staged engine (created on first use)
-  cudaStream_t aux_stream;
-  cudaEvent_t ev_fork, ev_join;
+  cudaStream_t aux_stream, aux2_stream;
+  cudaEvent_t ev_fork, ev_join, ev_c0, ev_c1, ev_cjoin, ev_probe;
   bool aux_made;
   int cta_cache[4];   // resident CTAs per SM of the persistent kernels on this handle's device (0 = not queried yet)
   // ptflash_flash_host pipeline: child handles (same component system, own workspace / streams / counters), one per chunk
@@ -104,9 +104,11 @@ ptf::Opt make_opt(const double* o) {
   r.stability_only = (int)o[PTFLASH_OPT_STABILITY_ONLY];
   r.hint_eta_search = (int)o[PTFLASH_OPT_HINT_ETA_SEARCH];
   r.hint_tr_cap = (int)o[PTFLASH_OPT_HINT_TR_CAP];
+  r.early_split_ss = (int)o[PTFLASH_OPT_EARLY_SPLIT_SS];
   r.prof_events = nullptr;
   r.prof_count = nullptr;
   r.aux_stream = r.ev_fork = r.ev_join = nullptr;
+  r.aux2_stream = r.ev_c0 = r.ev_c1 = r.ev_cjoin = r.ev_probe = nullptr;
   r.cta_cache = nullptr;
   return r;
 }
@@ -214,7 +216,11 @@ int ptflash_destroy(ptflash_handle_t h) {
   if (h->counters_host) cudaFreeHost(h->counters_host);
   if (h->events_made)
     for (int i = 0; i < PTF_MAX_STAGE_EVENTS; ++i) cudaEventDestroy(h->events[i]);
-  if (h->aux_made) { cudaStreamDestroy(h->aux_stream); cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join); }
+  if (h->aux_made) {
+    cudaStreamDestroy(h->aux_stream); cudaStreamDestroy(h->aux2_stream);
+    cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join);
+    cudaEventDestroy(h->ev_c0); cudaEventDestroy(h->ev_c1); cudaEventDestroy(h->ev_cjoin); cudaEventDestroy(h->ev_probe);
+  }
   for (int c = 0; c < h->n_child; ++c) {
     cudaStreamSynchronize(h->child_stream[c]);
     ptflash_destroy(h->child[c]);
@@ -245,7 +251,7 @@ int ptflash_set_option(ptflash_handle_t h, int key, double value) {
     case PTFLASH_OPT_SPLIT_TR_ITERS: case PTFLASH_OPT_SS_CAP: case PTFLASH_OPT_HINT_SS_CAP: case PTFLASH_OPT_HINT_TR_CAP:
       ok = value >= 0.0 && value <= 1.0e9 && value == std::floor(value); break;   // iteration counts
     case PTFLASH_OPT_USE_NEWTON: case PTFLASH_OPT_ENGINE: case PTFLASH_OPT_STAGE_PROFILE: case PTFLASH_OPT_STABILITY_ONLY:
-    case PTFLASH_OPT_HINT_ETA_SEARCH:
+    case PTFLASH_OPT_HINT_ETA_SEARCH: case PTFLASH_OPT_EARLY_SPLIT_SS:
       ok = value == 0.0 || value == 1.0; break;                   // switches
     case PTFLASH_OPT_HOST_CHUNKS:
       ok = value >= 1.0 && value <= (double)PTF_MAX_HOST_CHUNKS && value == std::floor(value); break;
@@ -306,9 +312,19 @@ int ptflash_flash_ex(ptflash_handle_t h, const ptflash_io_t* io, void* stream) {
       if (!cuda_ok(cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking), "cudaStreamCreate")) return PTFLASH_ECUDA;
       if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
       if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+      // the crawler stream has the highest priority: its few CTAs must be placed BEFORE the persistent Newton CTAs of the
+      // split fill every SM, else a crawler's serial chain (hundreds of iterations) starts only when those retire
+      int pr_least = 0, pr_greatest = 0;
+      cudaDeviceGetStreamPriorityRange(&pr_least, &pr_greatest);
+      if (!cuda_ok(cudaStreamCreateWithPriority(&h->aux2_stream, cudaStreamNonBlocking, pr_greatest), "cudaStreamCreate")) return PTFLASH_ECUDA;
+      if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_c0, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+      if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_c1, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+      if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_cjoin, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+      if (!cuda_ok(cudaEventCreateWithFlags(&h->ev_probe, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
       h->aux_made = true;
     }
     o.aux_stream = h->aux_stream; o.ev_fork = h->ev_fork; o.ev_join = h->ev_join;
+    o.aux2_stream = h->aux2_stream; o.ev_c0 = h->ev_c0; o.ev_c1 = h->ev_c1; o.ev_cjoin = h->ev_cjoin; o.ev_probe = h->ev_probe;
   }
   const int launches = fn(h->sys, o, d, h->ws, st);
   if (launches < 0) { cuda_ok(cudaGetLastError(), "kernel launch"); if (g_err.empty()) set_err("kernel launch failed"); return PTFLASH_ECUDA; }

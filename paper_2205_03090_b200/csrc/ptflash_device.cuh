@@ -27,6 +27,7 @@ struct Opt {
   double tol_ss, tol_newton_g, tol_newton_step, tol_newton_step_stab, probe_margin, trivial_tol, band, split_trivial_tol;
   int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap, hint_ss_cap, hint_tr_cap;
   int stability_only;   // 1: stop after the label; no phase split
+  int early_split_ss;   // 1: the SS stage of the probe-found splits starts right after the probe (PTFLASH_OPT_EARLY_SPLIT_SS)
   int hint_eta_search;  // 1: splits entered through a skip-stability hint run the eta search of B.4a (the oracle's path)
   // host only: cudaEvent_t[PTF_MAX_STAGE_EVENTS] recorded between the stage kernels when stage profiling is on (else null)
   void* prof_events;
@@ -34,6 +35,8 @@ struct Opt {
   // host only: second stream of the handle and two events (fork / join) so that the phase split of the mixtures the probe
   // already found unstable runs concurrently with the stability analysis of the others (null: everything on one stream)
   void *aux_stream, *ev_fork, *ev_join;
+  // host only: third stream for the crawlers of the phase split (stage2: split part 2) with its three events
+  void *aux2_stream, *ev_c0, *ev_c1, *ev_cjoin, *ev_probe;
   // host only: per-handle cache of the resident-CTA counts of the persistent kernels (0 = not yet queried); a handle is
   // bound to one device and one component system, so the occupancy query runs once per handle
   int* cta_cache;

@@ -426,10 +426,10 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
   constexpr bool ZS = split_z_in_smem<NC>();
   double* const sz = sS + 2 * NC * T;   // normalised feed z of the lane's mixture (read many times per trip), if it fits (ZS)
   const int64_t N = io.N;
-  const int n_front = w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON];           // slow-SS splits (k2_split_ss): taken first
-  const int total = n_front + w.qcount[part ? Q_SPLIT_NEWTON_BE : Q_SPLIT_NEWTON_E];   // the others sit at the end of the array
-  const int* const q_in = part ? w.q_split_newton_b : w.q_split_newton;
-  int* ticket = &w.qcount[part ? Q_TICKET_SPLIT_B : Q_TICKET_SPLIT];
+  const int n_front = w.qcount[qid_split_newton(part)];            // slow-SS splits (k2_split_ss): taken first
+  const int total = n_front + w.qcount[qid_split_newton_e(part)];   // the others sit at the end of the array
+  const int* const q_in = q_split_newton_of(w, part);
+  int* ticket = &w.qcount[qid_ticket_split(part)];
   bool busy = false, exhausted = false, first = true, reeval = false, searching = false, exact = false, polish = false;
   bool eta_mode = false;   // this lane's item runs the eta search of B.4a instead of the truncated modified-Cholesky step
   int tr_cap = 0;          // trust-region iteration cap of the lane's item (smaller for a skip-stability hint, reading C21)

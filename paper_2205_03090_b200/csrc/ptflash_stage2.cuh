@@ -280,17 +280,23 @@ __device__ __forceinline__ void store_split(const Io& io, const Work& w, int n, 
 template <int NC, bool KIJ0>
 __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
                                                                    const __grid_constant__ Io io, const __grid_constant__ Work w,
-                                                                   const int part) {
+                                                                   const int part, const int crawl_out) {
   __shared__ double s_exp[PTF_EXP_TAB];
   exp_tab_init(s_exp);
-  const int* const q_in = part ? w.q_split_b : w.q_split;
-  const int64_t cnt = w.qcount[part ? Q_SPLIT_B : Q_SPLIT];
+  // part 0 / 1: the splits found by the probe / by the stability analysis, from their K seed.  part 2 / 3: the crawlers they
+  // left behind (crawl_out != 0): still outside 0 < theta < 1 when the switch to the Newton stage was due; they resume here,
+  // on a stream of their own, with their iterate, iteration count, last residual and theta -- a few mixtures per million
+  // that take hundreds of iterations next to a bubble or dew point (reading C13) and would otherwise hold the whole SS
+  // stage (paper's 9-component workload: 1.8 ms instead of 0.5 ms).
+  const bool resume = part >= 2;
+  const int* const q_in = q_split_of(w, part);
+  const int64_t cnt = w.qcount[qid_split(part)];
   const int64_t pad = (cnt + 31) & ~(int64_t)31;
   const int64_t N = io.N;
   int my_max = 0;
   PTF_GRID_STRIDE(idx, pad) {
     const bool in = idx < cnt;
-    bool go_newton = false, slow = false;
+    bool go_newton = false, slow = false, crawl = false;
     int n = 0, k = 0, status = 0;
     if (in) {
       n = q_in[idx];
@@ -302,6 +308,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
 #pragma unroll
       for (int i = 0; i < NC; ++i) lnK[i] = w.lnK[(int64_t)i * N + n];
       double theta = -1.0e300, r_prev = -1.0;
+      if (resume) { k = w.ssk[n]; theta = w.crawl[n]; r_prev = w.crawl[N + n]; }
       const bool hinted = (w.pass == 0) && (w.status[n] & ST_INTERNAL_SKIPPED);
       double Zx = w.Zxy[n], Zy = w.Zxy[N + n];   // roots of the stage that produced lnK (0: none)
       bool converged = false, failed = false, final_rr = false;
@@ -323,6 +330,7 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         if (final_rr) { converged = true; break; }
         if (o.use_newton && k >= o.split_ss_iters && theta > 0.0 && theta < 1.0) { go_newton = true; break; }
         if (k >= o.ss_cap) { status |= ST_SPLIT_CAP; break; }
+        if (crawl_out && o.use_newton && k >= o.split_ss_iters) { crawl = true; break; }   // -> part 2
         // A skip-stability hint (C21) whose successive substitution has not brought theta into (0,1) after hint_ss_cap
         // iterations is dropped here (-> cold re-flash) instead of crawling towards the SS cap: next to the
         // phase boundary such a mixture can take 1e5 iterations (40 ms for the whole call) to fail.
@@ -350,7 +358,16 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
         }
         r_prev = rk;
       }
-      if (go_newton) {
+      if (crawl) {
+        // state of the iteration, resumed by the launch for part 2 (lnK as it stands; the Rachford-Rice is repeated there)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) w.lnK[(int64_t)i * N + n] = lnK[i];
+        w.ssk[n] = k;
+        w.crawl[n] = theta;
+        w.crawl[N + n] = r_prev;
+        w.Zxy[n] = Zx;
+        w.Zxy[N + n] = Zy;
+      } else if (go_newton) {
         // hand-over in the Newton variables: n^V_i = theta y_i (B.4)
         // ... of the MINORITY phase: for theta > 1/2 the roles of the two phases are exchanged (n^L = (1 - theta) x is
         // handed over as "n^V"), so that the majority composition (z - n)/(1 - sum n) is formed without cancellation; G
@@ -370,9 +387,9 @@ __global__ void __launch_bounds__(128, PTF_SPLIT_MINB) k2_split_ss(const __grid_
     count_add((status & ST_SPLIT_CAP) != 0, &w.ctr->n_split_capped);   // rare: no atomic unless a lane hit the cap
     // longest first: splits whose successive substitution was still contracting slowly (near-critical mixtures) are queued at
     // the front of the array, the others from its end (the Newton stage takes the front first)
-    queue_push(go_newton && slow, &w.qcount[part ? Q_SPLIT_NEWTON_B : Q_SPLIT_NEWTON], part ? w.q_split_newton_b : w.q_split_newton, n);
-    queue_push_back(go_newton && !slow, &w.qcount[part ? Q_SPLIT_NEWTON_BE : Q_SPLIT_NEWTON_E],
-                    (part ? w.q_split_newton_b : w.q_split_newton) + N - 1, n);
+    queue_push(go_newton && slow, &w.qcount[qid_split_newton(part)], q_split_newton_of(w, part), n);
+    queue_push_back(go_newton && !slow, &w.qcount[qid_split_newton_e(part)], q_split_newton_of(w, part) + N - 1, n);
+    queue_push(crawl, &w.qcount[qid_split(part + 2)], q_split_of(w, part + 2), n);
   }
   flush_max(my_max, &w.ctr->max_split_ss);
 }
@@ -431,7 +448,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   // queue and take the cold path together with the mixtures that came without a hint -- one pass, no second sweep
   // (in stability-only mode a hint is a verdict, not a split: nothing to run).
   if (io.flags && io.lnK0 && !o.stability_only) {
-    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0);
+    k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0, 0);
     mark();
     k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
     mark();
@@ -439,46 +456,78 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     mark();
     launches += 3;
   }
-  const int passes = 1;
-  for (int pass = 0; pass < passes; ++pass) {
-    w.pass = pass;
-    k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+  w.pass = 0;
+  k2_probe<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w);
+  mark();
+  // the crawlers (parts 2, 3) are few: a small grid for their SS, one Newton CTA per SM
+  const unsigned gC = grid_for(io.N < 65536 ? io.N : 65536);
+  const bool early = fork && !o.stability_only && o.early_split_ss;
+  cudaStream_t aux2 = (cudaStream_t)o.aux2_stream;
+  if (early) {
+    // PTFLASH_OPT_EARLY_SPLIT_SS: the SS stage of the probe-found splits (part 0) starts right after the probe, next to the
+    // stability analysis of the other mixtures, and hands its crawlers to the third stream at once: a crawler is a serial chain
+    // of hundreds of iterations (~3 us each) that nothing shortens, so it has to start early to end under the rest of the call.
+    // (The Newton stage of part 0 still waits for k_stab_decide: its persistent CTAs would hold half of the register file
+    // while the stability kernels need it.)
+    cudaEventRecord((cudaEvent_t)o.ev_probe, st);
+    cudaStreamWaitEvent(aux, (cudaEvent_t)o.ev_probe, 0);
+    k2_split_ss<NC, KIJ0><<<gN, threads, 0, aux>>>(s, o, io, w, 0, 1);
+    cudaEventRecord((cudaEvent_t)o.ev_c0, aux);
+    cudaStreamWaitEvent(aux2, (cudaEvent_t)o.ev_c0, 0);
+    k2_split_ss<NC, KIJ0><<<gC, threads, 0, aux2>>>(s, o, io, w, 2, 0);
+    k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, aux2>>>(s, o, io, w, 2);
+  }
+  k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
+  mark();
+  k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), NEWTON_THREADS, stab_bytes, st>>>(s, o, io, w);
+  mark();
+  k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
+  mark();
+  if (o.stability_only) {
+    k_label_only<NC><<<gN, threads, 0, st>>>(io, w);
     mark();
-    k2_stab_ss<NC, KIJ0><<<g2N, threads, 0, st>>>(s, o, io, w);
+    k_finalize_counters<<<1, 32, 0, st>>>(w);
     mark();
-    k3_stab_newton<NC, KIJ0><<<(unsigned)(sms * stab_cta), NEWTON_THREADS, stab_bytes, st>>>(s, o, io, w);
-    mark();
-    k_stab_decide<NC><<<gN, threads, 0, st>>>(s, o, io, w);
-    mark();
-    if (o.stability_only) {
-      k_label_only<NC><<<gN, threads, 0, st>>>(io, w);
-      mark();
-      k_finalize_counters<<<1, 32, 0, st>>>(w);
-      mark();
-      launches += 6;
-      break;
-    }
+    launches += 6;
+  } else {
     if (fork) {
       cudaEventRecord((cudaEvent_t)o.ev_fork, st);
       cudaStreamWaitEvent(aux, (cudaEvent_t)o.ev_fork, 0);
       // part 1 first: its hard items should start as early as possible, every one on a lane of its own if they fit
       // (one CTA per SM: 19 k lanes on B200, and room for part 0 next to it)
-      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1);
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1, 1);
+      cudaEventRecord((cudaEvent_t)o.ev_c1, st);
       k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 1);
-      k2_split_ss<NC, KIJ0><<<gN, threads, 0, aux>>>(s, o, io, w, 0);
+      if (!early) {
+        k2_split_ss<NC, KIJ0><<<gN, threads, 0, aux>>>(s, o, io, w, 0, 1);
+        cudaEventRecord((cudaEvent_t)o.ev_c0, aux);
+        cudaStreamWaitEvent(aux2, (cudaEvent_t)o.ev_c0, 0);
+        k2_split_ss<NC, KIJ0><<<gC, threads, 0, aux2>>>(s, o, io, w, 2, 0);
+        k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, aux2>>>(s, o, io, w, 2);
+      }
       k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, aux>>>(s, o, io, w, 0);
       cudaEventRecord((cudaEvent_t)o.ev_join, aux);
-      cudaStreamWaitEvent(st, (cudaEvent_t)o.ev_join, 0);   // join
+      // the crawlers of part 1 follow those of part 0 on the third stream
+      cudaStreamWaitEvent(aux2, (cudaEvent_t)o.ev_c1, 0);
+      k2_split_ss<NC, KIJ0><<<gC, threads, 0, aux2>>>(s, o, io, w, 3, 0);
+      k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, aux2>>>(s, o, io, w, 3);
+      cudaEventRecord((cudaEvent_t)o.ev_cjoin, aux2);
+      cudaStreamWaitEvent(st, (cudaEvent_t)o.ev_join, 0);    // join
+      cudaStreamWaitEvent(st, (cudaEvent_t)o.ev_cjoin, 0);
     } else {
-      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0);
-      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1);
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 0, 1);
+      k2_split_ss<NC, KIJ0><<<gN, threads, 0, st>>>(s, o, io, w, 1, 1);
+      k2_split_ss<NC, KIJ0><<<gC, threads, 0, st>>>(s, o, io, w, 2, 0);
+      k2_split_ss<NC, KIJ0><<<gC, threads, 0, st>>>(s, o, io, w, 3, 0);
       mark();
       k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
       k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 1);
+      k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 2);
+      k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 3);
     }
     k_finalize_counters<<<1, 32, 0, st>>>(w);
     mark();
-    launches += 9;
+    launches += 13;
   }
   if (o.prof_count) *o.prof_count = nev;
   return cudaGetLastError() == cudaSuccess ? launches : -1;

@@ -32,13 +32,27 @@ namespace ptf {
 enum : int { Q_PROBE = 0, Q_STAB = 1, Q_STAB_NEWTON = 2, Q_SPLIT = 3, Q_SPLIT_NEWTON = 4, Q_TICKET_STAB = 5, Q_TICKET_SPLIT = 6, Q_RETRY = 7,
               Q_SPLIT_B = 8, Q_SPLIT_NEWTON_B = 9, Q_TICKET_SPLIT_B = 10,
               Q_STAB_NEWTON_E = 11 /* fast engine: trials expected to be short, stored from the END of q_stab_newton */,
-              Q_SPLIT_NEWTON_E = 12, Q_SPLIT_NEWTON_BE = 13 /* the same for the two split queues */, Q_COUNT = 14 };
+              Q_SPLIT_NEWTON_E = 12, Q_SPLIT_NEWTON_BE = 13 /* the same for the two split queues */,
+              // part 2 of the phase split ("crawlers"): splits whose successive substitution is still outside 0 < theta < 1 when the
+              // switch to the Newton stage is due (reading C13: the SS goes on until theta is inside).  They are rare and can
+              // take hundreds of iterations, so they leave the SS kernel and finish on a stream of their own.
+              Q_SPLIT_C = 14, Q_SPLIT_NEWTON_C = 15, Q_TICKET_SPLIT_C = 16, Q_SPLIT_NEWTON_CE = 17,
+              Q_SPLIT_D = 18, Q_SPLIT_NEWTON_D = 19, Q_TICKET_SPLIT_D = 20, Q_SPLIT_NEWTON_DE = 21 /* part 3: the crawlers of part 1 */, Q_COUNT = 22 };
+// queue ids / arrays of split part 0 (probe-found), 1 (stability-found), 2 / 3 (the crawlers of part 0 / 1)
+__host__ __device__ __forceinline__ int qid_split(int part) { return part == 0 ? Q_SPLIT : part == 1 ? Q_SPLIT_B : part == 2 ? Q_SPLIT_C : Q_SPLIT_D; }
+__host__ __device__ __forceinline__ int qid_split_newton(int part) { return part == 0 ? Q_SPLIT_NEWTON : part == 1 ? Q_SPLIT_NEWTON_B : part == 2 ? Q_SPLIT_NEWTON_C : Q_SPLIT_NEWTON_D; }
+__host__ __device__ __forceinline__ int qid_split_newton_e(int part) { return part == 0 ? Q_SPLIT_NEWTON_E : part == 1 ? Q_SPLIT_NEWTON_BE : part == 2 ? Q_SPLIT_NEWTON_CE : Q_SPLIT_NEWTON_DE; }
+__host__ __device__ __forceinline__ int qid_ticket_split(int part) { return part == 0 ? Q_TICKET_SPLIT : part == 1 ? Q_TICKET_SPLIT_B : part == 2 ? Q_TICKET_SPLIT_C : Q_TICKET_SPLIT_D; }
 enum : int { TF_CONVERGED = 1, TF_EXACT = 2, TF_CAPPED = 4, TF_BETA = 8, TF_ITER_SHIFT = 8 + 0 };
 
+struct Work;
 struct Work {
   StageCounters* ctr;
   int* qcount;  // [Q_COUNT]
   int *q_probe, *q_stab, *q_stab_newton, *q_split, *q_split_newton, *q_retry, *q_split_b, *q_split_newton_b;
+  int *q_split_c, *q_split_newton_c, *q_split_d, *q_split_newton_d;   // crawlers (split parts 2, 3)
+  int* ssk;          // [N] SS iterations done when a crawler left k2_split_ss
+  double* crawl;     // [2][N] its theta and last SS residual
   int decide_part;  // queue set k_stab_decide feeds (0 / 1)
   int pass;  // 0: first pass; 1: re-flash of mixtures whose skip-stability hint failed (ST_WARM_RESTART)
   double *lnz, *d, *lnK;   // [NC][N]
@@ -51,6 +65,9 @@ struct Work {
   int *status, *iters, *stabit;  // [N]
   int* actmask;            // [N] bit i set <=> z_i > 0
 };
+
+__device__ __forceinline__ int* q_split_of(const Work& w, int part) { return part == 0 ? w.q_split : part == 1 ? w.q_split_b : part == 2 ? w.q_split_c : w.q_split_d; }
+__device__ __forceinline__ int* q_split_newton_of(const Work& w, int part) { return part == 0 ? w.q_split_newton : part == 1 ? w.q_split_newton_b : part == 2 ? w.q_split_newton_c : w.q_split_newton_d; }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -70,6 +87,12 @@ inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   p = take(n * 4); if (w) w->q_retry = (int*)p;
   p = take(n * 4); if (w) w->q_split_b = (int*)p;
   p = take(n * 4); if (w) w->q_split_newton_b = (int*)p;
+  p = take(n * 4); if (w) w->q_split_c = (int*)p;
+  p = take(n * 4); if (w) w->q_split_newton_c = (int*)p;
+  p = take(n * 4); if (w) w->q_split_d = (int*)p;
+  p = take(n * 4); if (w) w->q_split_newton_d = (int*)p;
+  p = take(n * 4); if (w) w->ssk = (int*)p;
+  p = take(2 * n * 8); if (w) w->crawl = (double*)p;
   if (w) { w->pass = 0; w->decide_part = 0; }
   p = take(c * n * 8); if (w) w->lnz = (double*)p;
   p = take(c * n * 8); if (w) w->d = (double*)p;
@@ -323,7 +346,8 @@ static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
     w.ctr->n_stab += w.qcount[Q_STAB];
     w.ctr->n_stab_newton += w.qcount[Q_STAB_NEWTON] + w.qcount[Q_STAB_NEWTON_E];
     w.ctr->n_split += w.qcount[Q_SPLIT] + w.qcount[Q_SPLIT_B];
-    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_B] + w.qcount[Q_SPLIT_NEWTON_E] + w.qcount[Q_SPLIT_NEWTON_BE];
+    w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_B] + w.qcount[Q_SPLIT_NEWTON_E] + w.qcount[Q_SPLIT_NEWTON_BE] +
+                             w.qcount[Q_SPLIT_NEWTON_C] + w.qcount[Q_SPLIT_NEWTON_CE] + w.qcount[Q_SPLIT_NEWTON_D] + w.qcount[Q_SPLIT_NEWTON_DE];
   }
 }
 

@@ -228,8 +228,8 @@ def _system_16(nc):
 @pytest.mark.parametrize("nc", [3, 13, 16])
 def test_other_component_counts(oracle_mod, nc):
     """nc = 3, 13 and 16 (the largest supported): every component count runs the register-resident stage kernels of
-    engine 1 (10 launches per call: k_init, k2_probe, k2_stab_ss, k3_stab_newton, k_stab_decide, 2 x k2_split_ss,
-    2 x k3_split_newton, k_finalize_counters); for nc >= 13 the Newton CTAs are sized by shared memory."""
+    engine 1 (14 launches per call: k_init, k2_probe, k2_stab_ss, k3_stab_newton, k_stab_decide, 4 x k2_split_ss,
+    4 x k3_split_newton, k_finalize_counters); for nc >= 13 the Newton CTAs are sized by shared memory."""
     system = W.make_system(["C1", "C3", "nC10"]) if nc == 3 else _system_16(nc)
     N = 3000
     n = np.arange(N)
@@ -243,7 +243,7 @@ def test_other_component_counts(oracle_mod, nc):
         rep = check(w, g, o)
         assert rep["two_phase"] > 100
         if engine == 1:
-            assert g["stats"]["kernel_launches"] == 10 and g["stats"]["n_stab_newton"] > 0 and g["stats"]["n_split_newton"] > 0
+            assert g["stats"]["kernel_launches"] == 14 and g["stats"]["n_stab_newton"] > 0 and g["stats"]["n_split_newton"] > 0
 
 
 @pytest.mark.parametrize("cfg,N", [(1, 600), (3, 1500)])
@@ -258,6 +258,45 @@ def test_pure_successive_substitution_mode(oracle_mod, cfg, N):
         check(w, g, o)
         if engine == 1:
             assert g["stats"]["n_stab_newton"] == 0 and g["stats"]["n_split_newton"] == 0
+
+
+def _paper9_with_crawlers(n_ordinary=3000):
+    """The first n_ordinary mixtures of the paper's 9-component workload with the eight "crawlers" of its first 10^6 mixtures
+    (tests/golden/paper9_crawlers.json, inputs only, written by tests/golden/make_paper9_crawlers.py) spread among them."""
+    import json
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper9_crawlers.json")))
+    base = W.paper9(n_ordinary)
+    P = np.array([float.fromhex(v) for v in g["P"]]); T = np.array([float.fromhex(v) for v in g["T"]])
+    z = np.array([[float.fromhex(v) for v in col] for col in g["z"]]).T          # [9, 8]
+    pos = np.linspace(17, n_ordinary - 17, len(P)).astype(int)                    # different warps and CTAs
+    Pn, Tn, zn = base.P.copy(), base.T.copy(), base.z.copy()
+    Pn[pos], Tn[pos], zn[:, pos] = P, T, z
+    return W.Workload("paper9_with_crawlers", base.system, Pn, Tn, np.ascontiguousarray(zn)), pos, g["oracle_split_ss_iters"]
+
+
+def test_split_crawlers_and_early_split_ss(oracle_mod):
+    """Splits still outside 0 < theta < 1 when the switch to the Newton stage is due continue the successive substitution
+    (reading C13) on the crawler stream (split parts 2 / 3, resumed from the saved iterate): same answers and the same
+    iteration counts as the oracle, whichever stream order is used (PTFLASH_OPT_EARLY_SPLIT_SS, with and without the fork)."""
+    w, pos, ss_iters = _paper9_with_crawlers()
+    o = oracle_mod.Oracle.from_system(w.system).flash(w.z, w.P, w.T)
+    assert sorted(int(v) for v in o["stage"][5][pos]) == sorted(ss_iters) and max(ss_iters) > 400
+    ref = None
+    for opts in (dict(), dict(early_split_ss=1), dict(stage_profile=1)):
+        g = _gpu_flash(w, 1, **opts)
+        check(w, g, o)
+        # iteration counts: probe + SS + Newton updates.  The SS part is the oracle's to the iteration (a crawler that ends
+        # inside the SS stage matches exactly); the Newton part takes the truncated step of C25 instead of the eta search
+        in_ss = o["stage"][6][pos] == 0
+        assert in_ss.any() and np.array_equal(g["iters"][pos][in_ss], o["iters"][pos][in_ss])
+        assert np.abs(g["iters"][pos] - o["iters"][pos]).max() <= 8
+        assert g["stats"]["max_split_ss_iters"] == max(ss_iters) and g["stats"]["kernel_launches"] == 14
+        assert g["stats"]["n_split_newton"] == int(o["stage"][8].sum())          # crawlers that reach the Newton stage are counted
+        if ref is None:
+            ref = g
+        else:
+            for k in ("beta", "x", "y", "phase", "iters", "status"):
+                assert np.array_equal(g[k], ref[k]), k
 
 
 def test_host_buffers_stream_and_stats(oracle_mod):
