@@ -246,6 +246,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--cpu-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="library option for this run (binding.OPTIONS, e.g. early_split_ss=1); recorded in config.options")
     ap.add_argument("--ncu-summary", default="", help="raw CSV of the ncu per-kernel pass -> markdown table + profiles/<tag>_flops.json")
     ap.add_argument("--ncu-tag", default="r02")
     args = ap.parse_args()
@@ -276,8 +278,9 @@ def main():
     workload = WORKLOADS[args.config]
     nc = w.system.nc
     f = B.PTFlash.from_system(w.system, engine=args.engine)
-    for kv in filter(None, os.environ.get("PTFLASH_BENCH_OPTS", "").split(",")):   # development only: option overrides for experiments
-        f.set_option(kv.split("=")[0], float(kv.split("=")[1]))
+    user_opts = {kv.split("=", 1)[0]: float(kv.split("=", 1)[1]) for kv in args.opt}
+    for k, v in user_opts.items():
+        f.set_option(k, v)
     z, P, T = (torch.from_numpy(a).to(dev) for a in (w.z, w.P, w.T))
     f64 = dict(dtype=torch.float64, device=dev)
     i32 = dict(dtype=torch.int32, device=dev)
@@ -474,6 +477,8 @@ def main():
                   "working set %.0f MB fits the 126 MB L2 (small-N sweep point; no flush between steps)" % (N * (16.0 * nc + 32 + 60.0 * nc) / 1e6)),
            "stats_last_step": stats}
     cfg.update(extra)
+    if user_opts:
+        cfg["options"] = user_opts
     if args.config == "paper9":
         cfg["paper_table4"] = dict(PAPER_TABLE4, ours={"two_phase_share": stats["n_two_phase"] / N, "probe_proved_share": stats["n_probe_case3"] / N})
     line = {
