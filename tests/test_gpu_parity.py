@@ -161,6 +161,10 @@ def test_parity_config5_warm_start(oracle_mod):
             g_eta = _gpu_flash(w, engine, lnK0=lnK0, flags=flags, hint_eta_search=1)
             check(w, g_eta, o_warm)
             assert np.sum(o_restarted != ((g_eta["status"] & 64) != 0)) <= 3
+            # the early start of the probe-found splits (scheduling only) also after a hinted pre-pass: identical bits
+            g_early = _gpu_flash(w, engine, lnK0=lnK0, flags=flags, early_split_ss=1)
+            for k in ("phase", "beta", "x", "y", "iters", "status"):
+                assert np.array_equal(g_early[k], g_warm[k]), k
         else:
             assert np.sum(o_restarted != restarted) <= 3          # engine 0 follows the oracle's path
         assert np.array_equal(g_warm["phase"][restarted], g_cold["phase"][restarted])
