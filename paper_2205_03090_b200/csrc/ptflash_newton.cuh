@@ -24,6 +24,9 @@ namespace ptf {
 #endif
 constexpr int NEWTON_THREADS = PTF_NEWTON_THREADS;
 
+#ifndef PTF_CHOL_PAIRS
+#define PTF_CHOL_PAIRS 1
+#endif
 #ifndef PTF_NEWTON_CTA_SYNC
 #define PTF_NEWTON_CTA_SYNC 1
 #endif
@@ -115,6 +118,73 @@ __device__ __forceinline__ void chol_row(const int i, double (&row)[NC], const L
 #pragma unroll
     for (int k = 0; k < NC; ++k)
       if (k < i) yv[k] = fma(-row[k], sl, yv[k]);
+  }
+}
+
+// The same for rows i and i + 1 TOGETHER (i + 1 < NC).  Within a row every element depends on the previous one, so one row
+// at a time is a single dependent chain (critical path 16 i cycles against 2 (i^2 / 2) cycles of work on sm_100a: latency
+// bound at two warps per scheduler).  Two rows give the in-order warp two independent chains, every finished L[j][k] read
+// from shared memory serves two products, and L[i+1][i] is formed from row i while it is still in registers.
+template <int NC>
+__device__ __forceinline__ void chol_pivot(double& acc, const double hii, bool& pd, const bool MOD) {
+  if (MOD) {
+    const double fl = 1.0e-10 * fabs(hii);
+    if (!(acc > fl)) { acc = dmax(-acc, fl); pd = false; }
+  } else {
+    pd = pd && (acc > 0.0);
+  }
+}
+template <int NC>
+__device__ __forceinline__ void chol_rows2(const int i, double (&ra)[NC], double (&rb)[NC], const LRows<NC>& L, double (&invd)[NC],
+                                           double (&yv)[NC], double (&s)[NC], const double rhsA, const double rhsB, bool& pd,
+                                           const bool MOD = false) {
+  const double hA = ra[i], hB = rb[i + 1];
+#pragma unroll
+  for (int j = 0; j < NC; ++j) {
+    if (j < i) {
+      double accA = ra[j], accB = rb[j];
+#pragma unroll
+      for (int k = 0; k < NC; ++k)
+        if (k < j) { const double l = L.at(j, k); accA = fma(-ra[k], l, accA); accB = fma(-rb[k], l, accB); }
+      ra[j] = accA * invd[j];
+      rb[j] = accB * invd[j];
+    }
+  }
+  // row i: pivot and forward substitution; element (i + 1, i) of row i + 1 from the registers of row i
+  double dA = ra[i], aA = rhsA, eB = rb[i];
+#pragma unroll
+  for (int k = 0; k < NC; ++k)
+    if (k < i) { dA = fma(-ra[k], ra[k], dA); aA = fma(-ra[k], yv[k], aA); eB = fma(-rb[k], ra[k], eB); }
+  chol_pivot<NC>(dA, hA, pd, MOD);
+  const double invA = rsqrt_fast(dA);
+  invd[i] = invA;
+  yv[i] = aA * invA;
+  rb[i] = eB * invA;
+  if (i > 0) {
+#pragma unroll
+    for (int j = 0; j < NC; ++j)
+      if (j < i) L.at(i, j) = ra[j];
+  }
+  // row i + 1
+  double dB = rb[i + 1], aB = rhsB;
+#pragma unroll
+  for (int k = 0; k < NC; ++k)
+    if (k <= i) { dB = fma(-rb[k], rb[k], dB); aB = fma(-rb[k], yv[k], aB); }
+  chol_pivot<NC>(dB, hB, pd, MOD);
+  const double invB = rsqrt_fast(dB);
+  invd[i + 1] = invB;
+  yv[i + 1] = aB * invB;
+  if (i + 1 < NC - 1) {
+#pragma unroll
+    for (int j = 0; j < NC; ++j)
+      if (j <= i) L.at(i + 1, j) = rb[j];
+  } else {
+    // the last row stays in registers: first step of the back substitution (see chol_row)
+    const double sl = yv[i + 1] * invB;
+    s[i + 1] = sl;
+#pragma unroll
+    for (int k = 0; k < NC; ++k)
+      if (k <= i) yv[k] = fma(-rb[k], sl, yv[k]);
   }
 }
 
@@ -320,14 +390,12 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
       for (int i = 0; i < NC; ++i) sa[i] = sa_of<NC>(S, q, i);
       double invd[NC], yv[NC], st[NC];
       bool good = true;
-#pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        // row i of M: M_ij = G0 + G1 wb_j + G2 S_j - q2 sa_i omk_ij sa_j with G = C F_i, F_i = (1, wb_i, S_i)
+      // row i of M: M_ij = G0 + G1 wb_j + G2 S_j - q2 sa_i omk_ij sa_j with G = C F_i, F_i = (1, wb_i, S_i)
+      auto gen_row = [&](const int i, double (&row)[NC], double& rhs) {
         const double G0 = fma(Sv[i], mc.c20, fma(S.wb[i], c10p, mc.c00));
         const double G1 = fma(Sv[i], c21p, fma(S.wb[i], c11p, c01p));
         const double G2 = fma(Sv[i], mc.c22, fma(S.wb[i], c12p, mc.c02));
         const double qs = mc.q2 * sa[i];
-        double row[NC];
 #pragma unroll
         for (int j = 0; j < NC; ++j) {
           if (j <= i) row[j] = fma(-(KIJ0 ? qs : qs * S.omk[i * NC + j]), sa[j], fma(G2, Sv[j], fma(G1, S.wb[j], G0)));
@@ -336,8 +404,30 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         const double ih = 2.0 * sqW * rcp_fast(sb[i * NEWTON_THREADS]);          // 1 / h_i (beta_i = 2 h_i sqrt(sum W))
         const double iw = ((act >> i) & 1u) ? ih * ih : 1.0e300;
         row[i] = fma(1.0 + 0.5 * ri + es.eta, iw, row[i]);
-        chol_row<NC>(i, row, L, invd, yv, st, -ri * sqW, good);
+        rhs = -ri * sqW;
+      };
+#if PTF_CHOL_PAIRS
+#pragma unroll
+      for (int i = 0; i < NC; i += 2) {
+        if (i + 1 < NC) {
+          double ra[NC], rb[NC], qa_, qb_;
+          gen_row(i, ra, qa_);
+          gen_row(i + 1, rb, qb_);
+          chol_rows2<NC>(i, ra, rb, L, invd, yv, st, qa_, qb_, good);
+        } else {
+          double row[NC], qa_;
+          gen_row(i, row, qa_);
+          chol_row<NC>(i, row, L, invd, yv, st, qa_, good);
+        }
       }
+#else
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        double row[NC], qa_;
+        gen_row(i, row, qa_);
+        chol_row<NC>(i, row, L, invd, yv, st, qa_, good);
+      }
+#endif
       chol_back<NC>(L, invd, yv, st);
       double sn = 0.0, sg = 0.0;
 #pragma unroll
@@ -596,15 +686,13 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       }
       double invd[NC], yv[NC], st[NC];
       bool pd = true;
-#pragma unroll
-      for (int i = 0; i < NC; ++i) {
+      auto gen_row = [&](const int i, double (&row)[NC]) {
         const double ob = one[i] * S.wb[i];
         const double G0 = fma(Sy[i], c30, fma(Sx[i], c20, fma(ob, c10, one[i] * c00)));
         const double G1 = fma(Sy[i], c31, fma(Sx[i], c21, fma(ob, c11, one[i] * c01)));
         const double G2 = fma(Sx[i], c22, fma(ob, c12, one[i] * c02));
         const double G3 = fma(Sy[i], c33, fma(ob, c13, one[i] * c03));
         const double qs = qa * sa[i];
-        double row[NC];
 #pragma unroll
         for (int j = 0; j < NC; ++j) {
           if (j <= i) {
@@ -614,8 +702,29 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
           }
         }
         row[i] = fma(sD[i * T], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
+      };
+#if PTF_CHOL_PAIRS
+#pragma unroll
+      for (int i = 0; i < NC; i += 2) {
+        if (i + 1 < NC) {
+          double ra[NC], rb[NC];
+          gen_row(i, ra);
+          gen_row(i + 1, rb);
+          chol_rows2<NC>(i, ra, rb, L, invd, yv, st, -sg[i * T], -sg[(i + 1) * T], pd, !eta_mode);
+        } else {
+          double row[NC];
+          gen_row(i, row);
+          chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd, !eta_mode);
+        }
+      }
+#else
+#pragma unroll
+      for (int i = 0; i < NC; ++i) {
+        double row[NC];
+        gen_row(i, row);
         chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd, !eta_mode);
       }
+#endif
       chol_back<NC>(L, invd, yv, st);
       // Restricted step without a search (C25): the direction of the (modified) factorisation is cut back to the trust region
       // and to 90 % of the way to the nearest face of the box 0 < n_i < z_i.  One factorisation, i.e. one trip, per
