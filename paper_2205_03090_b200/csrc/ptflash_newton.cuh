@@ -24,8 +24,8 @@ namespace ptf {
 #endif
 constexpr int NEWTON_THREADS = PTF_NEWTON_THREADS;
 
-#ifndef PTF_CHOL_PAIRS
-#define PTF_CHOL_PAIRS 1
+#ifndef PTF_CHOL_R
+#define PTF_CHOL_R 2   // rows eliminated together by the row-wise Cholesky of the Newton kernels
 #endif
 #ifndef PTF_NEWTON_CTA_SYNC
 #define PTF_NEWTON_CTA_SYNC 1
@@ -134,57 +134,69 @@ __device__ __forceinline__ void chol_pivot(double& acc, const double hii, bool& 
     pd = pd && (acc > 0.0);
   }
 }
-template <int NC>
-__device__ __forceinline__ void chol_rows2(const int i, double (&ra)[NC], double (&rb)[NC], const LRows<NC>& L, double (&invd)[NC],
-                                           double (&yv)[NC], double (&s)[NC], const double rhsA, const double rhsB, bool& pd,
-                                           const bool MOD = false) {
-  const double hA = ra[i], hB = rb[i + 1];
+// Rows i .. i + R - 1 together (all < NC); rw[r] is row i + r.  R = 2 is what pays (3, 4, 5, 10 measured: no further gain).
+template <int NC, int R>
+__device__ __forceinline__ void chol_rowsR(const int i, double (&rw)[R][NC], const LRows<NC>& L, double (&invd)[NC],
+                                           double (&yv)[NC], double (&s)[NC], const double (&rhs)[R], bool& pd, const bool MOD = false) {
+  double hd[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) hd[r] = rw[r][i + r];
+  // columns j < i: every finished L[j][k] serves R products
 #pragma unroll
   for (int j = 0; j < NC; ++j) {
     if (j < i) {
-      double accA = ra[j], accB = rb[j];
+      double acc[R];
 #pragma unroll
-      for (int k = 0; k < NC; ++k)
-        if (k < j) { const double l = L.at(j, k); accA = fma(-ra[k], l, accA); accB = fma(-rb[k], l, accB); }
-      ra[j] = accA * invd[j];
-      rb[j] = accB * invd[j];
+      for (int r = 0; r < R; ++r) acc[r] = rw[r][j];
+#pragma unroll
+      for (int k = 0; k < NC; ++k) {
+        if (k < j) {
+          const double l = L.at(j, k);
+#pragma unroll
+          for (int r = 0; r < R; ++r) acc[r] = fma(-rw[r][k], l, acc[r]);
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < R; ++r) rw[r][j] = acc[r] * invd[j];
     }
   }
-  // row i: pivot and forward substitution; element (i + 1, i) of row i + 1 from the registers of row i
-  double dA = ra[i], aA = rhsA, eB = rb[i];
+  // the R x R block on the diagonal, row by row, from the registers of the rows above
 #pragma unroll
-  for (int k = 0; k < NC; ++k)
-    if (k < i) { dA = fma(-ra[k], ra[k], dA); aA = fma(-ra[k], yv[k], aA); eB = fma(-rb[k], ra[k], eB); }
-  chol_pivot<NC>(dA, hA, pd, MOD);
-  const double invA = rsqrt_fast(dA);
-  invd[i] = invA;
-  yv[i] = aA * invA;
-  rb[i] = eB * invA;
-  if (i > 0) {
+  for (int r = 0; r < R; ++r) {
+    const int ir = i + r;
 #pragma unroll
-    for (int j = 0; j < NC; ++j)
-      if (j < i) L.at(i, j) = ra[j];
-  }
-  // row i + 1
-  double dB = rb[i + 1], aB = rhsB;
+    for (int c = 0; c < R; ++c) {
+      if (c < r) {          // element (i + r, i + c)
+        const int jc = i + c;
+        double acc = rw[r][jc];
 #pragma unroll
-  for (int k = 0; k < NC; ++k)
-    if (k <= i) { dB = fma(-rb[k], rb[k], dB); aB = fma(-rb[k], yv[k], aB); }
-  chol_pivot<NC>(dB, hB, pd, MOD);
-  const double invB = rsqrt_fast(dB);
-  invd[i + 1] = invB;
-  yv[i + 1] = aB * invB;
-  if (i + 1 < NC - 1) {
-#pragma unroll
-    for (int j = 0; j < NC; ++j)
-      if (j <= i) L.at(i + 1, j) = rb[j];
-  } else {
-    // the last row stays in registers: first step of the back substitution (see chol_row)
-    const double sl = yv[i + 1] * invB;
-    s[i + 1] = sl;
+        for (int k = 0; k < NC; ++k)
+          if (k < jc) acc = fma(-rw[r][k], rw[c][k], acc);
+        rw[r][jc] = acc * invd[jc];
+      }
+    }
+    double d = rw[r][ir], a = rhs[r];
 #pragma unroll
     for (int k = 0; k < NC; ++k)
-      if (k <= i) yv[k] = fma(-rb[k], sl, yv[k]);
+      if (k < ir) { d = fma(-rw[r][k], rw[r][k], d); a = fma(-rw[r][k], yv[k], a); }
+    chol_pivot<NC>(d, hd[r], pd, MOD);
+    const double inv = rsqrt_fast(d);
+    invd[ir] = inv;
+    yv[ir] = a * inv;
+    if (ir < NC - 1) {
+      if (ir > 0) {
+#pragma unroll
+        for (int j = 0; j < NC; ++j)
+          if (j < ir) L.at(ir, j) = rw[r][j];
+      }
+    } else {
+      // the last row stays in registers: first step of the back substitution (see chol_row)
+      const double sl = yv[ir] * inv;
+      s[ir] = sl;
+#pragma unroll
+      for (int k = 0; k < NC; ++k)
+        if (k < ir) yv[k] = fma(-rw[r][k], sl, yv[k]);
+    }
   }
 }
 
@@ -406,28 +418,23 @@ k3_stab_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o,
         row[i] = fma(1.0 + 0.5 * ri + es.eta, iw, row[i]);
         rhs = -ri * sqW;
       };
-#if PTF_CHOL_PAIRS
+      {
+        constexpr int R = PTF_CHOL_R;
+        constexpr int NB = NC / R * R;   // rows handled in blocks of R, the remainder one by one
 #pragma unroll
-      for (int i = 0; i < NC; i += 2) {
-        if (i + 1 < NC) {
-          double ra[NC], rb[NC], qa_, qb_;
-          gen_row(i, ra, qa_);
-          gen_row(i + 1, rb, qb_);
-          chol_rows2<NC>(i, ra, rb, L, invd, yv, st, qa_, qb_, good);
-        } else {
+        for (int i = 0; i < NB; i += R) {
+          double rw[R][NC], rh[R];
+#pragma unroll
+          for (int r = 0; r < R; ++r) gen_row(i + r, rw[r], rh[r]);
+          chol_rowsR<NC, R>(i, rw, L, invd, yv, st, rh, good);
+        }
+#pragma unroll
+        for (int i = NB; i < NC; ++i) {
           double row[NC], qa_;
           gen_row(i, row, qa_);
           chol_row<NC>(i, row, L, invd, yv, st, qa_, good);
         }
       }
-#else
-#pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        double row[NC], qa_;
-        gen_row(i, row, qa_);
-        chol_row<NC>(i, row, L, invd, yv, st, qa_, good);
-      }
-#endif
       chol_back<NC>(L, invd, yv, st);
       double sn = 0.0, sg = 0.0;
 #pragma unroll
@@ -587,7 +594,7 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
       for (int i = 0; i < NC; ++i) theta += sn[i * T] + sp[i * T];
       const double it = rcp_fast(theta), il = rcp_fast(1.0 - theta);
       double G_new = 0.0, gmax = 0.0;
-#pragma unroll 1
+#pragma unroll
       for (int ph = 0; ph < 2; ++ph) {
         double c[NC], lp[NC], Sv[NC];
 #pragma unroll
@@ -703,28 +710,23 @@ k3_split_newton(const __grid_constant__ Sys<NC> S, const __grid_constant__ Opt o
         }
         row[i] = fma(sD[i * T], deta, row[i]);                 // + D_i / tt + eta D_i (B.4a)
       };
-#if PTF_CHOL_PAIRS
+      {
+        constexpr int R = PTF_CHOL_R;
+        constexpr int NB = NC / R * R;   // rows handled in blocks of R, the remainder one by one
 #pragma unroll
-      for (int i = 0; i < NC; i += 2) {
-        if (i + 1 < NC) {
-          double ra[NC], rb[NC];
-          gen_row(i, ra);
-          gen_row(i + 1, rb);
-          chol_rows2<NC>(i, ra, rb, L, invd, yv, st, -sg[i * T], -sg[(i + 1) * T], pd, !eta_mode);
-        } else {
+        for (int i = 0; i < NB; i += R) {
+          double rw[R][NC], rh[R];
+#pragma unroll
+          for (int r = 0; r < R; ++r) { gen_row(i + r, rw[r]); rh[r] = -sg[(i + r) * T]; }
+          chol_rowsR<NC, R>(i, rw, L, invd, yv, st, rh, pd, !eta_mode);
+        }
+#pragma unroll
+        for (int i = NB; i < NC; ++i) {
           double row[NC];
           gen_row(i, row);
           chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd, !eta_mode);
         }
       }
-#else
-#pragma unroll
-      for (int i = 0; i < NC; ++i) {
-        double row[NC];
-        gen_row(i, row);
-        chol_row<NC>(i, row, L, invd, yv, st, -sg[i * T], pd, !eta_mode);
-      }
-#endif
       chol_back<NC>(L, invd, yv, st);
       // Restricted step without a search (C25): the direction of the (modified) factorisation is cut back to the trust region
       // and to 90 % of the way to the nearest face of the box 0 < n_i < z_i.  One factorisation, i.e. one trip, per
