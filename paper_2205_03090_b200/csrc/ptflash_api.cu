@@ -91,6 +91,8 @@ ptf::Opt make_opt(const double* o) {
   r.tol_newton_step_stab = o[PTFLASH_OPT_TOL_NEWTON_STEP_STAB];
   r.probe_margin = o[PTFLASH_OPT_PROBE_MARGIN];
   r.trivial_tol = o[PTFLASH_OPT_TRIVIAL_TOL];
+  r.triv_lo = std::exp(-r.trivial_tol);
+  r.triv_hi = std::exp(r.trivial_tol);
   r.band = o[PTFLASH_OPT_BAND];
   r.probe_iters = (int)o[PTFLASH_OPT_PROBE_ITERS];
   r.stab_ss_iters = (int)o[PTFLASH_OPT_STAB_SS_ITERS];

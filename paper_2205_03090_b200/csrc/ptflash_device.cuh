@@ -25,6 +25,7 @@ namespace ptf {
 // ------------------------------------------------------------------------------------------------
 struct Opt {
   double tol_ss, tol_newton_g, tol_newton_step, tol_newton_step_stab, probe_margin, trivial_tol, band, split_trivial_tol;
+  double triv_lo, triv_hi;   // exp(-trivial_tol), exp(+trivial_tol): |ln W_i - ln z_i| < trivial_tol  <=>  triv_lo < W_i / z_i < triv_hi
   int probe_iters, stab_ss_iters, stab_tr_iters, split_ss_iters, split_tr_iters, use_newton, ss_cap, hint_ss_cap, hint_tr_cap;
   int stability_only;   // 1: stop after the label; no phase split
   int early_split_ss;   // 1: the SS stage of the probe-found splits starts right after the probe (PTFLASH_OPT_EARLY_SPLIT_SS)

@@ -235,6 +235,45 @@ __global__ void __launch_bounds__(128, PTF_INIT_MINB) k_init(const __grid_consta
   }
 }
 
+// Result of one stability trial for k_stab_decide (cf. stab_finish of ptflash_flash.cuh, which engine 0 uses with ln W in
+// hand).  v = beta (TF_BETA: the trial was finished by the Newton stage) or ln W (it ended inside k2_stab_ss; m.lnz loaded).
+template <int NC>
+__device__ __forceinline__ void decide_trial(const Opt& o, const MixCtx<NC>& m, const double (&v)[NC], int flags, double tm,
+                                             double sumW, StabRes& res) {
+  bool triv = true;
+  if (flags & TF_BETA) {
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+      const double W = 0.25 * v[i] * v[i];
+      if (m.z[i] > 0.0) triv = triv && (W > m.z[i] * o.triv_lo) && (W < m.z[i] * o.triv_hi);
+    }
+  } else {
+    double d = 0.0;
+#pragma unroll
+    for (int i = 0; i < NC; ++i)
+      if (m.z[i] > 0.0) d = fmax(d, fabs(v[i] - m.lnz[i]));
+    triv = d < o.trivial_tol;
+  }
+  res.trivial = triv;
+  res.iters = flags >> TF_ITER_SHIFT;
+  res.capped = (flags & TF_CAPPED) != 0;
+  if (triv) { res.tm = 0.0; res.tpd = 0.0; }
+  else {
+    res.tm = (flags & TF_EXACT) ? (1.0 - sumW) : tm;
+    res.tpd = -log(1.0 - res.tm);  // tm is second-order accurate; tpd = -ln sum W = -ln(1 - tm) at a stationary point
+  }
+}
+// Label from the two finished trials (readings C9, C10): the part of stab_decide that needs no composition
+__device__ __forceinline__ bool stab_label(const Opt& o, const StabRes& sv, const StabRes& sl, double& tpd_min, int& status) {
+  if (sv.capped || sl.capped) status |= ST_STAB_CAP;
+  tpd_min = 0.0;
+  bool any = false;
+  if (!sv.trivial) { tpd_min = sv.tpd; any = true; }
+  if (!sl.trivial) { tpd_min = any ? fmin(tpd_min, sl.tpd) : sl.tpd; any = true; }
+  if (tpd_min != 0.0 && fabs(tpd_min) < o.band) status |= ST_BAND;
+  return tpd_min < 0.0;
+}
+
 // ---- K4 -------------------------------------------------------------------------------------------
 #ifndef PTF_DECIDE_MINB
 #define PTF_DECIDE_MINB 4
@@ -253,35 +292,41 @@ __global__ void __launch_bounds__(128, PTF_DECIDE_MINB) k_stab_decide(const __gr
     const bool in = idx < N && w.stabit[n] == -1;
     bool unstable = false;
     if (in) {
+      // A trial finished by the Newton stage comes back as beta = 2 sqrt(W) (B.1a).  Its trivial-solution test (reading C7)
+      // max_i |ln W_i - ln z_i| < trivial_tol is taken as triv_lo < W_i / z_i < triv_hi with W_i = (beta_i / 2)^2: no
+      // logarithm and no ln z; both are needed only for the K seed of an unstable mixture (2 % of them on config 3) and for
+      // the few trials that ended inside k2_stab_ss, which come back as ln W.
       MixCtx<NC> m;
       double P, T;
       load_feed<NC>(io, n, m.z, P, T);
-#pragma unroll
-      for (int i = 0; i < NC; ++i) m.lnz[i] = w.lnz[(int64_t)i * N + n];
-      StabState<NC> sv, sl;
-      StabRes rv, rl;
-#pragma unroll
-      for (int i = 0; i < NC; ++i) { sv.lnW[i] = w.lnW[(int64_t)i * N + n]; sl.lnW[i] = w.lnW[((int64_t)NC + i) * N + n]; }
       const int fv = w.tflags[n], fl_ = w.tflags[N + n];
       my_tr += ((fv & TF_BETA) ? 1 : 0) + ((fl_ & TF_BETA) ? 65536 : 0);
-      // trials finished by the Newton stage come back as beta = 2 sqrt(W) (B.1a): ln W = 2 ln(beta / 2)
-      if (fv & TF_BETA) {
+      double bv[NC], bl[NC];   // beta or ln W, as stored
 #pragma unroll
-        for (int i = 0; i < NC; ++i) sv.lnW[i] = 2.0 * log_fast_m(0.5 * sv.lnW[i], m.z[i] > 0.0);
-      }
-      if (fl_ & TF_BETA) {
+      for (int i = 0; i < NC; ++i) { bv[i] = w.lnW[(int64_t)i * N + n]; bl[i] = w.lnW[((int64_t)NC + i) * N + n]; }
+      const bool need_lnz = !(fv & TF_BETA) || !(fl_ & TF_BETA);
+      if (need_lnz) {
 #pragma unroll
-        for (int i = 0; i < NC; ++i) sl.lnW[i] = 2.0 * log_fast_m(0.5 * sl.lnW[i], m.z[i] > 0.0);
+        for (int i = 0; i < NC; ++i) m.lnz[i] = w.lnz[(int64_t)i * N + n];
       }
-      sv.tm = w.tm[n]; sv.sumW = w.sumW[n]; sv.iters = fv >> TF_ITER_SHIFT;
-      sv.converged = fv & TF_CONVERGED; sv.stationary_exact = fv & TF_EXACT; sv.capped = fv & TF_CAPPED;
-      sl.tm = w.tm[N + n]; sl.sumW = w.sumW[N + n]; sl.iters = fl_ >> TF_ITER_SHIFT;
-      sl.converged = fl_ & TF_CONVERGED; sl.stationary_exact = fl_ & TF_EXACT; sl.capped = fl_ & TF_CAPPED;
-      stab_finish<NC>(o, m, sv, rv);
-      stab_finish<NC>(o, m, sl, rl);
+      StabRes rv, rl;
+      decide_trial<NC>(o, m, bv, fv, w.tm[n], w.sumW[n], rv);
+      decide_trial<NC>(o, m, bl, fl_, w.tm[N + n], w.sumW[N + n], rl);
       double lnK[NC], tpd_min = 0.0;
       int status = w.status[n];
-      unstable = stab_decide<NC>(o, m, rv, rl, sv.lnW, sl.lnW, lnK, tpd_min, status);
+      unstable = stab_label(o, rv, rl, tpd_min, status);
+      if (unstable) {
+        // K seed (reading C10): K = z / W^L if tm^L < tm^V, else W^V / z
+        const bool liq = rl.tm < rv.tm;
+        const int fs = liq ? fl_ : fv;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          double lw = liq ? bl[i] : bv[i];
+          if (fs & TF_BETA) lw = 2.0 * log_fast_m(0.5 * lw, m.z[i] > 0.0);   // ln W = 2 ln(beta / 2)
+          const double lz = need_lnz ? m.lnz[i] : w.lnz[(int64_t)i * N + n];
+          lnK[i] = liq ? lz - lw : lw - lz;
+        }
+      }
       const int stab_iters = rv.iters + rl.iters;
       if (unstable) {
 #pragma unroll
