@@ -215,6 +215,8 @@ typedef struct ptflash_stats {
   int32_t max_probe_iters, max_stab_ss_iters[2], max_stab_tr_iters[2], max_split_ss_iters, max_split_tr_iters;
   int32_t reserved_;
 } ptflash_stats_t;
+/* Returns PTFLASH_ECUDA (reason in ptflash_last_error) also if the last call left an internal work queue longer than its
+ * array -- impossible by construction (every queue holds at most N, or 2 N, ids), verified on the device after every call. */
 int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out);
 
 /* Batched Rachford-Rice solve with its derivative -- what the paper's initializer training evaluates for every sample

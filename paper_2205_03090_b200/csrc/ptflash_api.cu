@@ -547,6 +547,7 @@ int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out) {
     sum = *h->counters_host;
   }
   const ptf::StageCounters& c = sum;
+  if (c.queue_overflow) { set_err("ptflash_get_stats: an internal work queue overflowed in the last call (results are not trustworthy); please report"); return PTFLASH_ECUDA; }
   out->n_total = h->last_N;
   out->kernel_launches = h->last_launches;
   if ((int)h->opts[PTFLASH_OPT_ENGINE]) {

@@ -33,6 +33,7 @@ struct StageCounters {
   long long n_stab_tr[2], n_stab_capped[2];    // stability trials that went on to the trust-region stage / hit an iteration cap
   long long n_split_capped;                    // phase splits that hit an iteration cap
   long long max_probe, max_stab_ss[2], max_stab_tr[2], max_split_ss, max_split_tr;   // largest iteration counts per stage
+  long long queue_overflow;                    // 1 if a work queue ended longer than its array (cannot happen by construction; checked after every call)
 };
 
 // Launchers return the number of kernels launched (>= 0) or -1 on error.

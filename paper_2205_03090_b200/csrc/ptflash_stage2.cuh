@@ -486,7 +486,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   if (o.stability_only) {
     k_label_only<NC><<<gN, threads, 0, st>>>(io, w);
     mark();
-    k_finalize_counters<<<1, 32, 0, st>>>(w);
+    k_finalize_counters<<<1, 32, 0, st>>>(w, (long long)io.N);
     mark();
     launches += 6;
   } else {
@@ -525,7 +525,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
       k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 2);
       k3_split_newton<NC, KIJ0><<<(unsigned)sms, NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 3);
     }
-    k_finalize_counters<<<1, 32, 0, st>>>(w);
+    k_finalize_counters<<<1, 32, 0, st>>>(w, (long long)io.N);
     mark();
     launches += 13;
   }

@@ -386,8 +386,16 @@ __global__ void __launch_bounds__(128) k_label_only(const __grid_constant__ Io i
 }
 
 // counters that are simply queue lengths (accumulated over the passes)
-static __global__ void k_finalize_counters(const __grid_constant__ Work w) {
+static __global__ void k_finalize_counters(const __grid_constant__ Work w, const long long N) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
+    // every queue holds at most N ids (the stability Newton queue 2 N, filled from both ends): argued in carve_workspace,
+    // verified here after the fact and reported by ptflash_get_stats
+    bool bad = w.qcount[Q_PROBE] > N || w.qcount[Q_STAB] > N || w.qcount[Q_RETRY] > N ||
+               (long long)w.qcount[Q_STAB_NEWTON] + w.qcount[Q_STAB_NEWTON_E] > 2 * N;
+#pragma unroll 1
+    for (int part = 0; part < 4; ++part)
+      bad = bad || w.qcount[qid_split(part)] > N || (long long)w.qcount[qid_split_newton(part)] + w.qcount[qid_split_newton_e(part)] > N;
+    if (bad) w.ctr->queue_overflow = 1;
     w.ctr->n_stab += w.qcount[Q_STAB];
     w.ctr->n_stab_newton += w.qcount[Q_STAB_NEWTON] + w.qcount[Q_STAB_NEWTON_E];
     w.ctr->n_split += w.qcount[Q_SPLIT] + w.qcount[Q_SPLIT_B];
