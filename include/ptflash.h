@@ -132,6 +132,54 @@ int ptflash_host_wait(ptflash_handle_t h);
 /* Synchronises the handle's last stream, frees constants and workspace.  NULL is a no-op. */
 int ptflash_destroy(ptflash_handle_t h);
 
+/* ptflash_flash_static: the same flash as ptflash_flash, for callers that must not allocate.
+ *
+ * Why it exists.  ptflash_flash keeps its work queues and the per-mixture state handed from stage kernel to stage kernel in
+ * a workspace (~0.66 KB per mixture at nc = 10) that the handle cudaMallocs on first use and replaces -- stream
+ * synchronise, cudaFree, cudaMalloc -- whenever a larger batch arrives; ptflash_create itself allocates pinned host memory.
+ * Some users of a flash library cannot accept that inside the call:
+ *   - a reservoir or process simulator that has already handed nearly all device memory to its own arena (or runs inside a
+ *     framework whose caching allocator has): a raw cudaMalloc from a library can then fail although the pool has room;
+ *   - a time-step loop with a latency budget: cudaMalloc and cudaFree serialise against the whole device, so a workspace
+ *     growth stalls every other stream of the process at an unpredictable step;
+ *   - a process held to a fixed memory budget (several jobs sharing one GPU), where a library must state its footprint up
+ *     front and never grow it.
+ * This entry point needs no handle and calls no cudaMalloc, cudaMallocHost, cudaFree, stream or event creation, nor any
+ * library routine that allocates.  Its workspace is an array of PTFLASH_STATIC_SCRATCH_BYTES (32 MiB) that is part of the
+ * library's device code: every GPU on which the library's code gets loaded holds those 32 MiB until the process exits,
+ * whether or not this function is ever called.  That fixed size is the price and the limit: N <= PTFLASH_STATIC_MAX_N.
+ *
+ *   nc, Tc, Pc, omega, kij   the component system, HOST arrays exactly as for ptflash_create (kij may be NULL); it is
+ *                            validated and folded into constants on every call (a few hundred flops on the host)
+ *   N                        0..PTFLASH_STATIC_MAX_N mixtures; N == 0 is a no-op; a larger N is refused with PTFLASH_EINVAL
+ *                            and a message naming the limit (nothing is launched) -- cut the batch, or use ptflash_flash
+ *   z, P, T, out_*           DEVICE pointers on the CURRENT device, meaning and layout as for ptflash_flash; the caller owns
+ *                            them; out_iters may be NULL; inputs and outputs must not alias
+ *   stream                   cudaStream_t of the current device (NULL = legacy default stream)
+ * Results are those of ptflash_flash on a fresh handle with default options: the same stage kernels run in the same order,
+ * all on `stream` (there is no internal second or third stream here, so on big batches it is somewhat slower; at these
+ * sizes a call is launch-latency bound anyway).  Asynchronous: returns once the kernels are queued.  No statistics, no
+ * options, no warm start: use a handle for those.
+ *
+ * Set-up.  The first call on a device looks up the device address of the workspace (cudaGetSymbolAddress) and, the first
+ * time it meets a given (nc, all-zero-kij or not) there, raises the shared-memory limit of the two Newton kernels and asks
+ * the occupancy calculator how many CTAs fit.  Both may make the CUDA runtime load the library's device code.  Make one
+ * call per device and per component system during start-up, before the region that must not allocate and before any stream
+ * capture begins.
+ *
+ * Sharing.  All calls on one device use the same array, whatever the thread or stream, and the array keeps whatever the
+ * previous call left in it.  The function clears the part that must start at zero (stage counters and queue lengths) on
+ * `stream` at the head of every call; nothing else is read before this call has written it.  Two calls that can run on the GPU
+ * at the same time (different streams without an ordering between them, or two host threads) corrupt each other's queues:
+ * order them yourself, e.g. keep to one stream per device.  Calls on different devices are independent.
+ * Returns PTFLASH_OK / PTFLASH_EINVAL (bad system, N out of range, null pointer) / PTFLASH_ECUDA. */
+#define PTFLASH_STATIC_MAX_N 32768
+#define PTFLASH_STATIC_SCRATCH_BYTES 33554432 /* 32 MiB: holds the workspace of 32768 mixtures of 16 components (29.6 MiB) */
+int ptflash_flash_static(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij,
+                         int64_t N, const double* z, const double* P, const double* T,
+                         double* out_beta, double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters,
+                         void* stream);
+
 /* Options (tolerances and caps); defaults in brackets follow DESIGN.md section 3 / PAPER.md:79,90,97,105,558 */
 enum {
   PTFLASH_OPT_TOL_SS = 0,          /* SS residual target, stability and split [1e-10] */

@@ -20,7 +20,9 @@ OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial
            "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol", "stability_only", "host_chunks", "hint_eta_search", "hint_tr_cap", "early_split_ss"]
 EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
            "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_get_stage_ms", "ptflash_fp64_peak",
-           "ptflash_last_error", "ptflash_version", "ptflash_math_probe", "ptflash_rachford_rice", "ptflash_flash_host_async", "ptflash_host_wait"]
+           "ptflash_last_error", "ptflash_version", "ptflash_math_probe", "ptflash_rachford_rice", "ptflash_flash_host_async", "ptflash_host_wait",
+           "ptflash_flash_static"]
+STATIC_MAX_N = 32768   # PTFLASH_STATIC_MAX_N
 
 
 class PTFlashError(RuntimeError):
@@ -91,6 +93,8 @@ def load_library():
     L.ptflash_math_probe.argtypes = [C.c_int, i64, vp, vp, vp]
     L.ptflash_rachford_rice.restype = C.c_int
     L.ptflash_rachford_rice.argtypes = [vp, i64] + [vp] * 7
+    L.ptflash_flash_static.restype = C.c_int
+    L.ptflash_flash_static.argtypes = [C.c_int, dp, dp, dp, dp, i64] + [vp] * 9
     L.ptflash_last_error.restype = C.c_char_p
     L.ptflash_version.restype = C.c_char_p
     _lib = L
@@ -169,6 +173,21 @@ def ptflash_host_wait(h):
 def ptflash_rachford_rice(h, N, lnK, z, out_theta, out_x=None, out_y=None, out_dtheta_dK=None, stream=None):
     _check(load_library().ptflash_rachford_rice(h, int(N), _ptr(lnK), _ptr(z), _ptr(out_theta), _ptr(out_x), _ptr(out_y),
                                                 _ptr(out_dtheta_dK), _stream(stream)), "ptflash_rachford_rice")
+
+
+def ptflash_flash_static(nc, Tc, Pc, omega, kij, N, z, P, T, out_beta, out_x, out_y, out_phase, out_iters=None, stream=None):
+    """The flash for callers that must not allocate (a simulator that has given all device memory to its own pool, a
+    time-step loop that cannot afford cudaMalloc's device-wide stall, a job on a fixed memory budget): no handle, the
+    workspace is a fixed 32 MiB array inside the library, N <= STATIC_MAX_N.  Tc, Pc, omega, kij: host arrays as for
+    ptflash_create; the rest as for ptflash_flash, on the current device.  Calls share the workspace: keep them ordered
+    on one stream per device.  See include/ptflash.h."""
+    L = load_library()
+    _a, pTc = _darr(Tc)
+    _b, pPc = _darr(Pc)
+    _c, pom = _darr(omega)
+    _d, pk = _darr(kij) if kij is not None else (None, None)
+    _check(L.ptflash_flash_static(int(nc), pTc, pPc, pom, pk, int(N), _ptr(z), _ptr(P), _ptr(T), _ptr(out_beta), _ptr(out_x),
+                                  _ptr(out_y), _ptr(out_phase), _ptr(out_iters), _stream(stream)), "ptflash_flash_static")
 
 
 def ptflash_destroy(h):

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 
 #include "../../include/ptflash.h"
@@ -607,3 +608,118 @@ int ptflash_math_probe(int fn, int64_t n, const double* x, double* y, void* stre
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// ptflash_flash_static: the staged flash on a workspace that is part of the library's device image, for callers that
+// must not allocate (see include/ptflash.h for who they are).  Nothing above this line is used differently by it: it
+// borrows the option defaults, make_opt and pick_launcher, and launches the same stage kernels as ptflash_flash_ex.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace {
+
+// The workspace itself.  A __device__ array at file scope: the CUDA runtime places one copy in the memory of every GPU
+// that loads this translation unit's device code and keeps it there until the process ends, so using it costs no
+// allocation call -- and nobody can give it back.  256-byte alignment is what carve_workspace assumes of its base.
+static __device__ __align__(256) unsigned char g_static_ws[PTFLASH_STATIC_SCRATCH_BYTES];
+
+// CAUTION for whoever edits this file: in HOST code the identifier g_static_ws is only the runtime's host-side stand-in
+// for the array.  Its host address is not a device address; handing &g_static_ws[0] to a kernel or to cudaMemsetAsync
+// makes the kernel fault (or, on a system where the GPU can reach host memory, scribble over the wrong bytes without
+// any error).  The device address has to be asked for, per device, with cudaGetSymbolAddress while that device is
+// current; static_workspace() below is the only place that does so and the only way the rest of the file gets the pointer.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+  void* ws;            // device address of g_static_ws on this device; nullptr = not asked for yet
+  int cta[17][2][4];   // resident-CTA counts of the persistent kernels per (nc, kij all zero): launch_stage2's cache (0 = not queried)
+};
+StaticDevice g_static_dev[kStaticMaxDevices];   // zero-initialised
+std::mutex g_static_mu;                         // guards g_static_dev; held for the (host-side) duration of a call
+
+// Device address of the static workspace on the CURRENT device `dev`, looked up on the first call there.  Caller holds g_static_mu.
+void* static_workspace(int dev) {
+  StaticDevice& sd = g_static_dev[dev];
+  if (sd.ws == nullptr) {
+    void* p = nullptr;
+    if (!cuda_ok(cudaGetSymbolAddress(&p, g_static_ws), "ptflash_flash_static: cudaGetSymbolAddress(workspace)")) return nullptr;
+    if (p == nullptr || ((uintptr_t)p & 255u) != 0) { set_err("ptflash_flash_static: the runtime returned an unusable workspace address"); return nullptr; }
+    sd.ws = p;
+  }
+  return sd.ws;
+}
+
+// The component system of a handle-free call: the checks and the constant folding (A.2d-g PAPER.md:420-427, eq. 6
+// PAPER.md:74) that ptflash_create applies once per handle, applied per call.
+bool static_system(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij, ptf::SysHost* out) {
+  if (nc < 2 || nc > PTFLASH_MAX_NC) { set_err("ptflash_flash_static: nc must be in [2, 16]"); return false; }
+  if (!Tc || !Pc || !omega) { set_err("ptflash_flash_static: null Tc/Pc/omega"); return false; }
+  ptf::SysHost& s = *out;
+  std::memset(&s, 0, sizeof(s));
+  s.nc = nc;
+  s.kij_zero = 1;
+  for (int i = 0; i < nc; ++i) {
+    if (!std::isfinite(Tc[i]) || !std::isfinite(Pc[i]) || !std::isfinite(omega[i]) || Tc[i] <= 0.0 || Pc[i] <= 0.0) {
+      set_err("ptflash_flash_static: Tc and Pc must be finite and positive, omega finite");
+      return false;
+    }
+    const double m = 0.480 + 1.574 * omega[i] - 0.176 * omega[i] * omega[i];
+    const double k = std::sqrt(0.42748 / Pc[i]);
+    s.u[i] = k * Tc[i] * (1.0 + m);
+    s.v[i] = k * std::sqrt(Tc[i]) * m;
+    s.wb[i] = 0.08664 * Tc[i] / Pc[i];
+    s.lnpc[i] = std::log(Pc[i]);
+    s.wil[i] = 5.373 * (1.0 + omega[i]);
+    s.tc[i] = Tc[i];
+    for (int j = 0; j < nc; ++j) {
+      const double kk = kij ? kij[i * nc + j] : 0.0;
+      if (!std::isfinite(kk) || (kij && kk != kij[j * nc + i]) || (i == j && kk != 0.0)) {
+        set_err("ptflash_flash_static: kij must be finite and symmetric with a zero diagonal");
+        return false;
+      }
+      s.omk[i * nc + j] = 1.0 - kk;
+      if (kk != 0.0) s.kij_zero = 0;
+    }
+  }
+  return true;
+}
+
+}  // namespace
+
+extern "C" int ptflash_flash_static(int nc, const double* Tc, const double* Pc, const double* omega, const double* kij,
+                                    int64_t N, const double* z, const double* P, const double* T, double* out_beta,
+                                    double* out_x, double* out_y, int32_t* out_phase, int32_t* out_iters, void* stream) {
+  g_err.clear();
+  ptf::SysHost sys;
+  if (!static_system(nc, Tc, Pc, omega, kij, &sys)) return PTFLASH_EINVAL;
+  if (N < 0) { set_err("ptflash_flash_static: N < 0"); return PTFLASH_EINVAL; }
+  if (N == 0) return PTFLASH_OK;
+  const size_t need = N <= PTFLASH_STATIC_MAX_N ? ptf::staged_workspace_bytes(nc, N) : 0;
+  if (N > PTFLASH_STATIC_MAX_N || need > (size_t)PTFLASH_STATIC_SCRATCH_BYTES) {
+    // the second condition cannot hold for nc <= 16 and N <= PTFLASH_STATIC_MAX_N; it keeps the two constants honest
+    set_err("ptflash_flash_static: N = " + std::to_string((long long)N) + " exceeds PTFLASH_STATIC_MAX_N = " +
+            std::to_string(PTFLASH_STATIC_MAX_N) + " (the static workspace is " + std::to_string(PTFLASH_STATIC_SCRATCH_BYTES >> 20) +
+            " MiB and cannot grow): cut the batch into pieces of at most that many mixtures, or use ptflash_flash");
+    return PTFLASH_EINVAL;
+  }
+  if (!z || !P || !T || !out_beta || !out_x || !out_y || !out_phase) { set_err("ptflash_flash_static: null required pointer"); return PTFLASH_EINVAL; }
+  ptf::launch_fn fn = pick_launcher(nc, 1);
+  if (!fn) { set_err("ptflash_flash_static: no kernel for this nc"); return PTFLASH_EINVAL; }
+  int dev = 0;
+  if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return PTFLASH_ECUDA;
+  if (dev < 0 || dev >= kStaticMaxDevices) { set_err("ptflash_flash_static: device ordinal beyond the 64 this entry point keeps state for"); return PTFLASH_EINVAL; }
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  void* ws = static_workspace(dev);
+  if (!ws) return PTFLASH_ECUDA;
+  ptf::Io d;
+  std::memset(&d, 0, sizeof(d));
+  d.N = N;
+  d.z = z; d.P = P; d.T = T;
+  d.beta = out_beta; d.x = out_x; d.y = out_y;
+  d.phase = out_phase; d.iters = out_iters;
+  // default options; no profiling events and no auxiliary streams, so launch_stage2 orders every stage kernel on `stream`.
+  // Its first action is a cudaMemsetAsync of the stage counters and queue lengths at the head of `ws`: the only part of the
+  // workspace that has to start at zero, and the array still holds the previous call's values.
+  ptf::Opt o = make_opt(kDefaultOpts);
+  o.cta_cache = g_static_dev[dev].cta[nc][sys.kij_zero ? 1 : 0];
+  const int launches = fn(sys, o, d, ws, (cudaStream_t)stream);
+  if (launches < 0) { cuda_ok(cudaGetLastError(), "ptflash_flash_static: kernel launch"); if (g_err.empty()) set_err("ptflash_flash_static: kernel launch failed"); return PTFLASH_ECUDA; }
+  return PTFLASH_OK;
+}
