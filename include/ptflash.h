@@ -234,7 +234,11 @@ enum {
                                       that serial chain ends under the rest of the call (paper's 9-component workload: 4.8 -> 4.0 ms
                                       per 1e6); without crawlers it costs ~5 % (the early stage no longer fills the machine next to
                                       the latency-bound tail of the stability-found splits) */
-  PTFLASH_NUM_OPTS = 23
+  PTFLASH_OPT_HOST_ROW_COPIES = 23, /* [0] 1 = ptflash_flash_host moves the strided slices of z, x, y with one plain copy per component row
+                                      instead of one 2D copy per array.  The call does that by itself when N * 8 bytes exceeds the
+                                      pitch a 2D copy accepts (2^31 - 1 bytes, i.e. N >= 2^28 mixtures); the option exists to
+                                      exercise that path at ordinary sizes.  Same results */
+  PTFLASH_NUM_OPTS = 24
 };
 int ptflash_set_option(ptflash_handle_t h, int key, double value);
 int ptflash_get_option(ptflash_handle_t h, int key, double* value);
@@ -264,7 +268,11 @@ typedef struct ptflash_stats {
   int32_t reserved_;
 } ptflash_stats_t;
 /* Returns PTFLASH_ECUDA (reason in ptflash_last_error) also if the last call left an internal work queue longer than its
- * array -- impossible by construction (every queue holds at most N, or 2 N, ids), verified on the device after every call. */
+ * array.  By construction that cannot happen (every queue holds at most N, or 2 N, ids; the argument is written out above
+ * carve_workspace in csrc/ptflash_staged.cuh), and the appends are not clamped; the last kernel of every call compares the
+ * final queue lengths with their capacities, so a violation is seen AFTER the fact -- memory behind the queue has then been
+ * overwritten and the call's results are not to be trusted -- and only here, since the flash calls return before the
+ * kernels have run. */
 int ptflash_get_stats(ptflash_handle_t h, ptflash_stats_t* out);
 
 /* Batched Rachford-Rice solve with its derivative -- what the paper's initializer training evaluates for every sample

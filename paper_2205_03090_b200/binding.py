@@ -17,7 +17,7 @@ PTFLASH_OK, PTFLASH_EINVAL, PTFLASH_ECUDA = 0, -1, -2
 ST_STAB_CAP, ST_SPLIT_CAP, ST_BAND, ST_SPLIT_FAILED, ST_LNK0_REJECTED = 1, 2, 4, 8, 32
 FLAG_SKIP_STABILITY, FLAG_USE_LNK0 = 1, 2
 OPTIONS = ["tol_ss", "tol_newton_g", "tol_newton_step", "probe_margin", "trivial_tol", "band", "probe_iters",
-           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol", "stability_only", "host_chunks", "hint_eta_search", "hint_tr_cap", "early_split_ss"]
+           "stab_ss_iters", "stab_tr_iters", "split_ss_iters", "split_tr_iters", "use_newton", "ss_cap", "engine", "stage_profile", "tol_newton_step_stab", "hint_ss_cap", "split_trivial_tol", "stability_only", "host_chunks", "hint_eta_search", "hint_tr_cap", "early_split_ss", "host_row_copies"]
 EXPORTS = ["ptflash_create", "ptflash_flash", "ptflash_flash_ex", "ptflash_flash_host", "ptflash_destroy",
            "ptflash_set_option", "ptflash_get_option", "ptflash_get_stats", "ptflash_get_stage_ms", "ptflash_fp64_peak",
            "ptflash_last_error", "ptflash_version", "ptflash_math_probe", "ptflash_rachford_rice", "ptflash_flash_host_async", "ptflash_host_wait",

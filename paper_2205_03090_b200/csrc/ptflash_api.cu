@@ -24,7 +24,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
   return false;
 }
 
-const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 12, 1e-5, 0, 8, 0, 15, 0};
+const double kDefaultOpts[PTFLASH_NUM_OPTS] = {1e-10, 1e-12, 1e-7, 1e-8, 1e-6, 1e-9, 3, 9, 60, 9, 60, 1, 100000, 1, 0, 1e-6, 12, 1e-5, 0, 8, 0, 15, 0, 0};
 
 }  // namespace
 
@@ -32,8 +32,10 @@ struct ptflash_handle_s {
   int device;
   ptf::SysHost sys;
   double opts[PTFLASH_NUM_OPTS];
-  cudaStream_t last_stream;
+  cudaStream_t last_stream;   // stream of the last FLASH call: what ptflash_get_stats / ptflash_get_stage_ms wait for
   bool used;
+  cudaStream_t rr_stream;     // stream of the last ptflash_rachford_rice call (it has no counters: only ptflash_destroy waits for it)
+  bool rr_used;
   // workspace of the staged engine (device) and its size
   void* ws;
   size_t ws_bytes;
@@ -150,6 +152,31 @@ bool ensure(void** buf, size_t* have, size_t need, cudaStream_t st, const char* 
   return true;
 }
 
+// Strided copy of `rows` rows of `width` bytes: the component rows of one chunk's slice of an SoA array ([nc][N] on the host,
+// [nc][Nc] on the device).  One cudaMemcpy2DAsync -- unless a pitch is beyond what the 2D copy accepts (cudaDevAttrMaxPitch,
+// 2^31 - 1 bytes, i.e. host arrays of N >= 2^28 mixtures: "invalid pitch") or the caller asks for it
+// (PTFLASH_OPT_HOST_ROW_COPIES): then one cudaMemcpyAsync per row, at most 16 of them.
+bool copy_rows(void* dst, size_t dpitch, const void* src, size_t spitch, size_t width, int rows, cudaMemcpyKind kind,
+               cudaStream_t st, size_t max_pitch, bool by_rows, const char* what) {
+  if (!by_rows && dpitch <= max_pitch && spitch <= max_pitch)
+    return cuda_ok(cudaMemcpy2DAsync(dst, dpitch, src, spitch, width, (size_t)rows, kind, st), what);
+  for (int r = 0; r < rows; ++r)
+    if (!cuda_ok(cudaMemcpyAsync((char*)dst + (size_t)r * dpitch, (const char*)src + (size_t)r * spitch, width, kind, st), what)) return false;
+  return true;
+}
+
+// A child handle of the host-buffer calls: same component system, its own workspace and counters.  nullptr on failure.
+ptflash_handle_s* make_child(const ptflash_handle_s* h) {
+  ptflash_handle_s* k = new ptflash_handle_s();
+  std::memset(k, 0, sizeof(*k));
+  k->device = h->device;
+  k->sys = h->sys;
+  k->a_last = -1;
+  if (!cuda_ok(cudaMallocHost((void**)&k->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete k; return nullptr; }
+  std::memset(k->counters_host, 0, sizeof(ptf::StageCounters));
+  return k;
+}
+
 }  // namespace
 
 extern "C" {
@@ -214,6 +241,7 @@ int ptflash_destroy(ptflash_handle_t h) {
   int rc = PTFLASH_OK;
   DeviceGuard guard(h->device);
   if (h->used && !cuda_ok(cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize")) rc = PTFLASH_ECUDA;
+  if (h->rr_used && !cuda_ok(cudaStreamSynchronize(h->rr_stream), "cudaStreamSynchronize")) rc = PTFLASH_ECUDA;
   if (h->ws) cudaFree(h->ws);
   if (h->stage) cudaFree(h->stage);
   if (h->counters_host) cudaFreeHost(h->counters_host);
@@ -254,7 +282,7 @@ int ptflash_set_option(ptflash_handle_t h, int key, double value) {
     case PTFLASH_OPT_SPLIT_TR_ITERS: case PTFLASH_OPT_SS_CAP: case PTFLASH_OPT_HINT_SS_CAP: case PTFLASH_OPT_HINT_TR_CAP:
       ok = value >= 0.0 && value <= 1.0e9 && value == std::floor(value); break;   // iteration counts
     case PTFLASH_OPT_USE_NEWTON: case PTFLASH_OPT_ENGINE: case PTFLASH_OPT_STAGE_PROFILE: case PTFLASH_OPT_STABILITY_ONLY:
-    case PTFLASH_OPT_HINT_ETA_SEARCH: case PTFLASH_OPT_EARLY_SPLIT_SS:
+    case PTFLASH_OPT_HINT_ETA_SEARCH: case PTFLASH_OPT_EARLY_SPLIT_SS: case PTFLASH_OPT_HOST_ROW_COPIES:
       ok = value == 0.0 || value == 1.0; break;                   // switches
     case PTFLASH_OPT_HOST_CHUNKS:
       ok = value >= 1.0 && value <= (double)PTF_MAX_HOST_CHUNKS && value == std::floor(value); break;
@@ -355,7 +383,7 @@ int ptflash_flash(ptflash_handle_t h, int64_t N, const double* z, const double* 
 }
 
 // Host-buffer variant.  The batch is cut into chunks of consecutive mixtures; chunk c is handled by child handle c on a
-// stream of its own: H2D copies of its slices of z, P, T (the SoA slices are strided: cudaMemcpy2DAsync) -> the flash kernels
+// stream of its own: H2D copies of its slices of z, P, T (the SoA slices are strided: copy_rows) -> the flash kernels
 // -> D2H copies of its results.  Streams of different chunks overlap, so the PCIe transfers of one chunk hide under the
 // kernels of the others (PCIe is full duplex: H2D and D2H use different copy engines).  The device buffers are chunk-local
 // SoA ([nc][Nc]), so each chunk is an ordinary ptflash_flash call.
@@ -374,16 +402,17 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
   int chunks = (int)h->opts[PTFLASH_OPT_HOST_CHUNKS];
   while (chunks > 1 && N / chunks < 32768) --chunks;
   while (h->n_child < chunks) {
+    // a slot counts (n_child) only once its handle, stream and events all exist; a failure on the way releases what was made
     const int c = h->n_child;
-    ptflash_handle_s* k = new ptflash_handle_s();
-    std::memset(k, 0, sizeof(*k));
-    k->device = h->device;
-    k->sys = h->sys;
-    if (!cuda_ok(cudaMallocHost((void**)&k->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete k; return PTFLASH_ECUDA; }
-    std::memset(k->counters_host, 0, sizeof(ptf::StageCounters));
-    if (!cuda_ok(cudaStreamCreateWithFlags(&h->child_stream[c], cudaStreamNonBlocking), "cudaStreamCreate")) return PTFLASH_ECUDA;
-    if (!cuda_ok(cudaEventCreateWithFlags(&h->child_done[c], cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
-    if (c == 0 && !cuda_ok(cudaEventCreateWithFlags(&h->host_begin, cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+    ptflash_handle_s* k = make_child(h);
+    if (!k) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaStreamCreateWithFlags(&h->child_stream[c], cudaStreamNonBlocking), "cudaStreamCreate")) { ptflash_destroy(k); return PTFLASH_ECUDA; }
+    if (!cuda_ok(cudaEventCreateWithFlags(&h->child_done[c], cudaEventDisableTiming), "cudaEventCreate")) {
+      cudaStreamDestroy(h->child_stream[c]); ptflash_destroy(k); return PTFLASH_ECUDA;
+    }
+    if (c == 0 && !cuda_ok(cudaEventCreateWithFlags(&h->host_begin, cudaEventDisableTiming), "cudaEventCreate")) {
+      cudaEventDestroy(h->child_done[c]); cudaStreamDestroy(h->child_stream[c]); ptflash_destroy(k); return PTFLASH_ECUDA;
+    }
     h->child[c] = k;
     h->n_child = c + 1;
   }
@@ -391,6 +420,10 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
   if (!cuda_ok(cudaEventRecord(h->host_begin, st), "cudaEventRecord")) return PTFLASH_ECUDA;
   const int64_t per = ((N + chunks - 1) / chunks + 31) & ~(int64_t)31;
   const size_t hp = (size_t)N * sizeof(double);   // pitch of the host SoA arrays
+  int max_pitch_attr = 0x7fffffff;
+  cudaDeviceGetAttribute(&max_pitch_attr, cudaDevAttrMaxPitch, h->device);
+  const size_t max_pitch = (size_t)max_pitch_attr;
+  const bool by_rows = (int)h->opts[PTFLASH_OPT_HOST_ROW_COPIES] != 0;
   int launches = 0;
   for (int c = 0; c < chunks; ++c) {
     const int64_t n0 = (int64_t)c * per;
@@ -411,15 +444,15 @@ int ptflash_flash_host(ptflash_handle_t h, int64_t N, const double* z, const dou
     int32_t* dphase = (int32_t*)(dy + nd * nc);
     int32_t* diters = dphase + nd;
     if (!cuda_ok(cudaStreamWaitEvent(cs, h->host_begin, 0), "cudaStreamWaitEvent")) return PTFLASH_ECUDA;
-    if (!cuda_ok(cudaMemcpy2DAsync(dz, dp, z + n0, hp, dp, (size_t)nc, cudaMemcpyHostToDevice, cs), "H2D z")) return PTFLASH_ECUDA;
+    if (!copy_rows(dz, dp, z + n0, hp, dp, nc, cudaMemcpyHostToDevice, cs, max_pitch, by_rows, "H2D z")) return PTFLASH_ECUDA;
     if (!cuda_ok(cudaMemcpyAsync(dP, P + n0, dp, cudaMemcpyHostToDevice, cs), "H2D P")) return PTFLASH_ECUDA;
     if (!cuda_ok(cudaMemcpyAsync(dT, T + n0, dp, cudaMemcpyHostToDevice, cs), "H2D T")) return PTFLASH_ECUDA;
     const int rc = ptflash_flash(k, nn, dz, dP, dT, dbeta, dx, dy, dphase, out_iters ? diters : nullptr, cs);
     if (rc != PTFLASH_OK) return rc;
     launches += k->last_launches;
     if (!cuda_ok(cudaMemcpyAsync(out_beta + n0, dbeta, dp, cudaMemcpyDeviceToHost, cs), "D2H beta")) return PTFLASH_ECUDA;
-    if (!cuda_ok(cudaMemcpy2DAsync(out_x + n0, hp, dx, dp, dp, (size_t)nc, cudaMemcpyDeviceToHost, cs), "D2H x")) return PTFLASH_ECUDA;
-    if (!cuda_ok(cudaMemcpy2DAsync(out_y + n0, hp, dy, dp, dp, (size_t)nc, cudaMemcpyDeviceToHost, cs), "D2H y")) return PTFLASH_ECUDA;
+    if (!copy_rows(out_x + n0, hp, dx, dp, dp, nc, cudaMemcpyDeviceToHost, cs, max_pitch, by_rows, "D2H x")) return PTFLASH_ECUDA;
+    if (!copy_rows(out_y + n0, hp, dy, dp, dp, nc, cudaMemcpyDeviceToHost, cs, max_pitch, by_rows, "D2H y")) return PTFLASH_ECUDA;
     if (!cuda_ok(cudaMemcpyAsync(out_phase + n0, dphase, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, cs), "D2H phase")) return PTFLASH_ECUDA;
     if (out_iters && !cuda_ok(cudaMemcpyAsync(out_iters + n0, diters, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, cs), "D2H iters")) return PTFLASH_ECUDA;
     if (!cuda_ok(cudaEventRecord(h->child_done[c], cs), "cudaEventRecord")) return PTFLASH_ECUDA;
@@ -451,15 +484,12 @@ int ptflash_flash_host_async(ptflash_handle_t h, int64_t N, const double* z, con
   const int slot = (int)(h->a_submitted % PTF_HOST_DEPTH);
   while (h->n_aslot <= slot) {
     const int c = h->n_aslot;
-    ptflash_handle_s* k = new ptflash_handle_s();
-    std::memset(k, 0, sizeof(*k));
-    k->device = h->device;
-    k->sys = h->sys;
-    k->a_last = -1;
-    if (!cuda_ok(cudaMallocHost((void**)&k->counters_host, sizeof(ptf::StageCounters)), "cudaMallocHost")) { delete k; return PTFLASH_ECUDA; }
-    std::memset(k->counters_host, 0, sizeof(ptf::StageCounters));
-    if (!cuda_ok(cudaStreamCreateWithFlags(&h->astream[c], cudaStreamNonBlocking), "cudaStreamCreate")) return PTFLASH_ECUDA;
-    if (!cuda_ok(cudaEventCreateWithFlags(&h->adone[c], cudaEventDisableTiming), "cudaEventCreate")) return PTFLASH_ECUDA;
+    ptflash_handle_s* k = make_child(h);
+    if (!k) return PTFLASH_ECUDA;
+    if (!cuda_ok(cudaStreamCreateWithFlags(&h->astream[c], cudaStreamNonBlocking), "cudaStreamCreate")) { ptflash_destroy(k); return PTFLASH_ECUDA; }
+    if (!cuda_ok(cudaEventCreateWithFlags(&h->adone[c], cudaEventDisableTiming), "cudaEventCreate")) {
+      cudaStreamDestroy(h->astream[c]); ptflash_destroy(k); return PTFLASH_ECUDA;
+    }
     h->aslot[c] = k;
     h->n_aslot = c + 1;
   }
@@ -501,6 +531,7 @@ int ptflash_flash_host_async(ptflash_handle_t h, int64_t N, const double* z, con
 }
 
 int ptflash_host_wait(ptflash_handle_t h) {
+  g_err.clear();
   if (!h) { set_err("ptflash_host_wait: null handle"); return PTFLASH_EINVAL; }
   DeviceGuard guard(h->device);
   for (int c = 0; c < h->n_aslot; ++c)
@@ -521,8 +552,9 @@ int ptflash_rachford_rice(ptflash_handle_t h, int64_t N, const double* lnK, cons
   ptf::RrIo io;
   io.N = N; io.lnK = lnK; io.z = z; io.theta = out_theta; io.x = out_x; io.y = out_y; io.dth = out_dtheta_dK;
   if (fn(io, (cudaStream_t)stream) < 0) { cuda_ok(cudaGetLastError(), "rachford-rice kernel"); if (g_err.empty()) set_err("kernel launch failed"); return PTFLASH_ECUDA; }
-  h->last_stream = (cudaStream_t)stream;
-  h->used = true;
+  // not last_stream: the statistics and stage times of the last flash stay tied to the stream that flash ran on
+  h->rr_stream = (cudaStream_t)stream;
+  h->rr_used = true;
   return PTFLASH_OK;
 }
 

@@ -437,7 +437,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
   // Fork after the stability stages.  The phase split has two parts: (0) the mixtures the probe (or the caller's flag)
   // declared unstable -- most of them, well conditioned -- and (1) the few the stability analysis found unstable: close
   // to the phase boundary, where single mixtures take ~100 trust-region trips, so that part 1 alone ends in a long tail
-  // with a handful of busy lanes (0.7 ms of a 4.2 ms call on config 3).  Part 1 runs on the caller's stream, part 0 on the
+  // with a handful of busy lanes (0.24 ms of a 3.2 ms call on config 3, profiles/r02g_kernels.md).  Part 1 runs on the caller's stream, part 0 on the
   // handle's second stream at the same time, so the tail of one is covered by the bulk of the other.  (Running part 0
   // earlier, concurrently with the stability kernels, gains little: those fill the register file on their own.)
   // With stage profiling on, everything stays on the caller's stream so that the event-to-event times are per stage.
@@ -452,7 +452,7 @@ int launch_stage2_impl(const Sys<NC>& s, const Opt& o, const Io& io, const Work&
     mark();
     k3_split_newton<NC, KIJ0><<<(unsigned)(sms * split_cta), NEWTON_THREADS, split_bytes, st>>>(s, o, io, w, 0);
     mark();
-    k_requeue_failed_hints<<<1, 1024, 0, st>>>(w);
+    k_requeue_failed_hints<<<1, 1024, 0, st>>>(w, (long long)io.N);
     mark();
     launches += 3;
   }

@@ -72,6 +72,21 @@ __device__ __forceinline__ int* q_split_newton_of(const Work& w, int part) { ret
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // Carves the workspace; with base == nullptr only the size is computed.
+// Queue capacities.  A queue entry is a mixture id (a trial id 2 n + start in q_stab_newton), and an id is appended by the
+// one thread that handled that mixture (trial) in the stage before, at most once per queue:
+//   k_init            sends every mixture to exactly one of q_probe / q_stab / q_split                       -> each <= N
+//   k_requeue_failed_hints  moves q_retry (hinted mixtures, which k_init had put in q_split, never in q_probe)
+//                     behind q_probe and empties q_split                                                     -> q_probe <= N
+//   k2_probe          sends every mixture of q_probe to q_stab or q_split (distinct from those already there) -> each <= N
+//   k2_stab_ss        appends each of the 2 |q_stab| trials at most once to q_stab_newton, hard ones from the
+//                     front, easy ones from the back of the same array                                       -> front + back <= 2 N
+//   k_stab_decide     appends a mixture of q_stab at most once to q_split_b                                  -> <= N
+//   k2_split_ss(p)    sends every mixture of split queue p to the front or the back of q_split_newton(p), or
+//                     (p = 0, 1 only) to the crawler queue q_split(p + 2)                                    -> front + back <= N, crawlers <= N
+//   a failed hint     is appended once to q_retry                                                            -> <= N
+// So no append can pass the end of its array.  The queue_push routines do not clamp (the index would cost every append);
+// k_requeue_failed_hints and k_finalize_counters compare the final lengths with these bounds instead -- a check after the
+// fact that raises StageCounters::queue_overflow if the argument above is ever broken by a change to the kernels.
 inline size_t carve_workspace(int nc, int64_t N, char* base, Work* w) {
   size_t off = 0;
   auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align256(bytes); return p; };
@@ -388,8 +403,9 @@ __global__ void __launch_bounds__(128) k_label_only(const __grid_constant__ Io i
 // counters that are simply queue lengths (accumulated over the passes)
 static __global__ void k_finalize_counters(const __grid_constant__ Work w, const long long N) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
-    // every queue holds at most N ids (the stability Newton queue 2 N, filled from both ends): argued in carve_workspace,
-    // verified here after the fact and reported by ptflash_get_stats
+    // every queue holds at most N ids (the stability Newton queue 2 N, filled from both ends): argued above carve_workspace,
+    // compared here with the final lengths (after the fact: an overflow has already written past its array) and reported by
+    // ptflash_get_stats
     bool bad = w.qcount[Q_PROBE] > N || w.qcount[Q_STAB] > N || w.qcount[Q_RETRY] > N ||
                (long long)w.qcount[Q_STAB_NEWTON] + w.qcount[Q_STAB_NEWTON_E] > 2 * N;
 #pragma unroll 1
@@ -407,11 +423,18 @@ static __global__ void k_finalize_counters(const __grid_constant__ Work w, const
 // Warm-start calls of the fast engine: the splits entered through a skip-stability hint run FIRST; the hints that failed
 // (Q_RETRY, reading C21) then join the probe queue of the mixtures without a hint, so the whole call stays one pass.
 // The split queues and tickets restart from zero for the probe- and stability-found splits that follow.
-static __global__ void k_requeue_failed_hints(const __grid_constant__ Work w) {
-  const int cnt = w.qcount[Q_RETRY], base = w.qcount[Q_PROBE];
+static __global__ void k_requeue_failed_hints(const __grid_constant__ Work w, const long long N) {
+  int cnt = w.qcount[Q_RETRY];
+  const int base = w.qcount[Q_PROBE];
+  // the queue lengths of the hinted pass are about to be reset: compare them with their capacities first (the same check
+  // as k_finalize_counters makes for the rest of the call), and never copy past the end of q_probe
+  const bool bad = cnt > N || base > N || (long long)base + cnt > N || w.qcount[Q_SPLIT] > N ||
+                   (long long)w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_E] > N;
+  if (bad) cnt = 0;
   for (int i = threadIdx.x; i < cnt; i += blockDim.x) w.q_probe[base + i] = w.q_retry[i];
   __syncthreads();
   if (threadIdx.x == 0) {
+    if (bad) w.ctr->queue_overflow = 1;
     w.ctr->n_restart += cnt;
     w.ctr->n_split += w.qcount[Q_SPLIT];
     w.ctr->n_split_newton += w.qcount[Q_SPLIT_NEWTON] + w.qcount[Q_SPLIT_NEWTON_E];
