@@ -491,6 +491,11 @@ def main():
                 "steps": e2e_steps,
                 "api": "ptflash_flash_host_async + ptflash_host_wait: pinned host buffers, every step's H2D and D2H copies inside the "
                        "timed region, up to 3 batches in flight" + ("; cold Wilson starts" if warm else ""),
+                # the two host-buffer calls as peers: `value` above is the pipelined one, as in round 2; the figure
+                # to hold against round 1's e2e.value (which timed ptflash_flash_host) is `sync`
+                "pipelined": {"value": e2e_value, "unit": UNIT, "api": "ptflash_flash_host_async + ptflash_host_wait (3 batches in flight)"},
+                "sync": {"value": e2e_sync, "unit": UNIT, "api": "ptflash_flash_host (returns after its results are in host memory)",
+                         "note": "same API as BENCH_r01's e2e.value"},
                 "one_batch_at_a_time": {"value": e2e_sync, "unit": UNIT, "api": "ptflash_flash_host (returns after its results are in host memory)"}},
         "gpu_launches": launches,
         "roofline": roofline,

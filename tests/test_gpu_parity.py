@@ -641,6 +641,61 @@ def test_pipelined_host_call(oracle_mod):
     f.close()
 
 
+def test_host_call_row_by_row_copies():
+    """ptflash_flash_host moves its strided SoA slices with 2D copies, whose pitch is limited to 2^31 - 1 bytes: from
+    N = 2^28 mixtures on it falls back to one copy per component row.  That size does not fit a test; the
+    host_row_copies option takes the same path at an ordinary size.  Both must give the bits of the device-buffer call,
+    also on a chunk boundary that is not a multiple of anything (2 chunks here)."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    N = 70_001
+    w = W.config3(N, offset=123_456)
+    ref = _gpu_flash(w, 1)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    z, P, T = pin(w.z), pin(w.P), pin(w.T)
+    for rows in (1, 0):
+        f = B.PTFlash.from_system(w.system, host_row_copies=rows)
+        assert B.ptflash_get_option(f.h, "host_row_copies") == rows
+        o = dict(beta=torch.full((N,), -7.0, dtype=torch.float64).pin_memory(), x=torch.full((10, N), -7.0, dtype=torch.float64).pin_memory(),
+                 y=torch.full((10, N), -7.0, dtype=torch.float64).pin_memory(), phase=torch.full((N,), -7, dtype=torch.int32).pin_memory(),
+                 iters=torch.full((N,), -7, dtype=torch.int32).pin_memory())
+        B.ptflash_flash_host(f.h, N, z, P, T, o["beta"], o["x"], o["y"], o["phase"], o["iters"])
+        for key in ("beta", "x", "y", "phase", "iters"):
+            assert np.array_equal(o[key].numpy(), ref[key], equal_nan=True), (rows, key)
+        assert f.stats()["n_two_phase"] == int((ref["phase"] == 2).sum())
+        f.close()
+    with pytest.raises(B.PTFlashError):
+        B.PTFlash.from_system(w.system, host_row_copies=2)
+
+
+def test_rachford_rice_leaves_the_flash_statistics_alone():
+    """ptflash_rachford_rice on another stream must not change what ptflash_get_stats waits for and reports:
+    the counters belong to the last flash and to the stream that flash ran on."""
+    import torch
+    from paper_2205_03090_b200 import binding as B
+    dev = torch.device("cuda:0")
+    w = W.config3(200_000)
+    f = B.PTFlash.from_system(w.system)
+    z, P, T = (torch.from_numpy(a).to(dev) for a in (w.z, w.P, w.T))
+    lnK = torch.zeros_like(z)
+    lnK[0] = 1.0
+    lnK[1] = -1.0
+    s_flash, s_rr = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s_flash):
+        out = f.flash(z, P, T)
+    s_flash.synchronize()
+    want = f.stats()
+    with torch.cuda.stream(s_flash):
+        out = f.flash(z, P, T)                      # still running when the Rachford-Rice call below is made ...
+    with torch.cuda.stream(s_rr):
+        rr = f.rachford_rice(lnK, z)                # ... on a stream that finishes long before it
+    got = f.stats()                                 # has to wait for the flash, not for the Rachford-Rice stream
+    assert got == want and got["n_total"] == w.N and got["n_two_phase"] == int((out["phase"] == 2).sum())
+    torch.cuda.synchronize()
+    assert torch.isfinite(rr["theta"]).all()
+    f.close()
+
+
 def test_second_device_keeps_current_device():
     """A handle created on cuda:1 is used and destroyed while cuda:0 is current: the caller's device is
     restored by every entry point and the results equal those of cuda:0."""
@@ -736,9 +791,11 @@ def test_math_routines_against_libm():
 
 
 MAX_ATTRIBUTED_MISSES = 3    # per 10^6 mixtures (configs 2-4): two-phase mixtures above 1e-8, each attributed (see adjudicate)
+MAX_ADJUDICATED_GAP = 1e-6   # ... and none of them further than this from the oracle, whatever the attribution
+ISOFUGACITY_TOL = 2e-9       # max_i |ln f_i^L - ln f_i^V| of a two-phase CUDA result, recomputed in numpy (measured: <= 4.1e-10 over every full-size batch, config 5 included; 1e-9 is asserted of the oracle)
 
 
-def _full_size(oracle_mod, w, g, o, lnK0=None, flags=None, max_misses=MAX_ATTRIBUTED_MISSES, excuse=None):
+def _full_size(oracle_mod, w, g, o, lnK0=None, flags=None, max_misses=MAX_ATTRIBUTED_MISSES, excuse=None, max_gap=MAX_ADJUDICATED_GAP):
     """Invariants on every mixture + element-by-element oracle parity on every mixture (the oracle flashes ~1e6
     mixtures per second on the box's host cores).  Misses above 1e-8 are adjudicated, listed and bounded."""
     N = w.N
@@ -750,6 +807,21 @@ def _full_size(oracle_mod, w, g, o, lnK0=None, flags=None, max_misses=MAX_ATTRIB
     # (1b); worst case is a Newton finish with beta within 1e-5 of 0 or 1 (x = (z - nV)/(1 - beta))
     assert np.abs(g["x"].sum(0) - 1).max() < 1e-9 and np.abs(g["y"].sum(0) - 1).max() < 1e-9
     assert (g["status"] & 3).sum() == 0                                                   # no iteration cap hit
+    # (2) iso-fugacity and the stability verdict on the CUDA results by themselves: ln phi recomputed here in numpy
+    # (tests/srk_check.py, pinned against the oracle on the CPU) -- a check that does not pass through the oracle's
+    # iteration, tolerances or acceptance rules, which were tuned side by side with the kernels
+    import srk_check
+    idx2 = np.nonzero(two)[0]
+    res = np.concatenate([srk_check.isofugacity_residual(w.system, w.P[c], w.T[c], g["x"][:, c], g["y"][:, c])
+                          for c in np.array_split(idx2, max(1, len(idx2) // 200_000))])
+    worst = idx2[np.argsort(res)[-3:]]
+    print(f"  iso-fugacity residual max_i |ln f_i^L - ln f_i^V| of the {len(idx2)} two-phase CUDA results: max {res.max():.3e}, "
+          f"99.99 % below {np.quantile(res, 0.9999):.3e}; worst n = {worst.tolist()}")
+    assert res.max() < ISOFUGACITY_TOL, f"iso-fugacity violated at n = {worst.tolist()}: {np.sort(res)[-3:]}"
+    # a mixture reported single phase has no trial phase with a TPD below the band -- unless the split of an unstable feed
+    # failed and says so (PTFLASH_ST_SPLIT_FAILED); NaN = stability analysis skipped on the caller's word
+    tpd1 = g["tpd_min"][~two & ((g["status"] & 8) == 0)]
+    assert np.all(np.isnan(tpd1) | (tpd1 >= -1e-9))
     rep = compare(w, g, o, excuse=excuse)
     print({k: v for k, v in rep.items() if k not in ("messages", "bad", "band")})
     for n in rep["band"]:
@@ -762,6 +834,12 @@ def _full_size(oracle_mod, w, g, o, lnK0=None, flags=None, max_misses=MAX_ATTRIB
         print("  miss above 1e-8:", r)
     assert all(r["attributed"] != "BUG" for r in rows), "a miss above 1e-8 that neither the oracle's rounding nor conditioning explains"
     assert len(rows) <= max_misses
+    # whatever the attribution, an adjudicated miss stays small in absolute terms.  Not so on config 5, whose
+    # mixtures all sit within 5 % of their phase boundary: there a handful per 1e6 are so ill-conditioned that the double
+    # oracle, the long-double oracle and the CUDA path disagree in the first digits of beta (VERDICT r2, weak point 4: they
+    # need a status bit of their own, which does not exist yet) -- that caller passes max_gap=None and lists them.
+    if max_gap is not None:
+        assert all(r["gap_gpu_oracle"] <= max_gap for r in rows), [r for r in rows if r["gap_gpu_oracle"] > max_gap]
     rep["misses"] = rows
     return rep
 
@@ -793,7 +871,7 @@ def test_full_size_config5_warm_and_cold(oracle_mod):
     g_cold = _gpu_flash(w, 1)
     # every mixture of this workload is within 5 % of its phase boundary, where G is flat: more conditioning-limited misses
     # than in configs 2-4 (each one adjudicated against the long double oracle and listed)
-    rc = _full_size(oracle_mod, w, g_cold, o_cold, max_misses=max(3, int(20e-6 * N)))
+    rc = _full_size(oracle_mod, w, g_cold, o_cold, max_misses=max(3, int(20e-6 * N)), max_gap=None)
     o_restarted = (o_warm["status"] & 64) != 0
     # Which hints fail is a property of the iteration path next to the boundary.  With PTFLASH_OPT_HINT_ETA_SEARCH = 1 the
     # hinted splits take the oracle's restricted step (eta search of B.4a) and the restart sets agree up to borderline
@@ -809,7 +887,7 @@ def test_full_size_config5_warm_and_cold(oracle_mod):
         assert differ.sum() <= bound
         excuse = differ & (g_warm["phase"] != o_warm["phase"])
         assert excuse.sum() <= max(1, 2e-5 * N)
-        rw = _full_size(oracle_mod, w, g_warm, o_warm, lnK0, flags, max_misses=max(3, int(20e-6 * N)), excuse=excuse)
+        rw = _full_size(oracle_mod, w, g_warm, o_warm, lnK0, flags, max_misses=max(3, int(20e-6 * N)), excuse=excuse, max_gap=None)
     assert 0.4 < rc["two_phase"] / N < 0.6
     two = (g_warm["phase"] == 2) & (g_cold["phase"] == 2)
     print("config5 N=%d: two-phase %.3f, restarts gpu %d oracle %d; mean iters (two-phase) warm %.2f cold %.2f" %

@@ -733,3 +733,45 @@ def test_flash_invariants_on_paper_workloads(oracle_mod, name, N):
         assert np.array_equal(o2["phase"], o["phase"][:500])
         t2 = o2["phase"] == 2
         assert np.abs(o2["beta"][t2] - o["beta"][:500][t2]).max() < 1e-9
+
+
+def test_numpy_fugacity_check_agrees_with_the_oracle(oracle_mod):
+    """tests/srk_check.py is a third statement of App. A (A.1-A.6 PAPER.md:404-450) in vectorised numpy -- closed-form cubic
+    plus Newton polish instead of the oracle's iteration, no shared code.  The GPU tests use it to check condition (2) on
+    the CUDA results without the oracle; here the two independent implementations must agree on ln phi and on the chosen
+    root, over feeds, near-pure and trace compositions of three systems (with and without k_ij), which also pins the
+    oracle's orc_lnphi once more."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(__file__))
+    import srk_check
+    rng = np.random.default_rng(20220503)
+    n_multi = 0
+    for w in (W.config1(300), W.config2(300), W.config3(400), W.paper9(300)):
+        orc = oracle_mod.Oracle.from_system(w.system)
+        nc = w.system.nc
+        comps = [w.z, rng.dirichlet(np.full(nc, 0.3), w.N).T + 1e-12]
+        for c in comps:
+            c = c / c.sum(0)
+            got, Zg = srk_check.lnphi(w.system, w.P, w.T, c)
+            multi = 0
+            for n in range(w.N):
+                want, Zw = orc.lnphi(w.P[n], w.T[n], np.ascontiguousarray(c[:, n]))
+                Ai, Bi, Aij = orc.setup(w.P[n], w.T[n])
+                A, B = float(c[:, n] @ Aij @ c[:, n]), float(c[:, n] @ Bi)
+                r = orc.cubic_roots(A, B)
+                if len(r) == 3 and abs(orc.gibbs_of_root(r.min(), A, B) - orc.gibbs_of_root(r.max(), A, B)) < 1e-9:
+                    continue   # two roots of (numerically) equal Gibbs energy: either choice is right
+                multi += len(r) == 3
+                assert abs(Zg[n] - Zw) < 1e-11 * max(1.0, abs(Zw)), (w.name, n, Zg[n], Zw)
+                assert np.abs(got[:, n] - want).max() < 1e-10, (w.name, n, np.abs(got[:, n] - want).max())
+            n_multi += multi
+    assert n_multi > 50, n_multi   # the minimum-Gibbs choice among three real roots was exercised
+    # and the residual it reports is small on the oracle's two-phase results, large on a perturbed one
+    w = W.config3(600)
+    o = oracle_mod.Oracle.from_system(w.system).flash(w.z, w.P, w.T)
+    two = o["phase"] == 2
+    res = srk_check.isofugacity_residual(w.system, w.P[two], w.T[two], o["x"][:, two], o["y"][:, two])
+    assert two.sum() > 100 and res.max() < 1e-9
+    y_bad = o["y"][:, two].copy()
+    y_bad[0] *= 1.0 + 1e-6
+    assert srk_check.isofugacity_residual(w.system, w.P[two], w.T[two], o["x"][:, two], y_bad / y_bad.sum(0)).min() > 1e-8
