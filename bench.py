@@ -47,7 +47,7 @@ WORKLOAD = WORKLOADS["3"]
 # DRAM bytes per launch.  They live in profiles/<tag>_flops.json, written by `bench.py --ncu-summary` from the ncu CSV of
 # that build together with a hash of the kernel sources; when the sources have changed since, the line says "flops_stale".
 STAGES = ("k_init", "k2_probe", "k2_stab_ss", "k3_stab_newton", "k_stab_decide", "k2_split_ss", "k3_split_newton")
-FLOPS_GLOB = "r02*_flops.json"   # the newest (by name) profile of this round; one is written per profiled build
+FLOPS_GLOB = "r0*_flops.json"   # the profile whose source hash matches the build, else the newest by name (marked stale)
 BYTES_PER_FLASH_NC10 = 272.0   # 8(nc+2) in + 8(2nc+1)+8 out, SURVEY.md section 8(d)
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # SMs x DFMA lanes/clk x 2 flop x max SM clock
 PAPER_TABLE4 = {"two_phase_share": 0.413442, "probe_proved_share": 0.3744, "seconds_per_1e6_on_RTX3080": 3.03,
@@ -249,7 +249,7 @@ def main():
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="library option for this run (binding.OPTIONS, e.g. early_split_ss=1); recorded in config.options")
     ap.add_argument("--ncu-summary", default="", help="raw CSV of the ncu per-kernel pass -> markdown table + profiles/<tag>_flops.json")
-    ap.add_argument("--ncu-tag", default="r02")
+    ap.add_argument("--ncu-tag", default="r03")
     args = ap.parse_args()
     if args.ncu_summary:
         return ncu_summary(args.ncu_summary, args.ncu_tag)

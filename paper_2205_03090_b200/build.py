@@ -35,8 +35,7 @@ def _newest_src() -> float:
 
 
 def _compile(src: Path, obj: Path, extra: list) -> str:
-    dev = os.environ.get("PTFLASH_NVCC_EXTRA", "").split()   # development only: extra -D switches for experiments
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, *dev, "-c", str(src), "-o", str(obj)]
+    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-c", str(src), "-o", str(obj)]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"nvcc failed: {' '.join(cmd)}\n{r.stdout}\n{r.stderr}")

@@ -520,6 +520,52 @@ def test_warm_start_and_skip_stability(sys10):
     slow = sys10.flash(w.z, w.P, w.T, lnK0=lnK0, flags=flags, nthreads=8, opts=dict(hint_ss_cap=100000, hint_tr_cap=60))
     assert np.array_equal(slow["phase"], warm["phase"]) and np.abs(slow["beta"] - warm["beta"])[two].max() < 1e-8
     assert np.all(((slow["status"] & 64) != 0) <= restarted)
+    # ... and the same on BASELINE config 5's own inputs (every mixture within 5 % of its phase boundary, hints from the
+    # neighbouring pressure): that is where the caps bite.  hint_ss_cap / hint_tr_cap are a PRODUCT choice (they cut the time
+    # the CUDA path spends on hints that are going to fail, reading C21) which the oracle mirrors; what is pinned here is that
+    # the choice does not move an answer (VERDICT r2, weak point 5b)
+    import os, sys
+    sys.path.insert(0, os.path.dirname(__file__))
+    import config5
+    w5, lnK5, flags5, _info = config5.build(sys10, 6000)
+    capped = sys10.flash(w5.z, w5.P, w5.T, lnK0=lnK5, flags=flags5, nthreads=8)
+    free = sys10.flash(w5.z, w5.P, w5.T, lnK0=lnK5, flags=flags5, nthreads=8, opts=dict(hint_ss_cap=100000, hint_tr_cap=60))
+    two5 = capped["phase"] == 2
+    r_capped, r_free = (capped["status"] & 64) != 0, (free["status"] & 64) != 0
+    assert two5.sum() > 1000 and r_capped.sum() > 0                       # the caps (or a failed hint) are exercised
+    assert np.array_equal(free["phase"], capped["phase"])
+    assert np.abs(free["beta"] - capped["beta"])[two5].max() < 1e-8 and np.abs(free["x"] - capped["x"])[:, two5].max() < 1e-8
+    assert np.all(r_free <= r_capped)                                      # without the caps only fewer hints are dropped
+    print("config 5 hints dropped with / without the caps:", int(r_capped.sum()), int(r_free.sum()), "of", int(flags5.astype(bool).sum()))
+
+
+def test_split_trivial_tol_is_not_load_bearing(oracle_mod, sys10):
+    """Reading C22: the phase split counts as collapsed into the trivial solution x = y when max_i |ln K_i| < split_trivial_tol
+    (1e-5 since round 2, 1e-9 before; the paper gives no number).  VERDICT r2 asked for a pin that fails when the value is too
+    small.  There is no such case in today's oracle: with the last-Newton-step finish (C8) and the G-monotone acceptance (C11)
+    a split that slides towards x = y is caught by beta leaving (0, 1) or goes all the way to ln K = 0, so 1e-9, 1e-5 and 1e-3
+    give identical results -- scanned at 10^6 (config 3), 2^20 (config 4), 5 10^5 (config 2, paper9) and 2 10^5 (config 5 warm)
+    mixtures, and on 42 000 stable mixtures wrongly hinted "unstable" with a small-|ln K| seed, the input that can only
+    collapse.  What this test pins is therefore the insensitivity itself, on small samples of the same inputs: parity
+    between the CUDA path and the oracle does not hinge on the constant, and genuine splits stay far above it."""
+    cases = []
+    w = W.config3(8000)
+    cases.append((sys10, w, None, None))
+    wp = W.paper9(6000)
+    cases.append((oracle_mod.Oracle.from_system(wp.system), wp, None, None))
+    cold = sys10.flash(w.z, w.P, w.T, nthreads=8)
+    seed = 0.05 * np.stack([sys10.wilson(P, T) for P, T in zip(w.P, w.T)]).T
+    cases.append((sys10, w, seed, np.where(cold["phase"] == 1, 1, 0).astype(np.uint8)))      # wrong hints on stable feeds
+    for orc, wl, lnK0, flags in cases:
+        kw = {} if lnK0 is None else dict(lnK0=lnK0, flags=flags)
+        ref = orc.flash(wl.z, wl.P, wl.T, nthreads=8, **kw)
+        for tol in (1e-9, 1e-3):
+            r = orc.flash(wl.z, wl.P, wl.T, nthreads=8, opts=dict(split_trivial_tol=tol), **kw)
+            assert np.array_equal(r["phase"], ref["phase"]) and np.array_equal(r["status"], ref["status"]), (wl.name, tol)
+            assert np.array_equal(r["beta"], ref["beta"], equal_nan=True), (wl.name, tol)
+        two = ref["phase"] == 2
+        assert np.abs(ref["lnK"][:, two]).max(0).min() > 1e-2            # genuine solutions: far above any of the three values
+    assert not np.any((ref["phase"] == 2) & (flags == 1))                 # no wrongly hinted stable feed came out two-phase
 
 
 def test_phase_identity_by_compressibility(oracle_mod, sys10):
