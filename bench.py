@@ -238,7 +238,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--n", type=int, default=1_000_000, help="mixtures per GPU per step")
+    ap.add_argument("--n", "--mixtures", dest="n", type=int, default=1_000_000,
+                    help="mixtures per GPU per step (under torchrun use --mixtures: its own parser claims the prefix --n)")
     ap.add_argument("--engine", type=int, default=1)
     ap.add_argument("--config", default="3", choices=sorted(WORKLOADS),
                     help="workload to time (3 = the headline: BASELINE.json configs[2]; the others report throughput only: "
@@ -268,9 +269,17 @@ def main():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
+    # the process group exists whenever a launcher set one up (torchrun exports MASTER_PORT), also for a single rank: the same
+    # NCCL init, barrier and max-over-ranks reduction then run at N = 1 as at N = 8, so that path is exercised on a 1-GPU box
+    use_dist = world > 1 or ("MASTER_PORT" in os.environ and "RANK" in os.environ)
+    if use_dist:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+        try:
+            dist.init_process_group("nccl", device_id=dev)
+        except Exception:
+            if world > 1:
+                raise
+            use_dist = False      # a single rank needs no group: leftover MASTER_* variables must not stop the N = 1 run
 
     N = args.n
     headline = args.config == "3"
@@ -299,7 +308,7 @@ def main():
             B.ptflash_flash(f.h, N, z, P, T, out["beta"], out["x"], out["y"], out["phase"], out["iters"])
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -346,7 +355,7 @@ def main():
         if acc and len(acc[0]) == len(STAGES):
             stage_ms = [float(np.mean([a[i] for a in acc])) for i in range(len(STAGES))]
     t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
+    if use_dist:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_total = float(t.item())
     ms_step = ms_total / args.steps
@@ -404,7 +413,7 @@ def main():
         B.ptflash_host_wait(f.h)      # the last results have landed in host memory
         barrier()
         te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if world > 1:
+        if use_dist:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         return world * N * steps / float(te.item())
 
@@ -418,7 +427,7 @@ def main():
             assert int((o["ph"] == 2).sum()) == n_two
 
     if rank != 0:
-        if world > 1:
+        if use_dist:
             dist.destroy_process_group()
         return
 
@@ -506,7 +515,7 @@ def main():
         os.remove(clk_path)
     except OSError:
         pass
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
 
 

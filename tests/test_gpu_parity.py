@@ -722,6 +722,32 @@ def test_second_device_keeps_current_device():
     assert torch.cuda.current_device() == 0
 
 
+@pytest.mark.parametrize("nproc", [1, 2])
+def test_bench_under_torchrun(nproc, tmp_path):
+    """bench.py launched the way the driver launches it for N > 1 (its NCCL init, per-rank shard offsets and
+    max-over-ranks timing had never run anywhere).  With one process the same code path runs on a 1-GPU box (the group is
+    created whenever torchrun set one up); with two it needs two GPUs.  Rank 0 prints ONE JSON line; the job-wide value
+    is ranks x N x steps / max-over-ranks time, so two ranks on two GPUs must land near twice the one-rank figure."""
+    import json, subprocess, sys, torch
+    if torch.cuda.device_count() < nproc:
+        pytest.skip(f"needs {nproc} GPUs")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    n = 200_000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={nproc}", "--master-addr", "127.0.0.1",
+           "--master-port", str(29500 + 17 * nproc + os.getpid() % 400), os.path.join(root, "bench.py"), "--gpus", str(nproc),
+           "--steps", "3", "--warmup", "3", "--no-cpu-baseline", "--mixtures", str(n)]
+    r = subprocess.run(cmd, capture_output=True, text=True, cwd=root, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout[-2000:]                      # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == nproc and d["steps"] == 3 and d["scaling"] == "weak" and d["config"]["mixtures_per_step"] == n
+    assert d["gpu_launches"] > 0 and d["roofline"]["frac"] > 0.05 and d["e2e"]["value"] > 0
+    # whole-job throughput: ranks x n mixtures per step over the slowest rank's time
+    assert abs(d["value"] - nproc * n / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
+    print(f"torchrun x{nproc}: {d['value'] / 1e6:.1f} M flashes/s, {d['ms_per_step']:.3f} ms per step of {n} mixtures per rank")
+
+
 def _ulps(y, ref):
     """|y - ref| in units of the spacing of doubles at ref (ref: numpy longdouble)."""
     r64 = ref.astype(np.float64)
