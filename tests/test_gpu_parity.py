@@ -592,7 +592,9 @@ def test_parity_paper_workloads(oracle_mod, name, N):
     """NEXT-3: the paper's own case studies (Tables 1-3; P in MPa), element by element against the oracle."""
     w = W.CONFIGS[name](N)
     o = oracle_mod.Oracle.from_system(w.system).flash(w.z, w.P, w.T)
-    for engine in (1, 0):
+    # engine 1 only at these sizes: engine 0 follows the oracle's statement order (DESIGN section 5), so agreeing with it is
+    # not independent evidence; it stays in the small parity tests (VERDICT r2, item 9)
+    for engine in (1,):
         g = _gpu_flash(w, engine)
         rep = compare(w, g, o)
         rows = adjudicate(oracle_mod, w, g, o, rep["bad"])
